@@ -1,0 +1,125 @@
+"""Integer model of the routing table / slot allocator / append positions -- TEST INFRASTRUCTURE.
+
+Follows PAPER.md:159-161 (routing table maps a request's token ranges to attention-node endpoints,
+historical owners + live tail), :149 and :240 (route updates are published only at token boundaries;
+existing ranges stay in place; future appends go to the new node), :173 (Fig. 5: [0,T/2)->A0,
+[T/2,T)->A1, then [T,..)->A2 appended with nothing else changing), :145 (tail appends K/V_new before
+attending).  Where the paper is silent the readings of DESIGN.md apply:
+
+  reading 7: fixed R tokens per range, range j = [jR, (j+1)R)
+  reading 8: at the boundary BEFORE appending, a request with len % R == 0 opens range len / R
+  reading 9: one global round-robin cursor: the k-th range ever allocated goes to partition k % P;
+             allocation order = ranges ascending within a request; requests ascending at a boundary;
+             slot = per-partition LIFO free list if non-empty, else bump allocator free_head[p]++
+  reading 10: exhaustion (slot >= slots_per_partition, or range index >= max_ranges) -> error ENOSPC
+
+Pure Python, no numpy: written to be checked against the text by eye.
+"""
+from __future__ import annotations
+
+from typing import Dict, List, Optional, Tuple
+
+
+class RoutingError(Exception):
+    pass
+
+
+class RoutingModel:
+    def __init__(self, n_partitions: int, range_tokens: int, max_requests: int,
+                 max_ranges_per_request: int, slots_per_partition: int):
+        self.P = n_partitions
+        self.R = range_tokens
+        self.B = max_requests
+        self.Jmax = max_ranges_per_request
+        self.slots = slots_per_partition
+        self.len: List[int] = [-1] * max_requests          # -1 = request closed
+        self.route: List[List[Tuple[int, int]]] = [[] for _ in range(max_requests)]
+        self.rr_cursor = 0
+        self.free_head = [0] * n_partitions                 # bump allocator
+        self.free_list: List[List[int]] = [[] for _ in range(n_partitions)]  # LIFO of released slots
+
+    # -- allocation -----------------------------------------------------------------------------
+    def _alloc(self, req: int) -> Tuple[int, int]:
+        if len(self.route[req]) >= self.Jmax:
+            raise RoutingError("ENOSPC: max_ranges_per_request")
+        p = self.rr_cursor % self.P
+        if self.free_list[p]:
+            slot = self.free_list[p][-1]
+        else:
+            slot = self.free_head[p]
+            if slot >= self.slots:
+                raise RoutingError("ENOSPC: partition full")
+        # commit
+        self.rr_cursor += 1
+        if self.free_list[p]:
+            self.free_list[p].pop()
+        else:
+            self.free_head[p] += 1
+        self.route[req].append((p, slot))
+        return p, slot
+
+    # -- API mirror -----------------------------------------------------------------------------
+    def open_request(self, req: int, n_tokens: int) -> None:
+        """Post-prefill initialisation: ceil(n/R) ranges, round-robin."""
+        if self.len[req] >= 0:
+            raise RoutingError("ESTATE: request already open")
+        if n_tokens < 0:
+            raise RoutingError("EINVAL")
+        self.len[req] = n_tokens
+        for _ in range(-(-n_tokens // self.R)):
+            self._alloc(req)
+
+    def token_boundary(self) -> List[Tuple[int, int, int, int]]:
+        """Open a new range for every open request whose tail range is full (reading 8).
+        Returns the events [(req, range_index, partition, slot)]."""
+        events = []
+        for r in range(self.B):
+            if self.len[r] < 0:
+                continue
+            if self.len[r] % self.R == 0 and len(self.route[r]) == self.len[r] // self.R:
+                p, s = self._alloc(r)
+                events.append((r, len(self.route[r]) - 1, p, s))
+        return events
+
+    def append_position(self, req: int) -> Tuple[int, int, int]:
+        """(partition, slot, token offset inside the range) where this step's K/V_new is written."""
+        n = self.len[req]
+        if n < 0:
+            raise RoutingError("ESTATE: closed request")
+        j = n // self.R
+        if j >= len(self.route[req]):
+            raise RoutingError("ESTATE: no route for the tail position (token_boundary not called)")
+        p, s = self.route[req][j]
+        return p, s, n - j * self.R
+
+    def step_commit(self) -> None:
+        for r in range(self.B):
+            if self.len[r] >= 0:
+                self.len[r] += 1
+
+    def close_request(self, req: int) -> None:
+        if self.len[req] < 0:
+            raise RoutingError("ESTATE: request not open")
+        for (p, s) in self.route[req]:       # ascending j
+            self.free_list[p].append(s)
+        self.route[req] = []
+        self.len[req] = -1
+
+    # -- inspection -----------------------------------------------------------------------------
+    def n_ranges(self, req: int) -> int:
+        return len(self.route[req])
+
+    def locate(self, req: int, pos: int) -> Tuple[int, int, int]:
+        """(partition, slot, offset) of logical token ``pos`` of a request."""
+        j = pos // self.R
+        p, s = self.route[req][j]
+        return p, s, pos - j * self.R
+
+    def snapshot(self) -> Dict[str, object]:
+        part = [[-1] * self.Jmax for _ in range(self.B)]
+        slot = [[-1] * self.Jmax for _ in range(self.B)]
+        for r in range(self.B):
+            for j, (p, s) in enumerate(self.route[r]):
+                part[r][j], slot[r][j] = p, s
+        return {"len": list(self.len), "n_ranges": [len(x) for x in self.route], "part": part,
+                "slot": slot, "free_head": list(self.free_head), "rr_cursor": self.rr_cursor}

@@ -1,0 +1,143 @@
+"""Pins for oracle/routing.py (integer routing / slot / append-position model)."""
+import pytest
+
+from oracle.routing import RoutingError, RoutingModel
+from kf_inputs import workloads
+from conftest import load_golden
+
+
+def test_fig5_scenario():
+    # [0,T/2)->A0, [T/2,T)->A1; when the context grows beyond T a new entry
+    # [T,...)->A2 is appended without modifying anything else.
+    T = 16
+    m = RoutingModel(n_partitions=3, range_tokens=T // 2, max_requests=1, max_ranges_per_request=4,
+                     slots_per_partition=2)
+    m.open_request(0, T)
+    assert m.route[0] == [(0, 0), (1, 0)]
+    before = list(m.route[0])
+    ev = m.token_boundary()
+    assert ev == [(0, 2, 2, 0)]
+    assert m.route[0][:2] == before and m.route[0][2] == (2, 0)
+    assert m.append_position(0) == (2, 0, 0)
+
+
+def test_closed_form_at_load():
+    # range number n = sum_{r'<r} J_r' + j  ->  (n mod P, n div P)
+    P, R = 5, 8
+    lens = [3, 8, 9, 40, 1, 17, 64]
+    m = RoutingModel(P, R, len(lens), 8, 10)
+    for r, n in enumerate(lens):
+        m.open_request(r, n)
+    n = 0
+    for r, L in enumerate(lens):
+        J = -(-L // R)
+        assert m.n_ranges(r) == J
+        for j in range(J):
+            assert m.route[r][j] == (n % P, n // P)
+            n += 1
+    assert m.rr_cursor == n and sum(m.free_head) == n
+
+
+def test_tiny_scenario_appendix_c():
+    g = load_golden("appendix_c_routing.json")["tiny"]
+    m = RoutingModel(g["P"], g["R"], 3, 8, 8)
+    for r, n in enumerate(g["load_lens"]):
+        m.open_request(r, n)
+    assert [[list(x) for x in m.route[r]] for r in range(3)] == g["after_load"]["routes"]
+    assert m.free_head == g["after_load"]["free_head"] and m.rr_cursor == g["after_load"]["cursor"]
+    for st in g["steps"]:
+        ev = m.token_boundary()
+        assert [[r, p, s] for (r, _, p, s) in ev] == st["opens"]
+        assert [list(m.append_position(r)) for r in range(3)] == st["append"]
+        m.step_commit()
+        assert m.len == st["lens_after"]
+        assert m.free_head == st["free_head"] and m.rr_cursor == st["cursor"]
+
+
+def test_invariants_random_walk():
+    import random
+    rnd = random.Random(5)
+    P, R, B = 3, 4, 6
+    m = RoutingModel(P, R, B, 16, 64)
+    for r in range(B):
+        m.open_request(r, rnd.randrange(0, 20))
+    seen = {}
+    for step in range(40):
+        prev = [list(x) for x in m.route]
+        prev_fh = list(m.free_head)
+        m.token_boundary()
+        for r in range(B):
+            assert m.route[r][:len(prev[r])] == prev[r]          # entries never change once written
+            p, s, off = m.append_position(r)
+            assert 0 <= off < R and (p, s) == m.route[r][-1]     # appends go to the tail range only
+            assert off == m.len[r] - (len(m.route[r]) - 1) * R
+        assert all(a >= b for a, b in zip(m.free_head, prev_fh))  # monotone
+        used = [ps for r in range(B) for ps in m.route[r]]
+        assert len(used) == len(set(used))                         # no (p, slot) used twice
+        assert sum(m.free_head) == sum(len(x) for x in m.route) == m.rr_cursor
+        m.step_commit()
+
+
+def test_cfg3_load():
+    g = load_golden("appendix_c_routing.json")["cfg3"]
+    w = workloads.cfg3()
+    m = RoutingModel(w.n_partitions, w.range_tokens, w.batch, 8, 8)
+    for r, S in enumerate(w.contexts):
+        m.open_request(r, S - 1)      # S-1 resident, the S-th arrives at step 0 (SURVEY 8(d) state prep)
+    m.token_boundary()
+    assert m.free_head == g["slots_after_load"]
+    assert [list(x) for x in m.route[2]] == g["request2_route"]
+    assert sum(len(x) for x in m.route) == g["total_ranges"]
+
+
+def test_cfg5_events():
+    g = load_golden("appendix_c_routing.json")["cfg5"]
+    w = workloads.cfg5()
+    lens0 = w.extra["len_before_step0"]
+    m = RoutingModel(w.n_partitions, w.range_tokens, w.batch, 9, 40)
+    for r, n in enumerate(lens0):
+        m.open_request(r, n)
+    assert m.free_head == g["free_head_after_load"] and m.rr_cursor == g["ranges_at_load"]
+    events = []
+    for step in range(64):
+        for (r, j, p, s) in m.token_boundary():
+            events.append((step, r))
+        m.step_commit()
+    assert events == [(4 * i, 8 * i) for i in range(16)]
+    assert m.free_head == g["free_head_final"] and m.rr_cursor == g["cursor_final"]
+    assert [list(x) for x in m.route[0]] == g["request0_final_route"]
+    assert [list(x) for x in m.route[120]] == g["request120_final_route"]
+
+
+def test_close_and_lifo_reuse():
+    m = RoutingModel(2, 4, 3, 4, 4)
+    m.open_request(0, 8)   # (0,0),(1,0)
+    m.open_request(1, 4)   # (0,1)
+    m.close_request(0)     # free lists: p0:[0], p1:[0]
+    assert m.len[0] == -1 and m.route[0] == []
+    m.open_request(2, 8)   # cursor=3 -> p1 reuse slot 0 ; cursor=4 -> p0 reuse slot 0
+    assert m.route[2] == [(1, 0), (0, 0)]
+    assert m.free_head == [2, 1]
+    with pytest.raises(RoutingError):
+        m.open_request(1, 4)
+    with pytest.raises(RoutingError):
+        m.close_request(0)
+
+
+def test_enospc():
+    m = RoutingModel(1, 4, 1, 8, 2)
+    m.open_request(0, 8)
+    with pytest.raises(RoutingError):
+        m.token_boundary()
+    m2 = RoutingModel(2, 4, 1, 2, 8)
+    m2.open_request(0, 8)
+    with pytest.raises(RoutingError):
+        m2.token_boundary()
+
+
+def test_kv_byte_formula():
+    # PAPER.md:234 C_total = sum_i 2*s_i*H_kv*d_h*L*2B; PAPER.md:35 sanity: Llama-3.1-8B, batch 64 x 4K
+    # tokens = 32 GiB (128 KiB/token over 32 layers)
+    per_token = 2 * 8 * 128 * 32 * 2
+    assert per_token == 128 * 1024
+    assert 64 * 4096 * per_token == 32 * 2 ** 30
