@@ -1,0 +1,186 @@
+/*
+ * kflume.h -- C ABI of libkflume: KernelFlume's data-parallel hot path on one B200 (sm_100a).
+ *
+ * What the library computes (arxiv/paper_2606_29207, text in PAPER.md):
+ *   a decode query for one new token runs GQA attention over each token-range KV partition that a
+ *   routing table assigns to a (here: emulated) weightless attention node; every range emits a partial
+ *   output and its log-sum-exp; the partials are merged into the exact softmax result
+ *   (PAPER.md:137, :143-147, :254).  A KV-append / route-update step feeds it: the new token's K/V
+ *   is appended to the request's tail range, and a new range is opened -- the routing table extended --
+ *   at the token boundary where the tail range is full.
+ *
+ * Conventions
+ *   - Plain C, no CUDA or torch types.  A `kf_stream` is a `cudaStream_t` cast to `void*` (NULL = the
+ *     legacy default stream).  Pointers are marked [device] or [host].
+ *   - fp16 tensors are passed as `const void*` to IEEE binary16 data.
+ *   - Every call returns an int: KF_OK (0) or a negative KF_E* code.  No exceptions, no aborts, nothing
+ *     is printed.  Errors found ON THE DEVICE (capacity, state) are latched in a device error word and
+ *     surfaced by kf_status() / kf_route_snapshot(); the launch that found them skips the faulty item.
+ *   - OWNERSHIP: the caller owns all device memory (KV pools, workspace, q/k/v/o buffers) and all
+ *     streams for the lifetime of the ctx.  The library owns only the host-side `kf_ctx`.  Hot calls
+ *     (token_boundary, kv_append, partial_attend, merge_partials, attend, step_commit) are asynchronous
+ *     on the caller's stream, never synchronise, never allocate, launch fixed grids and read all variable
+ *     state (lengths, routes, work plan) from device memory -- so a CUDA Graph captured around them stays
+ *     valid across route updates (the single-GPU analogue of PAPER.md:165-179, requirement R1 at :127).
+ *   - There is NO CPU fallback: without a CUDA device kf_create() returns KF_ECUDA.
+ *
+ * Notation: B = max_requests, H_q / H_kv = query / KV heads, G = H_q / H_kv, d = head_dim = 128,
+ *   R = range_tokens, P = n_partitions, Jmax = max_ranges_per_request, L = n_layers (physical).
+ *   len_r = tokens of request r committed so far; a decode step attends over len_r + 1 tokens (the token
+ *   appended in this step included: the tail node "appends, then computes attention").
+ *
+ * KV pool layout (one pool per partition = per emulated attention node; fp16):
+ *   K element (p, layer, slot, g, t, i) lives at byte
+ *       pool[p] + ((((layer*slots_per_partition + slot)*H_kv + g)*R + t)*128 + i)*2
+ *   and the V element at the same offset + kf_pool_bytes()/2.  A slot holds one token range of one
+ *   request for all physical layers ("[range][kv_head][token][128]" innermost order).
+ */
+#ifndef KFLUME_H
+#define KFLUME_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KF_VERSION 100 /* 0.1.0 */
+
+#define KF_OK 0
+#define KF_EINVAL (-1) /* bad argument / shape / alignment / null pointer */
+#define KF_ESTATE (-2) /* call not valid in this state (request closed/already open, no route for the tail) */
+#define KF_ENOSPC (-3) /* no free slot in the round-robin partition, or Jmax ranges exceeded (device-detected) */
+#define KF_ECUDA (-4)  /* a CUDA runtime/driver call failed (kf_last_cuda_error() has the text) */
+
+#define KF_IMPL_AUTO 0   /* fastest available attend kernel (TMA + tensor-core path) */
+#define KF_IMPL_SIMPLE 1 /* CUDA-core reference kernel (coalesced 128-bit loads, warp shuffles) */
+#define KF_IMPL_TMA 2    /* TMA-staged, mma.sync tensor-core kernel */
+
+typedef void *kf_stream;
+
+typedef struct kf_config {
+    int32_t n_q_heads;              /* H_q                                                        */
+    int32_t n_kv_heads;             /* H_kv; H_q % H_kv == 0 and G = H_q/H_kv in 1..8             */
+    int32_t head_dim;               /* must be 128                                                */
+    int32_t n_layers;               /* physical layer pools L >= 1                                */
+    int32_t range_tokens;           /* R, a power of two >= 1                                     */
+    int32_t n_partitions;           /* P in 1..64: emulated attention nodes        */
+    int32_t max_requests;           /* B in 1..4096                                               */
+    int32_t max_ranges_per_request; /* Jmax >= 1                                                  */
+    int32_t slots_per_partition;    /* token-range slots in each partition pool                   */
+    float softmax_scale;            /* 0 => 1/sqrt(head_dim); scores are scale * q.k              */
+    int32_t attend_impl;            /* KF_IMPL_*                                                  */
+    int32_t min_tiles_per_worker;   /* 0 => default; work-split granularity hint (16-token tiles)  */
+    int32_t reserved[4];            /* must be 0                                                  */
+} kf_config;
+
+typedef struct kf_ctx kf_ctx;
+
+/* ---- library ------------------------------------------------------------------------------------ */
+int kf_version(void);
+const char *kf_strerror(int code);
+/* Text of the last CUDA error seen by this ctx ("" if none).  [host] string owned by the ctx. */
+const char *kf_last_cuda_error(const kf_ctx *ctx);
+
+/* ---- sizes (pure host arithmetic, no GPU needed) --------------------------------------------------
+ * kf_pool_bytes: bytes of ONE partition pool (K + V, all physical layers) =
+ *   2 * L * slots_per_partition * H_kv * R * 128 * 2   (per-layer bytes per token 2*H_kv*d*2B).
+ * kf_workspace_bytes: bytes of the device workspace (routing table, work plan, partial buffers, staging).
+ * Both return 0 for an invalid config. */
+size_t kf_pool_bytes(const kf_config *cfg);
+size_t kf_workspace_bytes(const kf_config *cfg);
+/* Byte offset inside a partition pool of element (layer, slot, kv_head, token, 0) of K (is_v=0) or V (is_v=1).
+ * Returns (size_t)-1 on bad arguments. */
+size_t kf_pool_offset(const kf_config *cfg, int32_t layer, int32_t slot, int32_t kv_head, int32_t token,
+                      int32_t is_v);
+
+/* ---- lifetime ------------------------------------------------------------------------------------
+ * pool_ptrs: [host] array of P [device] pointers, each kf_pool_bytes() long, 1024-byte aligned.
+ * workspace: [device], kf_workspace_bytes() long, 256-byte aligned; zero-initialised by kf_create.
+ * Uses the current CUDA device.  All requests start closed; the routing table is empty. */
+int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *workspace,
+              size_t workspace_bytes);
+int kf_destroy(kf_ctx *ctx);
+
+/* ---- routing table --------------------------------------------------------------
+ * kf_open_request: "post-prefill initialisation": marks request `req` open with
+ *   len = n_tokens and allocates ceil(n_tokens/R) ranges j = 0.. in order.  The k-th range ever allocated
+ *   goes to partition k mod P (one global round-robin cursor); the slot comes from that partition's LIFO
+ *   free list if non-empty, else from its bump allocator.  Routes are layer-independent: an attention
+ *   node holds all L layers of a range.  Device errors: ESTATE (already open), ENOSPC.
+ * kf_close_request: returns the request's slots to the free lists (ascending j) and marks it closed. */
+int kf_open_request(kf_ctx *ctx, int32_t req, int32_t n_tokens, kf_stream stream);
+int kf_close_request(kf_ctx *ctx, int32_t req, kf_stream stream);
+
+/* kf_load_context: copies tokens [tok_begin, tok_begin + n_tokens) of request `req`, layer `layer`, into the
+ * routed slots.  k, v: [device] fp16 [H_kv][n_tokens][128].  Every position must already have a route
+ * (position < n_ranges*R), else device error ESTATE.  Does not change len. */
+int kf_load_context(kf_ctx *ctx, int32_t layer, int32_t req, int32_t tok_begin, int32_t n_tokens,
+                    const void *k, const void *v, kf_stream stream);
+
+/* ---- the decode step -----------------------------------------------------------------------------
+ * (a1) kf_token_boundary -- route update at the token boundary (Fig. 5 at :173).
+ *   For every open request, ascending, whose tail range is full (len % R == 0 and no range len/R yet):
+ *   allocate (partition, slot) as above and APPEND the route entry; earlier entries never change.  Then
+ *   rebuilds the device-side work plan for a step over len+1 tokens.  Call once per decode step, before
+ *   the per-layer calls.  Device errors: ENOSPC. */
+int kf_token_boundary(kf_ctx *ctx, kf_stream stream);
+
+/* (a2) kf_kv_append -- the tail node appends (K_new, V_new).
+ *   k_new, v_new: [device] fp16 [B][H_kv][128]; row r is written at token offset len_r - j*R of range
+ *   j = len_r / R of open request r (rows of closed requests are ignored).  Does NOT advance len (all
+ *   layers of a step append at the same position).  Device error ESTATE if that range has no route. */
+int kf_kv_append(kf_ctx *ctx, int32_t layer, const void *k_new, const void *v_new, kf_stream stream);
+
+/* (a3) kf_partial_attend -- local core attention per token range:
+ *   for every open request r, range j < J_r = ceil((len_r+1)/R) whose partition is selected, and query
+ *   head h (KV head h / G):  s_t = scale * q_h . K_t over the range's tokens,
+ *       lse_part[r][j][h] = ln sum_t exp(s_t),   o_part[r][j][h][:] = sum_t exp(s_t - lse) V_t.
+ *   q: [device] fp16 [B][H_q][128].  partition_mask: [host] uint8 [P] (non-zero = selected) or NULL = all.
+ *   o_part: [device] fp32 [B][Jmax][H_q][128];  lse_part: [device] fp32 [B][Jmax][H_q].
+ *   Rows of unselected / non-existent ranges are left untouched. */
+int kf_partial_attend(kf_ctx *ctx, int32_t layer, const void *q, const uint8_t *partition_mask, float *o_part,
+                      float *lse_part, kf_stream stream);
+
+/* (a4) kf_merge_partials -- online-softmax (log-sum-exp) reduction of the partials:
+ *   lse[r][h] = ln sum_j exp(lse_part[r][j][h]);  o[r][h] = sum_j exp(lse_part[r][j][h] - lse[r][h]) o_part[r][j][h]
+ *   over j < J_r.  J_r == 1 is an exact copy; a partial with lse = -inf has weight 0.
+ *   o: [device] fp32 [B][H_q][128]; lse: [device] fp32 [B][H_q].  Rows of closed requests untouched. */
+int kf_merge_partials(kf_ctx *ctx, const float *o_part, const float *lse_part, float *o, float *lse,
+                      kf_stream stream);
+
+/* (a3+a4) kf_attend -- both in ONE launch: the merge is fused into the tail of the attend kernel (the last
+ *   work item to finish a range / a request performs the reduction, in a fixed order, so results are
+ *   run-to-run identical and equal to the unfused path).  o_part / lse_part may be NULL (internal scratch). */
+int kf_attend(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, float *o_part, float *lse_part,
+              kf_stream stream);
+
+/* (a5) kf_step_commit -- len_r += 1 for every open request (the step boundary). */
+int kf_step_commit(kf_ctx *ctx, kf_stream stream);
+
+/* One layer-step with HOST buffers (end-to-end path): copies q / k_new / v_new [host, fp16, shapes as above]
+ * to device staging, runs kf_kv_append + kf_attend, copies o [B][H_q][128] and lse [B][H_q] (fp32) back to
+ * [host].  Asynchronous on `stream` (use pinned host memory); the caller synchronises the stream. */
+int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host,
+                       const void *v_new_host, float *o_host, float *lse_host, kf_stream stream);
+
+/* ---- inspection (tests, tools) -------------------------------------------------------------------
+ * kf_route_snapshot: downloads the routing state into [host] arrays (any may be NULL):
+ *   len[B] (-1 = closed), n_ranges[B], part[B][Jmax], slot[B][Jmax] (-1 where unused), free_head[P],
+ *   rr_cursor[1].  Synchronises `stream`.
+ * kf_status: synchronises `stream`, returns the device error word (KF_OK or the FIRST latched KF_E*) and
+ *   clears it.
+ * kf_plan_info: downloads the work-plan header into out[8] [host]: {n_units, n_tiles, n_workers_active,
+ *   n_pieces, n_range_entries, tile_tokens, max_workers, 0}.  Synchronises `stream`.
+ * kf_launch_count: number of CUDA kernels this ctx has launched so far (host-side counter). */
+int kf_route_snapshot(kf_ctx *ctx, int32_t *len, int32_t *n_ranges, int32_t *part, int32_t *slot,
+                      int32_t *free_head, int32_t *rr_cursor, kf_stream stream);
+int kf_status(kf_ctx *ctx, kf_stream stream);
+int kf_plan_info(kf_ctx *ctx, int32_t *out, kf_stream stream);
+int64_t kf_launch_count(const kf_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KFLUME_H */

@@ -40,6 +40,12 @@
 #include <omp.h>
 #endif
 
+/* POW2_M25[e] = 2^(e-25) for the biased binary16 exponent e = 1..30 (entries 0 and 31 unused). */
+static const double POW2_M25[32] = {
+    0.0,     0x1p-24, 0x1p-23, 0x1p-22, 0x1p-21, 0x1p-20, 0x1p-19, 0x1p-18, 0x1p-17, 0x1p-16, 0x1p-15,
+    0x1p-14, 0x1p-13, 0x1p-12, 0x1p-11, 0x1p-10, 0x1p-9,  0x1p-8,  0x1p-7,  0x1p-6,  0x1p-5,  0x1p-4,
+    0x1p-3,  0x1p-2,  0x1p-1,  0x1p0,   0x1p1,   0x1p2,   0x1p3,   0x1p4,   0x1p5,   0.0};
+
 /* IEEE binary16 -> double, exact (handles zero, subnormal, inf, nan). */
 static double half_to_double(uint16_t h)
 {
@@ -47,12 +53,13 @@ static double half_to_double(uint16_t h)
     int expo = (h >> 10) & 0x1f;
     int mant = h & 0x3ff;
     double v;
-    if (expo == 0)
-        v = ldexp((double)mant, -24);                 /* subnormal: mant * 2^-24 */
-    else if (expo == 31)
+    if (expo == 0) {
+        v = (double)mant * 0x1p-24;                   /* subnormal: mant * 2^-24 (exact) */
+    } else if (expo == 31) {
         v = mant ? NAN : INFINITY;
-    else
-        v = ldexp((double)(mant | 0x400), expo - 25); /* (1024+mant) * 2^(expo-15-10) */
+    } else {
+        v = (double)(mant | 0x400) * POW2_M25[expo];  /* (1024+mant) * 2^(expo-25), exact */
+    }
     return sign ? -v : v;
 }
 
@@ -69,12 +76,14 @@ int kfo_attend_head(const uint16_t *q, const uint16_t *K, const uint16_t *V, int
     int64_t n = t_end - t_begin;
     if (n <= 0) return -1;
     double *s = (double *)malloc((size_t)n * sizeof(double));
-    if (!s) return -1;
+    double *qd = (double *)malloc((size_t)d * sizeof(double));
+    if (!s || !qd) { free(s); free(qd); return -1; }
+    for (int i = 0; i < d; ++i) qd[i] = half_to_double(q[i]);
     double m = -INFINITY;
     for (int64_t t = 0; t < n; ++t) {
         const uint16_t *k = K + (size_t)(t_begin + t) * d;
         double acc = 0.0;
-        for (int i = 0; i < d; ++i) acc += half_to_double(q[i]) * half_to_double(k[i]);
+        for (int i = 0; i < d; ++i) acc += qd[i] * half_to_double(k[i]);
         s[t] = scale * acc;
         if (s[t] > m) m = s[t];
     }
@@ -89,6 +98,7 @@ int kfo_attend_head(const uint16_t *q, const uint16_t *K, const uint16_t *V, int
     for (int j = 0; j < d; ++j) o[j] /= l;
     *lse = m + log(l);
     free(s);
+    free(qd);
     return 0;
 }
 

@@ -1,0 +1,251 @@
+"""Thin ctypes binding of libkflume (include/kflume.h).  Argument marshalling only: every step of the path
+runs in the CUDA kernels behind the C ABI.  PyTorch is used for device memory and streams, nothing else.
+
+There is no CPU fallback: constructing a `KFlume` without a CUDA device (or without the built library) raises.
+"""
+from __future__ import annotations
+
+import ctypes
+from typing import Optional, Sequence
+
+from . import build as _build
+
+KF_OK, KF_EINVAL, KF_ESTATE, KF_ENOSPC, KF_ECUDA = 0, -1, -2, -3, -4
+KF_IMPL_AUTO, KF_IMPL_SIMPLE, KF_IMPL_TMA = 0, 1, 2
+
+EXPORTS = [
+    "kf_version", "kf_strerror", "kf_last_cuda_error", "kf_pool_bytes", "kf_workspace_bytes", "kf_pool_offset",
+    "kf_create", "kf_destroy", "kf_open_request", "kf_close_request", "kf_load_context", "kf_token_boundary",
+    "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_step_commit", "kf_layer_step_host",
+    "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count",
+]
+
+
+class kf_config(ctypes.Structure):
+    _fields_ = [
+        ("n_q_heads", ctypes.c_int32), ("n_kv_heads", ctypes.c_int32), ("head_dim", ctypes.c_int32),
+        ("n_layers", ctypes.c_int32), ("range_tokens", ctypes.c_int32), ("n_partitions", ctypes.c_int32),
+        ("max_requests", ctypes.c_int32), ("max_ranges_per_request", ctypes.c_int32),
+        ("slots_per_partition", ctypes.c_int32), ("softmax_scale", ctypes.c_float),
+        ("attend_impl", ctypes.c_int32), ("min_tiles_per_worker", ctypes.c_int32),
+        ("reserved", ctypes.c_int32 * 4),
+    ]
+
+
+class KFlumeError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libkflume: {msg} (code {code})")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree libkflume.so (building it if sources are newer) and declare the prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    L = ctypes.CDLL(_build.build())
+    vp, i32, i64, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t
+    cfgp = ctypes.POINTER(kf_config)
+    L.kf_version.restype = ctypes.c_int
+    L.kf_strerror.argtypes, L.kf_strerror.restype = [ctypes.c_int], ctypes.c_char_p
+    L.kf_last_cuda_error.argtypes, L.kf_last_cuda_error.restype = [vp], ctypes.c_char_p
+    L.kf_pool_bytes.argtypes, L.kf_pool_bytes.restype = [cfgp], sz
+    L.kf_workspace_bytes.argtypes, L.kf_workspace_bytes.restype = [cfgp], sz
+    L.kf_pool_offset.argtypes, L.kf_pool_offset.restype = [cfgp, i32, i32, i32, i32, i32], sz
+    L.kf_create.argtypes = [ctypes.POINTER(vp), cfgp, ctypes.POINTER(vp), vp, sz]
+    L.kf_destroy.argtypes = [vp]
+    L.kf_open_request.argtypes = [vp, i32, i32, vp]
+    L.kf_close_request.argtypes = [vp, i32, vp]
+    L.kf_load_context.argtypes = [vp, i32, i32, i32, i32, vp, vp, vp]
+    L.kf_token_boundary.argtypes = [vp, vp]
+    L.kf_kv_append.argtypes = [vp, i32, vp, vp, vp]
+    L.kf_partial_attend.argtypes = [vp, i32, vp, ctypes.POINTER(ctypes.c_uint8), vp, vp, vp]
+    L.kf_merge_partials.argtypes = [vp, vp, vp, vp, vp, vp]
+    L.kf_attend.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
+    L.kf_step_commit.argtypes = [vp, vp]
+    L.kf_layer_step_host.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
+    L.kf_route_snapshot.argtypes = [vp] + [ctypes.POINTER(i32)] * 6 + [vp]
+    L.kf_status.argtypes = [vp, vp]
+    L.kf_plan_info.argtypes = [vp, ctypes.POINTER(i32), vp]
+    L.kf_launch_count.argtypes, L.kf_launch_count.restype = [vp], i64
+    for name in EXPORTS:
+        if getattr(L, name).restype is None:
+            getattr(L, name).restype = ctypes.c_int
+    _lib = L
+    return L
+
+
+def make_config(n_q_heads, n_kv_heads, range_tokens, n_partitions, max_requests, max_ranges_per_request,
+                slots_per_partition, n_layers=1, softmax_scale=0.0, attend_impl=KF_IMPL_AUTO,
+                min_tiles_per_worker=0, head_dim=128) -> kf_config:
+    c = kf_config()
+    c.n_q_heads, c.n_kv_heads, c.head_dim, c.n_layers = n_q_heads, n_kv_heads, head_dim, n_layers
+    c.range_tokens, c.n_partitions, c.max_requests = range_tokens, n_partitions, max_requests
+    c.max_ranges_per_request, c.slots_per_partition = max_ranges_per_request, slots_per_partition
+    c.softmax_scale, c.attend_impl, c.min_tiles_per_worker = softmax_scale, attend_impl, min_tiles_per_worker
+    return c
+
+
+def _ptr(t) -> ctypes.c_void_p:
+    return ctypes.c_void_p(0 if t is None else t.data_ptr())
+
+
+class KFlume:
+    """One libkflume context plus the device memory it works on (allocated here with torch, owned by this object)."""
+
+    def __init__(self, cfg: kf_config, device: str = "cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise KFlumeError(KF_ECUDA, "no CUDA device: libkflume has no CPU fallback")
+        self.lib = load_library()
+        self.cfg = cfg
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        pb = self.lib.kf_pool_bytes(ctypes.byref(cfg))
+        wb = self.lib.kf_workspace_bytes(ctypes.byref(cfg))
+        if pb == 0 or wb == 0:
+            raise KFlumeError(KF_EINVAL, "invalid kf_config")
+        self.pool_bytes, self.workspace_bytes = pb, wb
+        self._pool_store = [torch.empty(pb + 1024, dtype=torch.uint8, device=self.device)
+                            for _ in range(cfg.n_partitions)]
+        self.pools = []
+        for t in self._pool_store:
+            off = (-t.data_ptr()) % 1024
+            self.pools.append(t[off:off + pb])
+        self._ws_store = torch.empty(wb + 256, dtype=torch.uint8, device=self.device)
+        off = (-self._ws_store.data_ptr()) % 256
+        self.workspace = self._ws_store[off:off + wb]
+        arr = (ctypes.c_void_p * cfg.n_partitions)(*[p.data_ptr() for p in self.pools])
+        h = ctypes.c_void_p()
+        rc = self.lib.kf_create(ctypes.byref(h), ctypes.byref(cfg), arr, _ptr(self.workspace), wb)
+        self.h = h
+        if rc != KF_OK:
+            msg = self.lib.kf_last_cuda_error(h).decode() if h else ""
+            if h:
+                self.lib.kf_destroy(h)
+                self.h = None
+            raise KFlumeError(rc, f"kf_create: {self.lib.kf_strerror(rc).decode()} {msg}")
+        self.B, self.Hq, self.Hkv = cfg.max_requests, cfg.n_q_heads, cfg.n_kv_heads
+        self.Jmax, self.P = cfg.max_ranges_per_request, cfg.n_partitions
+
+    # ------------------------------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "h", None):
+            self.torch.cuda.synchronize(self.device)
+            self.lib.kf_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _stream(self, stream=None) -> ctypes.c_void_p:
+        s = self.torch.cuda.current_stream(self.device) if stream is None else stream
+        return ctypes.c_void_p(s.cuda_stream)
+
+    def _check(self, rc: int, what: str):
+        if rc != KF_OK:
+            extra = self.lib.kf_last_cuda_error(self.h).decode() if rc == KF_ECUDA else ""
+            raise KFlumeError(rc, f"{what}: {self.lib.kf_strerror(rc).decode()} {extra}")
+
+    def _f16(self, t, shape):
+        assert t.is_cuda and t.dtype == self.torch.float16 and t.is_contiguous() and tuple(t.shape) == tuple(shape), \
+            (t.dtype, tuple(t.shape), tuple(shape))
+        return _ptr(t)
+
+    def _f32(self, t, shape):
+        assert t.is_cuda and t.dtype == self.torch.float32 and t.is_contiguous() and tuple(t.shape) == tuple(shape), \
+            (t.dtype, tuple(t.shape), tuple(shape))
+        return _ptr(t)
+
+    # ---- same names as the C ABI --------------------------------------------------------------------
+    def open_request(self, req: int, n_tokens: int, stream=None):
+        self._check(self.lib.kf_open_request(self.h, req, n_tokens, self._stream(stream)), "kf_open_request")
+
+    def close_request(self, req: int, stream=None):
+        self._check(self.lib.kf_close_request(self.h, req, self._stream(stream)), "kf_close_request")
+
+    def load_context(self, layer: int, req: int, tok_begin: int, k, v, stream=None):
+        n = k.shape[1]
+        self._check(self.lib.kf_load_context(self.h, layer, req, tok_begin, n, self._f16(k, (self.Hkv, n, 128)),
+                                             self._f16(v, (self.Hkv, n, 128)), self._stream(stream)),
+                    "kf_load_context")
+
+    def token_boundary(self, stream=None):
+        self._check(self.lib.kf_token_boundary(self.h, self._stream(stream)), "kf_token_boundary")
+
+    def kv_append(self, layer: int, k_new, v_new, stream=None):
+        shp = (self.B, self.Hkv, 128)
+        self._check(self.lib.kf_kv_append(self.h, layer, self._f16(k_new, shp), self._f16(v_new, shp),
+                                          self._stream(stream)), "kf_kv_append")
+
+    def partial_attend(self, layer: int, q, o_part, lse_part, partition_mask: Optional[Sequence[int]] = None,
+                       stream=None):
+        mask = None
+        if partition_mask is not None:
+            assert len(partition_mask) == self.P
+            mask = (ctypes.c_uint8 * self.P)(*[1 if x else 0 for x in partition_mask])
+        self._check(self.lib.kf_partial_attend(
+            self.h, layer, self._f16(q, (self.B, self.Hq, 128)), mask,
+            self._f32(o_part, (self.B, self.Jmax, self.Hq, 128)), self._f32(lse_part, (self.B, self.Jmax, self.Hq)),
+            self._stream(stream)), "kf_partial_attend")
+
+    def merge_partials(self, o_part, lse_part, o, lse, stream=None):
+        self._check(self.lib.kf_merge_partials(
+            self.h, self._f32(o_part, (self.B, self.Jmax, self.Hq, 128)),
+            self._f32(lse_part, (self.B, self.Jmax, self.Hq)), self._f32(o, (self.B, self.Hq, 128)),
+            self._f32(lse, (self.B, self.Hq)), self._stream(stream)), "kf_merge_partials")
+
+    def attend(self, layer: int, q, o, lse, o_part=None, lse_part=None, stream=None):
+        if o_part is not None:
+            self._f32(o_part, (self.B, self.Jmax, self.Hq, 128))
+            self._f32(lse_part, (self.B, self.Jmax, self.Hq))
+        self._check(self.lib.kf_attend(self.h, layer, self._f16(q, (self.B, self.Hq, 128)),
+                                       self._f32(o, (self.B, self.Hq, 128)), self._f32(lse, (self.B, self.Hq)),
+                                       _ptr(o_part), _ptr(lse_part), self._stream(stream)), "kf_attend")
+
+    def step_commit(self, stream=None):
+        self._check(self.lib.kf_step_commit(self.h, self._stream(stream)), "kf_step_commit")
+
+    def layer_step_host(self, layer: int, q_host, k_new_host, v_new_host, o_host, lse_host, stream=None):
+        for t in (q_host, k_new_host, v_new_host, o_host, lse_host):
+            assert not t.is_cuda and t.is_contiguous()
+        assert q_host.numel() == self.B * self.Hq * 128 and k_new_host.numel() == self.B * self.Hkv * 128
+        assert o_host.numel() == self.B * self.Hq * 128 and o_host.dtype == self.torch.float32
+        self._check(self.lib.kf_layer_step_host(self.h, layer, _ptr(q_host), _ptr(k_new_host), _ptr(v_new_host),
+                                                _ptr(o_host), _ptr(lse_host), self._stream(stream)),
+                    "kf_layer_step_host")
+
+    def route_snapshot(self, stream=None) -> dict:
+        i32 = ctypes.c_int32
+        ln, nr = (i32 * self.B)(), (i32 * self.B)()
+        part, slot = (i32 * (self.B * self.Jmax))(), (i32 * (self.B * self.Jmax))()
+        fh, cur = (i32 * self.P)(), (i32 * 1)()
+        self._check(self.lib.kf_route_snapshot(self.h, ln, nr, part, slot, fh, cur, self._stream(stream)),
+                    "kf_route_snapshot")
+        J = self.Jmax
+        return {"len": list(ln), "n_ranges": list(nr),
+                "part": [list(part[r * J:(r + 1) * J]) for r in range(self.B)],
+                "slot": [list(slot[r * J:(r + 1) * J]) for r in range(self.B)],
+                "free_head": list(fh), "rr_cursor": cur[0]}
+
+    def status(self, stream=None) -> int:
+        return self.lib.kf_status(self.h, self._stream(stream))
+
+    def plan_info(self, stream=None) -> dict:
+        out = (ctypes.c_int32 * 8)()
+        self._check(self.lib.kf_plan_info(self.h, out, self._stream(stream)), "kf_plan_info")
+        keys = ["n_units", "n_tiles", "n_workers", "n_pieces", "n_entries", "tile_tokens", "max_workers", "pad"]
+        return dict(zip(keys, list(out)))
+
+    def launch_count(self) -> int:
+        return int(self.lib.kf_launch_count(self.h))
+
+    def pool_offset(self, layer: int, slot: int, kv_head: int, token: int, is_v: bool) -> int:
+        return int(self.lib.kf_pool_offset(ctypes.byref(self.cfg), layer, slot, kv_head, token, 1 if is_v else 0))

@@ -1,0 +1,463 @@
+// kf_api.cu -- the C ABI of libkflume (include/kflume.h): argument checking, workspace layout, TMA descriptor
+// creation and kernel launches.  No arithmetic of the method happens on the host.
+#include <cuda.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "kf_common.cuh"
+
+using namespace kf;
+
+struct kf_ctx {
+    kf_config cfg;
+    Dev dev;
+    int sm_count;
+    int n_ctas;
+    int impl;
+    bool plan_dirty;
+    int64_t launches;
+    char cuda_err[256];
+};
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
+
+struct Layout {
+    size_t len, n_ranges, route_part, route_slot, rr_cursor, free_head, free_cnt, free_stack, error, plan, units, spans,
+        scratch, unit_counter, group_counter, piece_o, piece_lse, range_o, range_lse, stage_q, stage_k, stage_v,
+        stage_o, stage_lse, tmaps, total;
+};
+
+bool valid_config(const kf_config *c) {
+    if (!c) return false;
+    if (c->head_dim != kHeadDim) return false;
+    if (c->n_q_heads < 1 || c->n_kv_heads < 1 || c->n_q_heads % c->n_kv_heads) return false;
+    const int G = c->n_q_heads / c->n_kv_heads;
+    if (G < 1 || G > kMaxGroup) return false;
+    if (c->n_q_heads > 128) return false;
+    if (c->n_layers < 1) return false;
+    if (c->range_tokens < 1 || (c->range_tokens & (c->range_tokens - 1))) return false;
+    if (c->n_partitions < 1 || c->n_partitions > kMaxPartitions) return false;
+    if (c->max_requests < 1 || c->max_requests > 4096) return false;
+    if (c->max_ranges_per_request < 1 || c->slots_per_partition < 1) return false;
+    if (!(c->softmax_scale >= 0.f) || !isfinite(c->softmax_scale)) return false;
+    if (c->attend_impl < KF_IMPL_AUTO || c->attend_impl > KF_IMPL_TMA) return false;
+    if (c->min_tiles_per_worker < 0) return false;
+    for (int i = 0; i < 4; ++i)
+        if (c->reserved[i]) return false;
+    // rows of one K (or V) half-pool must fit the int32 TMA coordinate
+    const double rows = (double)c->n_layers * c->slots_per_partition * c->n_kv_heads * c->range_tokens;
+    if (rows >= 2147483647.0) return false;
+    if ((double)c->max_requests * c->max_ranges_per_request * c->n_kv_heads >= 1e9) return false;
+    return true;
+}
+
+Layout make_layout(const kf_config *c) {
+    Layout L;
+    const size_t B = c->max_requests, J = c->max_ranges_per_request, P = c->n_partitions, Hq = c->n_q_heads,
+                 Hkv = c->n_kv_heads, G = Hq / Hkv, S = c->slots_per_partition;
+    const size_t E = B * J, U = E * Hkv, max_piece_slots = 2 * (size_t)kMaxWorkers + 2;
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        const size_t o = off;
+        off = align_up(off + bytes);
+        return o;
+    };
+    L.len = take(B * 4);
+    L.n_ranges = take(B * 4);
+    L.route_part = take(E * 4);
+    L.route_slot = take(E * 4);
+    L.rr_cursor = take(4);
+    L.free_head = take(P * 4);
+    L.free_cnt = take(P * 4);
+    L.free_stack = take(P * S * 4);
+    L.error = take(4);
+    L.plan = take(sizeof(PlanHeader));
+    L.units = take(U * sizeof(Unit));
+    L.spans = take((size_t)kMaxWorkers * sizeof(Span));
+    L.scratch = take((B + B + (B + 1) + E + (E + 1) + kMaxWorkers) * 4);
+    L.unit_counter = take(U * 4);
+    L.group_counter = take(B * Hkv * 4);
+    L.piece_o = take(max_piece_slots * G * kHeadDim * 4);
+    L.piece_lse = take(max_piece_slots * G * 4);
+    L.range_o = take(E * Hq * kHeadDim * 4);
+    L.range_lse = take(E * Hq * 4);
+    L.stage_q = take(B * Hq * kHeadDim * 2);
+    L.stage_k = take(B * Hkv * kHeadDim * 2);
+    L.stage_v = take(B * Hkv * kHeadDim * 2);
+    L.stage_o = take(B * Hq * kHeadDim * 4);
+    L.stage_lse = take(B * Hq * 4);
+    L.tmaps = take(P * 2 * 128);
+    L.total = off;
+    return L;
+}
+
+size_t half_pool_bytes(const kf_config *c) {
+    return (size_t)c->n_layers * c->slots_per_partition * c->n_kv_heads * c->range_tokens * (size_t)(kHeadDim * 2);
+}
+
+int cuda_fail(kf_ctx *ctx, cudaError_t e) {
+    if (ctx) snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+    return KF_ECUDA;
+}
+
+// after a launch: count it, surface launch errors
+int after_launch(kf_ctx *ctx, int n) {
+    if (n < 0) return n;
+    ctx->launches += n;
+    const cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return cuda_fail(ctx, e);
+    }
+    return KF_OK;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// One 2-D map per partition and per K / V half: [rows][128] fp16, box 16 rows x 64 halfs, 128B swizzle.
+int encode_tmaps(kf_ctx *ctx, void *const *pools) {
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    if (!fn || qres != cudaDriverEntryPointSuccess) {
+        snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled entry point unavailable");
+        return KF_ECUDA;
+    }
+    EncodeTiledFn encode = (EncodeTiledFn)fn;
+    const kf_config &c = ctx->cfg;
+    const cuuint64_t rows = (cuuint64_t)c.n_layers * c.slots_per_partition * c.n_kv_heads * c.range_tokens;
+    alignas(64) CUtensorMap maps[2 * kMaxPartitions];
+    for (int p = 0; p < c.n_partitions; ++p) {
+        for (int v = 0; v < 2; ++v) {
+            void *base = (unsigned char *)pools[p] + (v ? ctx->dev.v_off : 0);
+            const cuuint64_t dims[2] = {(cuuint64_t)kHeadDim, rows};
+            const cuuint64_t strides[1] = {(cuuint64_t)kHeadDim * 2};
+            const cuuint32_t box[2] = {64, (cuuint32_t)kTileTokens};
+            const cuuint32_t estr[2] = {1, 1};
+            const CUresult r = encode(&maps[2 * p + v], CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, base, dims, strides, box,
+                                      estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) {
+                snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled failed: CUresult %d", (int)r);
+                return KF_ECUDA;
+            }
+        }
+    }
+    static_assert(sizeof(CUtensorMap) == 128, "tensor map stride");
+    e = cudaMemcpy((void *)ctx->dev.tmaps, maps, (size_t)c.n_partitions * 2 * sizeof(CUtensorMap),
+                   cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return KF_OK;
+}
+
+int ensure_plan(kf_ctx *ctx, cudaStream_t s) {
+    if (!ctx->plan_dirty) return KF_OK;
+    const int rc = after_launch(ctx, launch_plan(ctx->dev, s));
+    if (rc == KF_OK) ctx->plan_dirty = false;
+    return rc;
+}
+
+int run_attend(kf_ctx *ctx, const AttendParams &ap, cudaStream_t s) {
+    if (ctx->impl == KF_IMPL_SIMPLE) return after_launch(ctx, launch_attend_simple(ap, ctx->n_ctas, s));
+    return after_launch(ctx, launch_attend_tma(ap, ctx->n_ctas, s));
+}
+
+bool bad_layer(const kf_ctx *ctx, int layer) { return layer < 0 || layer >= ctx->cfg.n_layers; }
+
+}  // namespace
+
+extern "C" {
+
+int kf_version(void) { return KF_VERSION; }
+
+const char *kf_strerror(int code) {
+    switch (code) {
+        case KF_OK: return "ok";
+        case KF_EINVAL: return "invalid argument";
+        case KF_ESTATE: return "call not valid in this state";
+        case KF_ENOSPC: return "no free KV slot / range entry";
+        case KF_ECUDA: return "CUDA error";
+        default: return "unknown error";
+    }
+}
+
+const char *kf_last_cuda_error(const kf_ctx *ctx) { return ctx ? ctx->cuda_err : ""; }
+
+size_t kf_pool_bytes(const kf_config *cfg) { return valid_config(cfg) ? 2 * half_pool_bytes(cfg) : 0; }
+
+size_t kf_workspace_bytes(const kf_config *cfg) { return valid_config(cfg) ? make_layout(cfg).total : 0; }
+
+size_t kf_pool_offset(const kf_config *c, int32_t layer, int32_t slot, int32_t kv_head, int32_t token, int32_t is_v) {
+    if (!valid_config(c) || layer < 0 || layer >= c->n_layers || slot < 0 || slot >= c->slots_per_partition ||
+        kv_head < 0 || kv_head >= c->n_kv_heads || token < 0 || token >= c->range_tokens)
+        return (size_t)-1;
+    const size_t row = (((size_t)layer * c->slots_per_partition + slot) * c->n_kv_heads + kv_head) * c->range_tokens + token;
+    return row * (size_t)(kHeadDim * 2) + (is_v ? half_pool_bytes(c) : 0);
+}
+
+int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *workspace, size_t workspace_bytes) {
+    if (!out) return KF_EINVAL;
+    *out = nullptr;
+    if (!valid_config(cfg) || !pool_ptrs || !workspace) return KF_EINVAL;
+    const Layout L = make_layout(cfg);
+    if (workspace_bytes < L.total || ((uintptr_t)workspace & (kAlign - 1))) return KF_EINVAL;
+    for (int p = 0; p < cfg->n_partitions; ++p)
+        if (!pool_ptrs[p] || ((uintptr_t)pool_ptrs[p] & 1023)) return KF_EINVAL;
+
+    kf_ctx *ctx = new (std::nothrow) kf_ctx();
+    if (!ctx) return KF_EINVAL;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->cfg = *cfg;
+    *out = ctx;  // returned even on KF_ECUDA so that kf_last_cuda_error() can be read; caller destroys it
+
+    int dev_id = 0;
+    cudaError_t e = cudaGetDevice(&dev_id);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev_id);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    ctx->sm_count = prop.multiProcessorCount;
+    ctx->n_ctas = ctx->sm_count;
+    if (ctx->n_ctas * kWarpsPerCta > kMaxWorkers) ctx->n_ctas = kMaxWorkers / kWarpsPerCta;
+    ctx->impl = cfg->attend_impl == KF_IMPL_AUTO ? KF_IMPL_TMA : cfg->attend_impl;
+    ctx->plan_dirty = true;
+
+    unsigned char *ws = (unsigned char *)workspace;
+    e = cudaMemset(ws, 0, L.total);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    // len = -1 (closed), routes = -1 (unused)
+    e = cudaMemset(ws + L.len, 0xFF, (size_t)cfg->max_requests * 4);
+    if (e == cudaSuccess) e = cudaMemset(ws + L.route_part, 0xFF, (size_t)cfg->max_requests * cfg->max_ranges_per_request * 4);
+    if (e == cudaSuccess) e = cudaMemset(ws + L.route_slot, 0xFF, (size_t)cfg->max_requests * cfg->max_ranges_per_request * 4);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+
+    Dev &d = ctx->dev;
+    d.Hq = cfg->n_q_heads;
+    d.Hkv = cfg->n_kv_heads;
+    d.G = d.Hq / d.Hkv;
+    d.L = cfg->n_layers;
+    d.R = cfg->range_tokens;
+    d.P = cfg->n_partitions;
+    d.B = cfg->max_requests;
+    d.Jmax = cfg->max_ranges_per_request;
+    d.slots = cfg->slots_per_partition;
+    d.max_workers = ctx->n_ctas * kWarpsPerCta;
+    d.min_tiles = cfg->min_tiles_per_worker > 0 ? cfg->min_tiles_per_worker : 4;
+    const float scale = cfg->softmax_scale > 0.f ? cfg->softmax_scale : 1.0f / sqrtf((float)kHeadDim);
+    d.scale_log2 = scale * 1.4426950408889634f;
+    d.len = (int32_t *)(ws + L.len);
+    d.n_ranges = (int32_t *)(ws + L.n_ranges);
+    d.route_part = (int32_t *)(ws + L.route_part);
+    d.route_slot = (int32_t *)(ws + L.route_slot);
+    d.rr_cursor = (int32_t *)(ws + L.rr_cursor);
+    d.free_head = (int32_t *)(ws + L.free_head);
+    d.free_cnt = (int32_t *)(ws + L.free_cnt);
+    d.free_stack = (int32_t *)(ws + L.free_stack);
+    d.error = (int32_t *)(ws + L.error);
+    d.plan = (PlanHeader *)(ws + L.plan);
+    d.units = (Unit *)(ws + L.units);
+    d.spans = (Span *)(ws + L.spans);
+    d.scratch = (int32_t *)(ws + L.scratch);
+    d.unit_counter = (int32_t *)(ws + L.unit_counter);
+    d.group_counter = (int32_t *)(ws + L.group_counter);
+    d.piece_o = (float *)(ws + L.piece_o);
+    d.piece_lse = (float *)(ws + L.piece_lse);
+    d.range_o = (float *)(ws + L.range_o);
+    d.range_lse = (float *)(ws + L.range_lse);
+    d.stage_q = (__half *)(ws + L.stage_q);
+    d.stage_k = (__half *)(ws + L.stage_k);
+    d.stage_v = (__half *)(ws + L.stage_v);
+    d.stage_o = (float *)(ws + L.stage_o);
+    d.stage_lse = (float *)(ws + L.stage_lse);
+    d.tmaps = ws + L.tmaps;
+    d.v_off = half_pool_bytes(cfg);
+    for (int p = 0; p < cfg->n_partitions; ++p) d.pool[p] = (unsigned char *)pool_ptrs[p];
+
+    if (ctx->impl == KF_IMPL_TMA) {
+        int rc = encode_tmaps(ctx, pool_ptrs);
+        if (rc != KF_OK) return rc;
+        if (attend_tma_setup() != 0) return cuda_fail(ctx, cudaGetLastError());
+    }
+    e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return KF_OK;
+}
+
+int kf_destroy(kf_ctx *ctx) {
+    if (!ctx) return KF_EINVAL;
+    delete ctx;
+    return KF_OK;
+}
+
+int kf_open_request(kf_ctx *ctx, int32_t req, int32_t n_tokens, kf_stream stream) {
+    if (!ctx || req < 0 || req >= ctx->cfg.max_requests || n_tokens < 0) return KF_EINVAL;
+    ctx->plan_dirty = true;
+    return after_launch(ctx, launch_open_request(ctx->dev, req, n_tokens, (cudaStream_t)stream));
+}
+
+int kf_close_request(kf_ctx *ctx, int32_t req, kf_stream stream) {
+    if (!ctx || req < 0 || req >= ctx->cfg.max_requests) return KF_EINVAL;
+    ctx->plan_dirty = true;
+    return after_launch(ctx, launch_close_request(ctx->dev, req, (cudaStream_t)stream));
+}
+
+int kf_load_context(kf_ctx *ctx, int32_t layer, int32_t req, int32_t tok_begin, int32_t n_tokens, const void *k,
+                    const void *v, kf_stream stream) {
+    if (!ctx || bad_layer(ctx, layer) || req < 0 || req >= ctx->cfg.max_requests || tok_begin < 0 || n_tokens < 0)
+        return KF_EINVAL;
+    if (n_tokens == 0) return KF_OK;
+    if (!k || !v || ((uintptr_t)k & 15) || ((uintptr_t)v & 15)) return KF_EINVAL;
+    if ((int64_t)tok_begin + n_tokens > (int64_t)ctx->cfg.max_ranges_per_request * ctx->cfg.range_tokens) return KF_EINVAL;
+    return after_launch(ctx, launch_load_context(ctx->dev, layer, req, tok_begin, n_tokens, (const __half *)k,
+                                                 (const __half *)v, (cudaStream_t)stream));
+}
+
+int kf_token_boundary(kf_ctx *ctx, kf_stream stream) {
+    if (!ctx) return KF_EINVAL;
+    int rc = after_launch(ctx, launch_token_boundary(ctx->dev, (cudaStream_t)stream));
+    if (rc != KF_OK) return rc;
+    ctx->plan_dirty = true;
+    return ensure_plan(ctx, (cudaStream_t)stream);
+}
+
+int kf_kv_append(kf_ctx *ctx, int32_t layer, const void *k_new, const void *v_new, kf_stream stream) {
+    if (!ctx || bad_layer(ctx, layer) || !k_new || !v_new || ((uintptr_t)k_new & 15) || ((uintptr_t)v_new & 15))
+        return KF_EINVAL;
+    return after_launch(ctx, launch_kv_append(ctx->dev, layer, (const __half *)k_new, (const __half *)v_new,
+                                              (cudaStream_t)stream));
+}
+
+int kf_partial_attend(kf_ctx *ctx, int32_t layer, const void *q, const uint8_t *partition_mask, float *o_part,
+                      float *lse_part, kf_stream stream) {
+    if (!ctx || bad_layer(ctx, layer) || !q || !o_part || !lse_part || ((uintptr_t)q & 15) || ((uintptr_t)o_part & 15))
+        return KF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_plan(ctx, s);
+    if (rc != KF_OK) return rc;
+    AttendParams ap;
+    ap.d = ctx->dev;
+    ap.layer = layer;
+    ap.q = (const __half *)q;
+    ap.o_part = o_part;
+    ap.lse_part = lse_part;
+    ap.o = nullptr;
+    ap.lse = nullptr;
+    ap.fused = 0;
+    ap.part_mask = 0;
+    for (int p = 0; p < ctx->cfg.n_partitions; ++p)
+        if (!partition_mask || partition_mask[p]) ap.part_mask |= 1ull << p;
+    rc = run_attend(ctx, ap, s);
+    if (rc != KF_OK) return rc;
+    return after_launch(ctx, launch_merge_units(ap, ctx->n_ctas, s));
+}
+
+int kf_merge_partials(kf_ctx *ctx, const float *o_part, const float *lse_part, float *o, float *lse, kf_stream stream) {
+    if (!ctx || !o_part || !lse_part || !o || !lse || ((uintptr_t)o_part & 15) || ((uintptr_t)o & 15)) return KF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_plan(ctx, s);
+    if (rc != KF_OK) return rc;
+    return after_launch(ctx, launch_merge_ranges(ctx->dev, o_part, lse_part, o, lse, s));
+}
+
+int kf_attend(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, float *o_part, float *lse_part,
+              kf_stream stream) {
+    if (!ctx || bad_layer(ctx, layer) || !q || !o || !lse || ((uintptr_t)q & 15) || ((uintptr_t)o & 15)) return KF_EINVAL;
+    if ((o_part == nullptr) != (lse_part == nullptr) || ((uintptr_t)o_part & 15)) return KF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_plan(ctx, s);
+    if (rc != KF_OK) return rc;
+    AttendParams ap;
+    ap.d = ctx->dev;
+    ap.layer = layer;
+    ap.q = (const __half *)q;
+    ap.o_part = o_part ? o_part : ctx->dev.range_o;
+    ap.lse_part = lse_part ? lse_part : ctx->dev.range_lse;
+    ap.o = o;
+    ap.lse = lse;
+    ap.fused = 1;
+    ap.part_mask = ~0ull;
+    return run_attend(ctx, ap, s);
+}
+
+int kf_step_commit(kf_ctx *ctx, kf_stream stream) {
+    if (!ctx) return KF_EINVAL;
+    ctx->plan_dirty = true;
+    return after_launch(ctx, launch_step_commit(ctx->dev, (cudaStream_t)stream));
+}
+
+int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host, const void *v_new_host,
+                       float *o_host, float *lse_host, kf_stream stream) {
+    if (!ctx || bad_layer(ctx, layer) || !q_host || !k_new_host || !v_new_host || !o_host || !lse_host) return KF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const Dev &d = ctx->dev;
+    const size_t qb = (size_t)d.B * d.Hq * kHeadDim * 2, kb = (size_t)d.B * d.Hkv * kHeadDim * 2;
+    cudaError_t e = cudaMemcpyAsync(d.stage_q, q_host, qb, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d.stage_k, k_new_host, kb, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d.stage_v, v_new_host, kb, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    int rc = kf_kv_append(ctx, layer, d.stage_k, d.stage_v, stream);
+    if (rc != KF_OK) return rc;
+    rc = kf_attend(ctx, layer, d.stage_q, d.stage_o, d.stage_lse, nullptr, nullptr, stream);
+    if (rc != KF_OK) return rc;
+    e = cudaMemcpyAsync(o_host, d.stage_o, (size_t)d.B * d.Hq * kHeadDim * 4, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(lse_host, d.stage_lse, (size_t)d.B * d.Hq * 4, cudaMemcpyDeviceToHost, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return KF_OK;
+}
+
+int kf_route_snapshot(kf_ctx *ctx, int32_t *len, int32_t *n_ranges, int32_t *part, int32_t *slot, int32_t *free_head,
+                      int32_t *rr_cursor, kf_stream stream) {
+    if (!ctx) return KF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const Dev &d = ctx->dev;
+    const size_t B = d.B, E = (size_t)d.B * d.Jmax;
+    cudaError_t e = cudaSuccess;
+    if (len && e == cudaSuccess) e = cudaMemcpyAsync(len, d.len, B * 4, cudaMemcpyDeviceToHost, s);
+    if (n_ranges && e == cudaSuccess) e = cudaMemcpyAsync(n_ranges, d.n_ranges, B * 4, cudaMemcpyDeviceToHost, s);
+    if (part && e == cudaSuccess) e = cudaMemcpyAsync(part, d.route_part, E * 4, cudaMemcpyDeviceToHost, s);
+    if (slot && e == cudaSuccess) e = cudaMemcpyAsync(slot, d.route_slot, E * 4, cudaMemcpyDeviceToHost, s);
+    if (free_head && e == cudaSuccess) e = cudaMemcpyAsync(free_head, d.free_head, (size_t)d.P * 4, cudaMemcpyDeviceToHost, s);
+    if (rr_cursor && e == cudaSuccess) e = cudaMemcpyAsync(rr_cursor, d.rr_cursor, 4, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return KF_OK;
+}
+
+int kf_status(kf_ctx *ctx, kf_stream stream) {
+    if (!ctx) return KF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int32_t word = 0;
+    cudaError_t e = cudaMemcpyAsync(&word, ctx->dev.error, 4, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    if (word != 0) {
+        e = cudaMemsetAsync(ctx->dev.error, 0, 4, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+    }
+    return word;
+}
+
+int kf_plan_info(kf_ctx *ctx, int32_t *out, kf_stream stream) {
+    if (!ctx || !out) return KF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_plan(ctx, s);
+    if (rc != KF_OK) return rc;
+    cudaError_t e = cudaMemcpyAsync(out, ctx->dev.plan, sizeof(PlanHeader), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return KF_OK;
+}
+
+int64_t kf_launch_count(const kf_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,312 @@
+// kf_attend_tma.cu -- KF_IMPL_TMA: the roofline kernel for split-KV decode attention over token-range
+// partitions (PAPER.md:137, :145; "decode attention is bandwidth-bound", :225).
+//
+// Design (B200 / sm_100a):
+//  * Persistent grid, one CTA of 8 warps per SM.  Every WARP is an independent worker that owns an equal,
+//    contiguous span of the step's 16-token tiles (stream-K split built on the device by plan_kernel), its
+//    own 3-stage shared-memory ring and its own mbarriers: there is no CTA-wide synchronisation at all.
+//  * K/V tiles are fetched by TMA (cp.async.bulk.tensor.2d, one elected lane) straight from the routed pool
+//    slot into 128B-swizzled shared memory; each of the 1184 workers keeps up to 24 KB in flight
+//    (~190 KB per SM) -- Little's law at ~6.5 TB/s x ~1 us needs ~50 KB per SM.
+//  * The G query heads of a GQA group are packed into the M dimension of mma.sync.m16n8k16 (fp16 in, fp32
+//    accumulate): S = Q K^T and O += P V run on the tensor cores so the ALUs only do the online softmax.
+//    K fragments come from ldmatrix, V fragments from ldmatrix.trans; the hardware swizzle makes both
+//    bank-conflict free.
+//  * Online softmax in fp32, base 2, quad shuffles; the accumulator rescale is skipped when no running
+//    maximum moved.
+//  * The partial (o, lse) of each piece goes to the range-partial rows or to a piece buffer; in fused mode
+//    the last-arriving worker merges pieces -> range -> request (kf_merge.cuh).
+#include <cuda.h>
+
+#include "kf_merge.cuh"
+
+namespace kf {
+
+constexpr int kStages = 3;
+constexpr int kSubTile = kTileTokens * 128;     // 16 rows x 128 B (64 halfs): one TMA box
+constexpr int kStageBytes = 4 * kSubTile;       // K lo | K hi | V lo | V hi = 8 KB
+constexpr int kWarpSmem = kStages * kStageBytes;
+constexpr int kTmaSmemBytes = kWarpsPerCta * kWarpSmem + 1024;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "KF_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra KF_DONE;\n"
+        "bra KF_WAIT;\n"
+        "KF_DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const void *tmap, int x, int y, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(dst),
+        "l"(tmap), "r"(bar), "r"(x), "r"(y)
+        : "memory");
+}
+__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_trans(uint32_t addr, uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(addr));
+}
+// D(16x8,f32) += A(16x16,f16,row) * B(16x8,f16,col); rows 8..15 of A are zero (a1 = a3 = 0): G <= 8 heads
+__device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a2, uint32_t b0, uint32_t b1) {
+    const uint32_t z = 0u;
+    asm volatile(
+        "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+        : "r"(a0), "r"(z), "r"(a2), "r"(z), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ float fast_exp2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
+    const __half2 h = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<const uint32_t *>(&h);
+}
+__device__ __forceinline__ Unit load_unit(const Unit *units, int u) {
+    const int4 *p = reinterpret_cast<const int4 *>(units + u);
+    const int4 a = __ldg(p), b = __ldg(p + 1);
+    Unit un;
+    un.req = a.x;
+    un.range = a.y;
+    un.part = a.z;
+    un.slot = a.w;
+    un.cnt = b.x;
+    un.tile_begin = b.y;
+    un.piece_begin = b.z;
+    un.n_pieces = b.w;
+    return un;
+}
+
+__global__ void __launch_bounds__(kWarpsPerCta * 32, 1) attend_tma_kernel(const AttendParams p) {
+    extern __shared__ unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t bars[kWarpsPerCta][kStages];
+    const Dev &d = p.d;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int w = blockIdx.x * kWarpsPerCta + warp;
+    const Span sp = d.spans[w];
+    const int n_tiles = sp.n_tiles;
+    if (n_tiles == 0) return;  // idle worker: safe, the kernel has no CTA-wide barrier
+
+    const uint32_t wbase = ((smem_u32(smem_raw) + 1023u) & ~1023u) + warp * kWarpSmem;
+    const uint32_t bar0 = smem_u32(&bars[warp][0]);
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) mbar_init(bar0 + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncwarp();
+
+    const int G = d.G, Hkv = d.Hkv;
+    const int row_stride_unit = d.R;  // rows per (slot, kv head)
+    const unsigned char *tmaps = reinterpret_cast<const unsigned char *>(d.tmaps);
+
+    // ---- load cursor (runs kStages tiles ahead of the compute cursor) --------------------------------
+    int lu = sp.unit, lt = sp.tile_in_unit, l_left = n_tiles;
+    Unit lun = load_unit(d.units, lu);
+    int l_ntiles = (lun.cnt + kTileTokens - 1) / kTileTokens;
+    int l_rowbase = ((p.layer * d.slots + lun.slot) * Hkv + (lu % Hkv)) * row_stride_unit;
+    auto issue_tile = [&](int stage) {
+        if (lane == 0) {
+            const uint32_t sb = wbase + stage * kStageBytes, bar = bar0 + 8 * stage;
+            const int row = l_rowbase + lt * kTileTokens;
+            const unsigned char *tk = tmaps + (size_t)lun.part * 256;
+            mbar_expect_tx(bar, kStageBytes);
+            tma_load_2d(sb, tk, 0, row, bar);
+            tma_load_2d(sb + kSubTile, tk, 64, row, bar);
+            tma_load_2d(sb + 2 * kSubTile, tk + 128, 0, row, bar);
+            tma_load_2d(sb + 3 * kSubTile, tk + 128, 64, row, bar);
+        }
+        ++lt;
+        --l_left;
+        if (lt == l_ntiles && l_left > 0) {
+            ++lu;
+            lt = 0;
+            lun = load_unit(d.units, lu);
+            l_ntiles = (lun.cnt + kTileTokens - 1) / kTileTokens;
+            l_rowbase = ((p.layer * d.slots + lun.slot) * Hkv + (lu % Hkv)) * row_stride_unit;
+        }
+    };
+#pragma unroll
+    for (int s = 0; s < kStages; ++s)
+        if (s < n_tiles) issue_tile(s);
+
+    // ---- per-lane shared-memory offsets of the ldmatrix rows (128B hardware swizzle: chunk ^= row & 7) ----
+    const int l7 = lane & 7, mi = lane >> 3;
+    const uint32_t k_row = l7 * 128;
+    const uint32_t k_x0 = ((mi) ^ l7) << 4, k_x1 = ((4 + mi) ^ l7) << 4;
+    const uint32_t v_row = ((mi & 1) * 8 + l7) * 128;
+    const int v_c = mi >> 1;
+    const int qrow = lane >> 2, qcol = (lane & 3) * 2;
+
+    // ---- compute cursor ------------------------------------------------------------------------------
+    int cu = sp.unit, ct = sp.tile_in_unit, piece = sp.piece;
+    Unit cun = load_unit(d.units, cu);
+    int c_ntiles = (cun.cnt + kTileTokens - 1) / kTileTokens;
+
+    uint32_t qa[8][2];  // A fragments of Q: [k-step][a0, a2]
+    auto load_q = [&]() {
+        const __half *qg = p.q + ((size_t)cun.req * d.Hq + (size_t)(cu % Hkv) * G + qrow) * kHeadDim + qcol;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+            qa[ks][0] = qrow < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16)) : 0u;
+            qa[ks][1] = qrow < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16 + 8)) : 0u;
+        }
+    };
+    load_q();
+
+    float o[16][4];
+    float m_run = -INFINITY, l_run = 0.f;
+#pragma unroll
+    for (int n = 0; n < 16; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
+
+    for (int i = 0; i < n_tiles; ++i) {
+        const int stage = i % kStages;
+        const uint32_t sb = wbase + stage * kStageBytes;
+        mbar_wait(bar0 + 8 * stage, (i / kStages) & 1);
+
+        const int valid = min(kTileTokens, cun.cnt - ct * kTileTokens);
+        const bool ragged = valid < kTileTokens;
+        if (ragged) {
+            // rows >= valid hold whatever the pool holds (maybe NaN patterns): zero them in V so 0 * V = 0
+            for (int idx = lane; idx < (kTileTokens - valid) * 16; idx += 32) {
+                const int row = valid + (idx >> 4), rem = idx & 15;
+                const uint32_t a = sb + 2 * kSubTile + (rem >> 3) * kSubTile + row * 128 + (rem & 7) * 16;
+                asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
+            }
+            __syncwarp();
+        }
+
+        // ---- S = Q K^T : 16 (heads, padded) x 16 tokens ------------------------------------------------
+        float s[2][4];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) s[j][0] = s[j][1] = s[j][2] = s[j][3] = 0.f;
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii) {
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                uint32_t b0, b1, b2, b3;
+                ldsm_x4(sb + (ii >> 1) * kSubTile + j * 1024 + k_row + ((ii & 1) ? k_x1 : k_x0), b0, b1, b2, b3);
+                mma16816(s[j], qa[2 * ii][0], qa[2 * ii][1], b0, b1);
+                mma16816(s[j], qa[2 * ii + 1][0], qa[2 * ii + 1][1], b2, b3);
+            }
+        }
+
+        // ---- online softmax on row `qrow` (c0, c1 of each n-tile), base 2 ------------------------------
+        float mx = -INFINITY;
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const float v = s[j][e] * d.scale_log2;
+                s[j][e] = (8 * j + qcol + e < valid) ? v : -INFINITY;
+                mx = fmaxf(mx, s[j][e]);
+            }
+        }
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
+        const float m_new = fmaxf(m_run, mx);
+        const float alpha = fast_exp2(m_run - m_new);
+        const float p00 = fast_exp2(s[0][0] - m_new), p01 = fast_exp2(s[0][1] - m_new);
+        const float p10 = fast_exp2(s[1][0] - m_new), p11 = fast_exp2(s[1][1] - m_new);
+        l_run = l_run * alpha + ((p00 + p01) + (p10 + p11));
+        m_run = m_new;
+        if (__any_sync(0xffffffffu, alpha != 1.f)) {
+#pragma unroll
+            for (int n = 0; n < 16; ++n) {
+                o[n][0] *= alpha;
+                o[n][1] *= alpha;
+            }
+        }
+        const uint32_t pa0 = pack_half2(p00, p01), pa2 = pack_half2(p10, p11);
+
+        // ---- O += P V : 16 x 128 -----------------------------------------------------------------------
+#pragma unroll
+        for (int nd = 0; nd < 16; nd += 2) {
+            uint32_t b0, b1, b2, b3;
+            ldsm_x4_trans(sb + 2 * kSubTile + (nd >> 3) * kSubTile + v_row + ((((nd & 7) + v_c) ^ l7) << 4), b0, b1, b2,
+                          b3);
+            mma16816(o[nd], pa0, pa2, b0, b1);
+            mma16816(o[nd + 1], pa0, pa2, b2, b3);
+        }
+
+        __syncwarp();  // every lane is done reading this stage
+        if (i + kStages < n_tiles) {
+            if (ragged && lane == 0) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            issue_tile(stage);
+        }
+
+        ++ct;
+        if (ct == c_ntiles || i == n_tiles - 1) {
+            // ---- end of a piece: emit its partial (o, lse) --------------------------------------------
+            const int g = cu % Hkv;
+            float lt = l_run + __shfl_xor_sync(0xffffffffu, l_run, 1);
+            lt += __shfl_xor_sync(0xffffffffu, lt, 2);
+            const bool selected = (p.part_mask >> cun.part) & 1ull;
+            if (selected) {
+                const PieceDest pd = piece_dest(p, cun, cu, g, piece);
+                if (qrow < G) {
+                    const float inv = 1.f / lt;
+                    float *dst = pd.o + (size_t)qrow * kHeadDim + qcol;
+#pragma unroll
+                    for (int n = 0; n < 16; ++n)
+                        *reinterpret_cast<float2 *>(dst + 8 * n) = make_float2(o[n][0] * inv, o[n][1] * inv);
+                    const float lse = (m_run + log2f(lt)) * 0.6931471805599453f;
+                    if ((lane & 3) == 0) pd.lse[qrow] = lse;
+                    if (pd.o2) {
+                        float *dst2 = pd.o2 + (size_t)qrow * kHeadDim + qcol;
+#pragma unroll
+                        for (int n = 0; n < 16; ++n)
+                            *reinterpret_cast<float2 *>(dst2 + 8 * n) = make_float2(o[n][0] * inv, o[n][1] * inv);
+                        if ((lane & 3) == 0) pd.lse2[qrow] = lse;
+                    }
+                }
+                if (p.fused) finish_piece(p, cu, cun, g, lane);
+            }
+            if (i + 1 < n_tiles) {
+                ++cu;
+                ct = 0;
+                ++piece;
+                cun = load_unit(d.units, cu);
+                c_ntiles = (cun.cnt + kTileTokens - 1) / kTileTokens;
+                load_q();
+                m_run = -INFINITY;
+                l_run = 0.f;
+#pragma unroll
+                for (int n = 0; n < 16; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
+            }
+        }
+    }
+}
+
+int attend_tma_setup() {
+    cudaError_t e = cudaFuncSetAttribute(attend_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTmaSmemBytes);
+    return e == cudaSuccess ? 0 : KF_ECUDA;
+}
+
+int launch_attend_tma(const AttendParams &p, int n_ctas, cudaStream_t s) {
+    attend_tma_kernel<<<n_ctas, kWarpsPerCta * 32, kTmaSmemBytes, s>>>(p);
+    return 1;
+}
+
+}  // namespace kf

@@ -1,0 +1,124 @@
+// kf_common.cuh -- device-side state, work plan and launch parameters shared by the kernels of libkflume.
+// Product code: shares nothing with oracle/.
+#pragma once
+
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/kflume.h"
+
+namespace kf {
+
+constexpr int kHeadDim = 128;
+constexpr int kTileTokens = 16;       // work-plan granule = one MMA k-step of tokens
+constexpr int kWarpsPerCta = 8;       // one worker = one warp
+constexpr int kMaxWorkers = 2048;     // >= SMs * kWarpsPerCta on any Blackwell part (148 * 8 = 1184)
+constexpr int kMaxGroup = 8;          // G = H_q / H_kv
+constexpr int kMaxPartitions = 64;
+
+// One unit of attention work: (request, token range, kv head).  Built by the plan kernel.
+struct Unit {
+    int32_t req;
+    int32_t range;
+    int32_t part;
+    int32_t slot;
+    int32_t cnt;         // tokens of this range attended in this step (1..R)
+    int32_t tile_begin;  // first global tile index of this unit
+    int32_t piece_begin; // first global piece index of this unit
+    int32_t n_pieces;    // pieces (worker spans intersecting this unit)
+};
+
+// Contiguous span of global tiles given to one worker (warp): stream-K style equal split.
+struct Span {
+    int32_t unit;         // unit holding the first tile
+    int32_t tile_in_unit; // index of the first tile inside that unit
+    int32_t n_tiles;      // 0 => idle worker
+    int32_t piece;        // global piece index of the first piece
+};
+
+struct PlanHeader {
+    int32_t n_units;
+    int32_t n_tiles;
+    int32_t n_workers; // active workers
+    int32_t n_pieces;
+    int32_t n_entries; // (request, range) entries = n_units / H_kv
+    int32_t tile_tokens;
+    int32_t max_workers;
+    int32_t pad;
+};
+
+// Device pointers into the caller's workspace + immutable config.  Passed BY VALUE to every kernel.
+struct Dev {
+    // config
+    int32_t Hq, Hkv, G, L, R, P, B, Jmax, slots;
+    int32_t max_workers, min_tiles;
+    float scale_log2;  // softmax_scale * log2(e)
+    // routing state
+    int32_t *len;        // [B]   -1 = closed
+    int32_t *n_ranges;   // [B]
+    int32_t *route_part; // [B][Jmax]
+    int32_t *route_slot; // [B][Jmax]
+    int32_t *rr_cursor;  // [1]
+    int32_t *free_head;  // [P]
+    int32_t *free_cnt;   // [P]
+    int32_t *free_stack; // [P][slots]
+    int32_t *error;      // [1]
+    // work plan
+    PlanHeader *plan;
+    Unit *units;            // [B*Jmax*Hkv]
+    Span *spans;            // [kMaxWorkers]
+    int32_t *scratch;       // plan scratch: [B] J, [B] S, [B+1] entry prefix, [E+1] tile prefix, [E] tiles, [W] cuts
+    int32_t *unit_counter;  // [B*Jmax*Hkv]  last-arriver counters (self-resetting)
+    int32_t *group_counter; // [B*Hkv]
+    // partial buffers
+    float *piece_o;   // [max_pieces][G][128]
+    float *piece_lse; // [max_pieces][G]
+    float *range_o;   // [B][Jmax][Hq][128]  scratch when the caller passes no o_part
+    float *range_lse; // [B][Jmax][Hq]
+    // staging for kf_layer_step_host
+    __half *stage_q, *stage_k, *stage_v; // [B][Hq][128], [B][Hkv][128] x2
+    float *stage_o, *stage_lse;          // [B][Hq][128], [B][Hq]
+    // pools
+    unsigned char *pool[kMaxPartitions];
+    size_t v_off;        // byte offset of the V half of a pool
+    const void *tmaps;   // [P][2] CUtensorMap (K, V) in device memory, 128-byte stride
+};
+
+struct AttendParams {
+    Dev d;
+    int32_t layer;
+    const __half *q; // [B][Hq][128]
+    float *o_part;   // [B][Jmax][Hq][128]
+    float *lse_part; // [B][Jmax][Hq]
+    float *o;        // [B][Hq][128] (fused only)
+    float *lse;      // [B][Hq]
+    uint64_t part_mask;
+    int32_t fused;
+};
+
+__device__ __forceinline__ void set_error(const Dev &d, int code) { atomicCAS(d.error, 0, code); }
+
+// byte offset (within a partition pool) of K row (layer, slot, g, t)
+__device__ __forceinline__ size_t row_offset(const Dev &d, int layer, int slot, int g, int t) {
+    return ((((size_t)layer * d.slots + slot) * d.Hkv + g) * d.R + t) * (size_t)(kHeadDim * 2);
+}
+
+// host-side launchers (definitions in the respective .cu files); each returns the number of kernels launched
+// or a negative KF_E* code.
+int launch_open_request(const Dev &d, int req, int n_tokens, cudaStream_t s);
+int launch_close_request(const Dev &d, int req, cudaStream_t s);
+int launch_token_boundary(const Dev &d, cudaStream_t s);
+int launch_plan(const Dev &d, cudaStream_t s);
+int launch_step_commit(const Dev &d, cudaStream_t s);
+int launch_load_context(const Dev &d, int layer, int req, int tok_begin, int n_tokens, const __half *k,
+                        const __half *v, cudaStream_t s);
+int launch_kv_append(const Dev &d, int layer, const __half *k_new, const __half *v_new, cudaStream_t s);
+int launch_attend_simple(const AttendParams &p, int n_ctas, cudaStream_t s);
+int launch_attend_tma(const AttendParams &p, int n_ctas, cudaStream_t s);
+int attend_tma_setup();  // cudaFuncSetAttribute for the dynamic shared memory; 0 or KF_ECUDA
+int launch_merge_units(const AttendParams &p, int n_ctas, cudaStream_t s);
+int launch_merge_ranges(const Dev &d, const float *o_part, const float *lse_part, float *o, float *lse,
+                        cudaStream_t s);
+
+}  // namespace kf

@@ -301,3 +301,16 @@ def test_golden_cfg4_ranges_and_one_full_head():
     op, lp = oracle.attend_ranges(q[0:1], K, V, R)
     om, lm = oracle.merge(op, lp)
     assert np.abs(om - o).max() < 1e-14 and abs(lm[0] - lse[0]) < 1e-12
+
+
+def test_half_conversion_exhaustive():
+    """Every fp16 bit pattern passes through the oracle's own half->double conversion unchanged
+    (1-token context returns V exactly), compared with numpy's conversion."""
+    pats = np.arange(65536, dtype=np.uint16).view(np.float16)
+    q = np.zeros((1, 128), np.float16)
+    K = np.zeros((1, 1, 128), np.float16)
+    for a in range(0, 65536, 128):
+        V = pats[a:a + 128].reshape(1, 1, 128).copy()
+        o, lse = oracle.attend(q, K, V)
+        assert np.array_equal(o[0], V[0, 0].astype(np.float64), equal_nan=True)
+        assert lse[0] == 0.0
