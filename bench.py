@@ -1,0 +1,395 @@
+#!/usr/bin/env python
+"""bench.py -- decode core-attention HBM GB/s and us per layer-step (BASELINE.json `metric`) on B200.
+
+A "step" is one pass of the whole hot path over one batch of synthetic input:
+    kf_token_boundary -> per layer { kf_kv_append -> kf_attend (split-KV attention + fused LSE merge) } -> kf_step_commit
+so the contexts grow by one token per step exactly as in decoding.  Default workload: cfg3 (configs[2] of
+BASELINE.json: B=16, Llama-3.1-8B shape, log-normal contexts with median 80K, 32K ranges over 8 partitions) -- the
+configuration the north_star target ">= 80% of peak HBM bandwidth at >= 32K context" is quoted on and the stand-in for
+the paper's serving trace.  `--workload cfg1|cfg2|cfg4|cfg5` selects the others.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference]
+
+N > 1 (torchrun): every rank runs an independent batch of the same recipe (seed + rank): the path shards over
+independent requests with no data-path collective -> "scaling": "weak"; NCCL is used only for the barrier and the
+max-over-ranks of the device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "decode_core_attention_hbm_gbps"
+UNIT = "GB/s"
+NOMINAL_PEAK_GBS = 8000.0        # BASELINE.json's "~8 TB/s" denominator (context)
+FALLBACK_PEAK_GBS = 6650.0       # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+
+# dram__bytes_read.sum + dram__bytes_write.sum per kf_attend launch from the committed `ncu --set full` capture
+# (profiles/r01_attend_tma_full.md); None where no capture exists for that workload.
+NCU_TRAFFIC_BYTES = {}
+
+
+def load_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    except Exception:
+        return FALLBACK_PEAK_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ---------------------------------------------------------------------------------------------------------
+def algorithmic_bytes(wl, lens_before, n_layers):
+    """Bytes the method must move in one step: per layer, every context token's
+    K and V rows (2*H_kv*128*2 B) + q read + appended K/V rows read and written + outputs written +
+    range partials written and re-read for requests with more than one range."""
+    per_tok = wl.kv_bytes_per_token()
+    B, Hq, Hkv, R = wl.batch, wl.n_q_heads, wl.n_kv_heads, wl.range_tokens
+    kv = sum((n + 1) * per_tok for n in lens_before)
+    q = B * Hq * 128 * 2
+    app = 2 * (2 * B * Hkv * 128 * 2)
+    out = B * Hq * (128 + 1) * 4
+    part = 0
+    for n in lens_before:
+        J = -(-(n + 1) // R)
+        if J > 1:
+            part += 2 * J * Hq * (128 + 1) * 4
+    return n_layers * (kv + q + app + out + part), n_layers * kv
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows, self.proc, self.gpu = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def mark(self):
+        return time.perf_counter()
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        time.sleep(0.06)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.06] or [r for (_, r) in self.rows[-3:]]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0]))
+                mx = float(f[1])
+                for n, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------------------
+def cpu_baseline_sample(wl, lens_before, step, budget_s=15.0):
+    """Time the fp64 oracle (as it stands) on the host cores, on a bounded sample of the same workload:
+    the shortest requests of the batch, all query heads, until ~budget_s of CPU work (estimated from a probe)."""
+    import numpy as np
+    import oracle
+    from kf_inputs import gen, gen_device
+    order = sorted(range(wl.batch), key=lambda r: lens_before[r])
+    # probe: one request-slice of 2048 tokens
+    r0 = order[0]
+    n0 = min(2048, lens_before[r0] + 1)
+    K = gen_device.fill(gen.STREAM_K, 0, r0, 0, n0, wl.n_kv_heads, seed=wl.seed).cpu().numpy()
+    V = gen_device.fill(gen.STREAM_V, 0, r0, 0, n0, wl.n_kv_heads, seed=wl.seed).cpu().numpy()
+    q = gen.gen_q(0, r0, step, wl.n_q_heads, wl.seed)
+    t = time.perf_counter()
+    oracle.attend(q, K, V)
+    rate = n0 / max(time.perf_counter() - t, 1e-6)          # tokens/s (all heads)
+    chosen, tok = [], 0
+    for r in order:
+        n = lens_before[r] + 1
+        if chosen and (tok + n) / rate > budget_s:
+            break
+        chosen.append(r)
+        tok += n
+    if tok / rate > 2 * budget_s:                              # a single huge request: take a prefix of its tokens
+        tok = int(rate * budget_s)
+        chosen = [(chosen[0], tok)]
+    else:
+        chosen = [(r, lens_before[r] + 1) for r in chosen]
+    data = []
+    for r, n in chosen:
+        K = gen_device.fill(gen.STREAM_K, 0, r, 0, n, wl.n_kv_heads, seed=wl.seed).cpu().numpy()
+        V = gen_device.fill(gen.STREAM_V, 0, r, 0, n, wl.n_kv_heads, seed=wl.seed).cpu().numpy()
+        data.append((gen.gen_q(0, r, step, wl.n_q_heads, wl.seed), K, V))
+    t = time.perf_counter()
+    for q, K, V in data:
+        oracle.attend(q, K, V)
+    dt = time.perf_counter() - t
+    nbytes = sum(n for _, n in chosen) * wl.kv_bytes_per_token()
+    return {"value": nbytes / dt / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{wl.name} layer 0 step {step}: requests {[r for r, _ in chosen]} "
+                      f"({sum(n for _, n in chosen)} context tokens, all {wl.n_q_heads} query heads), "
+                      f"oracle.attend fp64, {dt:.2f} s",
+            "seconds": dt}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, timed on the host cores on bounded samples (no GPU work
+    other than producing the seeded inputs with the generator's device twin when a GPU is present)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import numpy as np
+    import oracle
+    from kf_inputs import gen, workloads
+    wl = workloads.by_name(args.workload)
+    lens = [s - 1 for s in wl.contexts]
+    # bounded sample: a 4096-token prefix of the shortest request, all heads, per step
+    r = min(range(wl.batch), key=lambda i: lens[i])
+    n = min(4096, lens[r] + 1)
+    pos = np.arange(n)
+    K, V = gen.gen_k(0, r, pos, wl.n_kv_heads, wl.seed), gen.gen_v(0, r, pos, wl.n_kv_heads, wl.seed)
+    times = []
+    for step in range(args.warmup + args.steps):
+        q = gen.gen_q(0, r, step, wl.n_q_heads, wl.seed)
+        t = time.perf_counter()
+        oracle.attend(q, K, V)
+        if step >= args.warmup:
+            times.append(time.perf_counter() - t)
+    dt = sum(times) / len(times)
+    val = n * wl.kv_bytes_per_token() / dt / 1e9
+    sample = f"{wl.name}: request {r}, first {n} context tokens, all {wl.n_q_heads} heads, one layer, per step"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "note": wl.note, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "kind": "oracle", "cores": oracle.num_threads(), "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--attend-impl", type=int, default=0, help="KF_IMPL_*: 0 auto, 1 simple, 2 tma")
+    ap.add_argument("--layers-phys", type=int, default=0, help="physical layer pools (0 = auto)")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 50)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--min-tiles", type=int, default=0)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    from kf_inputs import workloads
+    from paper_2606_29207_b200.workload import Session
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    wl = workloads.by_name(args.workload)
+    wl.seed = wl.seed + rank                       # independent batch per rank (weak scaling)
+    n_layers = wl.n_layers
+    e2e_steps = args.e2e_steps or min(args.steps, 50)
+    total_steps = args.warmup + args.steps + e2e_steps + 2
+    if args.layers_phys:
+        L_phys = args.layers_phys
+    else:
+        free, _ = torch.cuda.mem_get_info(dev)
+        per_layer = wl.slots_per_partition(total_steps) * wl.n_partitions * wl.range_tokens * wl.kv_bytes_per_token()
+        L_phys = max(1, min(n_layers, int(0.85 * free // per_layer)))
+    ses = Session(wl, impl=args.attend_impl, n_layers_phys=L_phys, steps=total_steps, min_tiles=args.min_tiles,
+                  device=str(dev))
+    kf = ses.kf
+    ses.prepare()
+    assert kf.status() == 0
+
+    # per-step inputs, resident in HBM before the timed region (keyed by physical layer)
+    def inputs(step):
+        return [(ses.q_for(lp, step),) + ses.kv_new_for(lp, step) for lp in range(L_phys)]
+
+    lens = list(ses.len0)
+
+    def run_step(step_inputs, ev=None):
+        kf.token_boundary()
+        for layer in range(n_layers):
+            q, kn, vn = step_inputs[layer % L_phys]
+            kf.kv_append(layer % L_phys, kn, vn)
+            if ev is not None:
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                kf.attend(layer % L_phys, q, ses.o, ses.lse)
+                b.record()
+                ev.append((a, b))
+            else:
+                kf.attend(layer % L_phys, q, ses.o, ses.lse)
+        kf.step_commit()
+
+    step = 0
+    for _ in range(args.warmup):
+        run_step(inputs(step))
+        step += 1
+    timed_inputs = [inputs(step + i) for i in range(args.steps)] if n_layers * args.steps <= 4096 else None
+    total_bytes = kv_bytes = 0
+    for i in range(args.steps):
+        b, k = algorithmic_bytes(wl, [n + step + i for n in lens], n_layers)
+        total_bytes += b
+        kv_bytes += k
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.15)
+    torch.cuda.synchronize(dev)
+    if dist:
+        dist.barrier()
+    launches0 = kf.launch_count()
+    attend_events = []
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = sampler.mark()
+    e0.record()
+    for i in range(args.steps):
+        run_step(timed_inputs[i] if timed_inputs else inputs(step + i), attend_events)
+    e1.record()
+    torch.cuda.synchronize(dev)
+    t1 = sampler.mark()
+    if dist:
+        dist.barrier()
+    launches = kf.launch_count() - launches0
+    step += args.steps
+    ms = e0.elapsed_time(e1)
+    attend_ms = sum(a.elapsed_time(b) for a, b in attend_events) / len(attend_events)
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
+    assert kf.status() == 0
+    if dist:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        tb = torch.tensor([float(total_bytes), float(launches)], dtype=torch.float64, device=dev)
+        dist.all_reduce(tb, op=dist.ReduceOp.SUM)
+        total_bytes_all, launches_all = float(tb[0].item()), int(tb[1].item())
+    else:
+        total_bytes_all, launches_all = float(total_bytes), launches
+    value = total_bytes_all / (ms * 1e-3) / 1e9
+    ms_per_step = ms / args.steps
+
+    # ---- end to end: host buffers through kf_layer_step_host, copies inside the timed region -------------------
+    B, Hq, Hkv = wl.batch, wl.n_q_heads, wl.n_kv_heads
+    host_in = []
+    for i in range(e2e_steps):
+        host_in.append([tuple(t.cpu().pin_memory() for t in x) for x in inputs(step + i)])
+    o_h = torch.zeros((B, Hq, 128), dtype=torch.float32).pin_memory()
+    l_h = torch.zeros((B, Hq), dtype=torch.float32).pin_memory()
+    e2e_bytes = 0
+    for i in range(e2e_steps):
+        e2e_bytes += algorithmic_bytes(wl, [n + step + i for n in lens], n_layers)[0]
+    torch.cuda.synchronize(dev)
+    if dist:
+        dist.barrier()
+    e0.record()
+    for i in range(e2e_steps):
+        kf.token_boundary()
+        for layer in range(n_layers):
+            qh, kh, vh = host_in[i][layer % L_phys]
+            kf.layer_step_host(layer % L_phys, qh, kh, vh, o_h, l_h)
+        kf.step_commit()
+        torch.cuda.current_stream(dev).synchronize()      # the caller reads o_h / l_h every step
+    e1.record()
+    torch.cuda.synchronize(dev)
+    e2e_ms = e0.elapsed_time(e1)
+    if dist:
+        t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    step += e2e_steps
+    e2e_value = e2e_bytes * world / (e2e_ms * 1e-3) / 1e9
+    h2d = n_layers * (B * Hq * 128 * 2 + 2 * B * Hkv * 128 * 2)
+    d2h = n_layers * (B * Hq * 128 * 4 + B * Hq * 4)
+    assert kf.status() == 0
+
+    if rank != 0:
+        if dist:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = load_peak()
+    attend_bytes = total_bytes / (args.steps * n_layers)   # per kf_attend launch (append rows are ~1e-5 of it)
+    achieved = attend_bytes / (attend_ms * 1e-3) / 1e9
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline_sample(wl, [n + step for n in lens], step)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f16 storage, f32 accumulate", "data": "synthetic",
+        "config": {"workload": wl.name, "note": wl.note, "batch": B, "n_q_heads": Hq, "n_kv_heads": Hkv,
+                   "range_tokens": wl.range_tokens, "n_partitions": wl.n_partitions, "layers_logical": n_layers,
+                   "layers_physical": L_phys, "context_tokens_step0": sum(lens) + B,
+                   "l2": "inputs larger than L2 (KV read per layer-step >> 126 MB); no flush needed"
+                         if kv_bytes / (args.steps * n_layers) > 4 * 126e6 else
+                         "KV fits L2: numbers are L2-warm (see profiles for the cold protocol)",
+                   "attend_impl": {0: "tma", 1: "simple", 2: "tma"}[args.attend_impl]},
+        "us_per_layer_step": ms_per_step * 1e3 / n_layers,
+        "pct_of_nominal_8TBs": 100.0 * value / world / NOMINAL_PEAK_GBS,
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
+        "gpu_launches": launches_all,
+        "roofline": {"bound": "hbm", "kernel": "attend_tma_kernel" if args.attend_impl != 1 else "attend_simple_kernel",
+                     "achieved": achieved, "peak": peak, "unit": UNIT, "frac": achieved / peak,
+                     "traffic": NCU_TRAFFIC_BYTES.get(wl.name), "algorithmic_bytes_per_launch": attend_bytes,
+                     "avg_launch_ms": attend_ms, "peak_source": peak_src,
+                     "frac_of_nominal_8000": achieved / NOMINAL_PEAK_GBS},
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    if dist:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
