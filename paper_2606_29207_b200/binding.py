@@ -17,7 +17,7 @@ EXPORTS = [
     "kf_version", "kf_strerror", "kf_last_cuda_error", "kf_pool_bytes", "kf_workspace_bytes", "kf_pool_offset",
     "kf_create", "kf_destroy", "kf_open_request", "kf_close_request", "kf_load_context", "kf_token_boundary",
     "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_step_commit", "kf_layer_step_host",
-    "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count",
+    "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count", "kf_worker_times",
 ]
 
 
@@ -71,6 +71,7 @@ def load_library():
     L.kf_status.argtypes = [vp, vp]
     L.kf_plan_info.argtypes = [vp, ctypes.POINTER(i32), vp]
     L.kf_launch_count.argtypes, L.kf_launch_count.restype = [vp], i64
+    L.kf_worker_times.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i32), vp]
     for name in EXPORTS:
         if getattr(L, name).restype is None:
             getattr(L, name).restype = ctypes.c_int
@@ -243,6 +244,13 @@ class KFlume:
         self._check(self.lib.kf_plan_info(self.h, out, self._stream(stream)), "kf_plan_info")
         keys = ["n_units", "n_tiles", "n_workers", "n_pieces", "n_entries", "tile_tokens", "max_workers", "pad"]
         return dict(zip(keys, list(out)))
+
+    def worker_times(self, stream=None):
+        """[(smid, t_start, t_first, t_end)] in ns for every worker of the last attend launch."""
+        n = ctypes.c_int32(0)
+        buf = (ctypes.c_int64 * (2048 * 4))()
+        self._check(self.lib.kf_worker_times(self.h, buf, ctypes.byref(n), self._stream(stream)), "kf_worker_times")
+        return [tuple(buf[4 * i:4 * i + 4]) for i in range(n.value)]
 
     def launch_count(self) -> int:
         return int(self.lib.kf_launch_count(self.h))

@@ -30,7 +30,7 @@ inline size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a
 struct Layout {
     size_t len, n_ranges, route_part, route_slot, rr_cursor, free_head, free_cnt, free_stack, error, plan, units, spans,
         scratch, unit_counter, group_counter, piece_o, piece_lse, range_o, range_lse, stage_q, stage_k, stage_v,
-        stage_o, stage_lse, tmaps, total;
+        stage_o, stage_lse, tmaps, worker_times, total;
 };
 
 bool valid_config(const kf_config *c) {
@@ -93,6 +93,7 @@ Layout make_layout(const kf_config *c) {
     L.stage_o = take(B * Hq * kHeadDim * 4);
     L.stage_lse = take(B * Hq * 4);
     L.tmaps = take(P * 2 * 128);
+    L.worker_times = take((size_t)kMaxWorkers * 4 * 8);
     L.total = off;
     return L;
 }
@@ -279,6 +280,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.stage_o = (float *)(ws + L.stage_o);
     d.stage_lse = (float *)(ws + L.stage_lse);
     d.tmaps = ws + L.tmaps;
+    d.worker_times = (long long *)(ws + L.worker_times);
     d.v_off = half_pool_bytes(cfg);
     for (int p = 0; p < cfg->n_partitions; ++p) d.pool[p] = (unsigned char *)pool_ptrs[p];
 
@@ -459,5 +461,16 @@ int kf_plan_info(kf_ctx *ctx, int32_t *out, kf_stream stream) {
 }
 
 int64_t kf_launch_count(const kf_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int kf_worker_times(kf_ctx *ctx, int64_t *out, int32_t *n_workers, kf_stream stream) {
+    if (!ctx || !out || !n_workers) return KF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    *n_workers = ctx->dev.max_workers;
+    cudaError_t e = cudaMemcpyAsync(out, ctx->dev.worker_times, (size_t)ctx->dev.max_workers * 4 * 8,
+                                    cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return KF_OK;
+}
 
 }  // extern "C"

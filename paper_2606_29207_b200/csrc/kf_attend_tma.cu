@@ -82,6 +82,16 @@ __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {
     const __half2 h = __floats2half2_rn(lo, hi);
     return *reinterpret_cast<const uint32_t *>(&h);
 }
+__device__ __forceinline__ long long global_ns() {
+    long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ int sm_id() {
+    int v;
+    asm volatile("mov.u32 %0, %smid;" : "=r"(v));
+    return v;
+}
 __device__ __forceinline__ Unit load_unit(const Unit *units, int u) {
     const int4 *p = reinterpret_cast<const int4 *>(units + u);
     const int4 a = __ldg(p), b = __ldg(p + 1);
@@ -105,7 +115,15 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 1) attend_tma_kernel(const 
     const int w = blockIdx.x * kWarpsPerCta + warp;
     const Span sp = d.spans[w];
     const int n_tiles = sp.n_tiles;
-    if (n_tiles == 0) return;  // idle worker: safe, the kernel has no CTA-wide barrier
+    const long long t_start = global_ns();
+    long long t_first = 0;
+    if (n_tiles == 0) {  // idle worker: safe, the kernel has no CTA-wide barrier
+        if (lane == 0) {
+            d.worker_times[4 * w] = sm_id();
+            d.worker_times[4 * w + 1] = d.worker_times[4 * w + 2] = d.worker_times[4 * w + 3] = 0;
+        }
+        return;
+    }
 
     const uint32_t wbase = ((smem_u32(smem_raw) + 1023u) & ~1023u) + warp * kWarpSmem;
     const uint32_t bar0 = smem_u32(&bars[warp][0]);
@@ -184,6 +202,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 1) attend_tma_kernel(const 
         const int stage = i % kStages;
         const uint32_t sb = wbase + stage * kStageBytes;
         mbar_wait(bar0 + 8 * stage, (i / kStages) & 1);
+        if (i == 0) t_first = global_ns();
 
         const int valid = min(kTileTokens, cun.cnt - ct * kTileTokens);
         const bool ragged = valid < kTileTokens;
@@ -296,6 +315,12 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 1) attend_tma_kernel(const 
                 for (int n = 0; n < 16; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
             }
         }
+    }
+    if (lane == 0) {
+        d.worker_times[4 * w] = sm_id();
+        d.worker_times[4 * w + 1] = t_start;
+        d.worker_times[4 * w + 2] = t_first;
+        d.worker_times[4 * w + 3] = global_ns();
     }
 }
 

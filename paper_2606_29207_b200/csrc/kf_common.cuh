@@ -83,6 +83,7 @@ struct Dev {
     unsigned char *pool[kMaxPartitions];
     size_t v_off;        // byte offset of the V half of a pool
     const void *tmaps;   // [P][2] CUtensorMap (K, V) in device memory, 128-byte stride
+    long long *worker_times;  // [kMaxWorkers][4]: {smid, t_start, t_first_tile, t_end} (globaltimer ns), diagnostics
 };
 
 struct AttendParams {

@@ -61,46 +61,82 @@ __device__ __forceinline__ PieceDest piece_dest(const AttendParams &p, const Uni
 
 // One warp merges n partials of a head group: source partial j has o rows at src_o + j*o_stride + i*128 and
 // lse at src_lse[j*lse_stride + i], i < G.  Lane l owns columns [4l, 4l+4).  Loads bypass L1 (__ldcg): the
-// partials were written by other SMs in this same launch.
+// partials were written by other SMs in this same launch.  Four heads are reduced together and the inner loop
+// is unrolled so that ~16 independent 16-byte loads are in flight per lane (the merge is L2-latency bound).
+// The accumulation order is j ascending for every head, whoever calls this.
 __device__ __forceinline__ void warp_merge(const float *src_o, size_t o_stride, const float *src_lse,
                                            size_t lse_stride, int n, int G, float *dst_o, float *dst_lse,
                                            float *dst2_o, float *dst2_lse, int lane) {
-    for (int i = 0; i < G; ++i) {
-        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        float lse;
+    for (int i0 = 0; i0 < G; i0 += 4) {
+        const int nh = min(4, G - i0);
+        float4 acc[4];
+        float lse_h[4];
+#pragma unroll
+        for (int hh = 0; hh < 4; ++hh) {
+            acc[hh] = make_float4(0.f, 0.f, 0.f, 0.f);
+            lse_h[hh] = -INFINITY;
+        }
         if (n == 1) {  // exact copy
-            lse = __ldcg(src_lse + i);
-            acc = __ldcg(reinterpret_cast<const float4 *>(src_o + (size_t)i * kHeadDim) + lane);
+#pragma unroll
+            for (int hh = 0; hh < 4; ++hh) {
+                if (hh < nh) {
+                    lse_h[hh] = __ldcg(src_lse + i0 + hh);
+                    acc[hh] = __ldcg(reinterpret_cast<const float4 *>(src_o + (size_t)(i0 + hh) * kHeadDim) + lane);
+                }
+            }
         } else {
-            float M = -INFINITY;
-            for (int j = lane; j < n; j += 32) M = fmaxf(M, __ldcg(src_lse + (size_t)j * lse_stride + i));
-            M = warp_max(M);
-            if (M == -INFINITY) {
-                lse = -INFINITY;
-            } else {
-                float sum = 0.f;
-                for (int j = lane; j < n; j += 32) sum += expf(__ldcg(src_lse + (size_t)j * lse_stride + i) - M);
-                sum = warp_sum(sum);
-                lse = M + logf(sum);
-                for (int j = 0; j < n; ++j) {
-                    const float w = expf(__ldcg(src_lse + (size_t)j * lse_stride + i) - lse);
-                    if (w != 0.f) {
-                        const float4 v = __ldcg(
-                            reinterpret_cast<const float4 *>(src_o + (size_t)j * o_stride + (size_t)i * kHeadDim) +
-                            lane);
-                        acc.x = fmaf(w, v.x, acc.x);
-                        acc.y = fmaf(w, v.y, acc.y);
-                        acc.z = fmaf(w, v.z, acc.z);
-                        acc.w = fmaf(w, v.w, acc.w);
+#pragma unroll
+            for (int hh = 0; hh < 4; ++hh) {
+                if (hh < nh) {
+                    const float *lp = src_lse + i0 + hh;
+                    float M = -INFINITY;
+                    for (int j = lane; j < n; j += 32) M = fmaxf(M, __ldcg(lp + (size_t)j * lse_stride));
+                    M = warp_max(M);
+                    if (M != -INFINITY) {
+                        float sum = 0.f;
+                        for (int j = lane; j < n; j += 32) sum += expf(__ldcg(lp + (size_t)j * lse_stride) - M);
+                        sum = warp_sum(sum);
+                        lse_h[hh] = M + logf(sum);
+                    }
+                }
+            }
+            for (int jb = 0; jb < n; jb += 32) {
+                float wl[4];  // this lane's weights of partial jb + lane
+#pragma unroll
+                for (int hh = 0; hh < 4; ++hh) {
+                    wl[hh] = 0.f;
+                    if (hh < nh && jb + lane < n && lse_h[hh] != -INFINITY)
+                        wl[hh] = expf(__ldcg(src_lse + (size_t)(jb + lane) * lse_stride + i0 + hh) - lse_h[hh]);
+                }
+                const int cnt = min(32, n - jb);
+#pragma unroll 4
+                for (int jj = 0; jj < cnt; ++jj) {
+                    const float *row = src_o + (size_t)(jb + jj) * o_stride + (size_t)i0 * kHeadDim;
+#pragma unroll
+                    for (int hh = 0; hh < 4; ++hh) {
+                        const float w = __shfl_sync(0xffffffffu, wl[hh], jj);
+                        if (hh < nh) {
+                            float4 v = __ldcg(reinterpret_cast<const float4 *>(row + (size_t)hh * kHeadDim) + lane);
+                            if (w == 0.f) v = make_float4(0.f, 0.f, 0.f, 0.f);  // lse_j = -inf: ignore its o_j
+                            acc[hh].x = fmaf(w, v.x, acc[hh].x);
+                            acc[hh].y = fmaf(w, v.y, acc[hh].y);
+                            acc[hh].z = fmaf(w, v.z, acc[hh].z);
+                            acc[hh].w = fmaf(w, v.w, acc[hh].w);
+                        }
                     }
                 }
             }
         }
-        reinterpret_cast<float4 *>(dst_o + (size_t)i * kHeadDim)[lane] = acc;
-        if (lane == 0) dst_lse[i] = lse;
-        if (dst2_o) {
-            reinterpret_cast<float4 *>(dst2_o + (size_t)i * kHeadDim)[lane] = acc;
-            if (lane == 0) dst2_lse[i] = lse;
+#pragma unroll
+        for (int hh = 0; hh < 4; ++hh) {
+            if (hh < nh) {
+                reinterpret_cast<float4 *>(dst_o + (size_t)(i0 + hh) * kHeadDim)[lane] = acc[hh];
+                if (lane == 0) dst_lse[i0 + hh] = lse_h[hh];
+                if (dst2_o) {
+                    reinterpret_cast<float4 *>(dst2_o + (size_t)(i0 + hh) * kHeadDim)[lane] = acc[hh];
+                    if (lane == 0) dst2_lse[i0 + hh] = lse_h[hh];
+                }
+            }
         }
     }
 }
