@@ -25,10 +25,16 @@ struct kf_ctx {
 namespace {
 
 constexpr size_t kAlign = 256;
+constexpr int kDefaultWarps = 8, kDefaultStages = 3;
+constexpr int kDefaultFirstPct = 50, kDefaultDecayPct = 50;
+
+size_t max_chunks_of(const kf_config *c) {
+    return (size_t)c->max_requests * c->max_ranges_per_request * c->n_kv_heads + kChunkSlack;
+}
 inline size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t len, n_ranges, route_part, route_slot, rr_cursor, free_head, free_cnt, free_stack, error, plan, units, spans,
+    size_t len, n_ranges, route_part, route_slot, rr_cursor, free_head, free_cnt, free_stack, error, plan, units, chunks, sched,
         scratch, unit_counter, group_counter, piece_o, piece_lse, range_o, range_lse, stage_q, stage_k, stage_v,
         stage_o, stage_lse, tmaps, worker_times, total;
 };
@@ -48,8 +54,12 @@ bool valid_config(const kf_config *c) {
     if (!(c->softmax_scale >= 0.f) || !isfinite(c->softmax_scale)) return false;
     if (c->attend_impl < KF_IMPL_AUTO || c->attend_impl > KF_IMPL_TMA) return false;
     if (c->min_tiles_per_worker < 0) return false;
-    for (int i = 0; i < 4; ++i)
-        if (c->reserved[i]) return false;
+    if (c->workers_per_sm != 0 && c->workers_per_sm != 4 && c->workers_per_sm != 8) return false;
+    if (c->pipeline_stages != 0 &&
+        !attend_tma_shape_ok(c->workers_per_sm ? c->workers_per_sm : kDefaultWarps, c->pipeline_stages))
+        return false;
+    if (c->sched_first_pct < 0 || c->sched_first_pct > 100) return false;
+    if (c->sched_decay_pct < 0 || c->sched_decay_pct > 99) return false;
     // rows of one K (or V) half-pool must fit the int32 TMA coordinate
     const double rows = (double)c->n_layers * c->slots_per_partition * c->n_kv_heads * c->range_tokens;
     if (rows >= 2147483647.0) return false;
@@ -61,7 +71,7 @@ Layout make_layout(const kf_config *c) {
     Layout L;
     const size_t B = c->max_requests, J = c->max_ranges_per_request, P = c->n_partitions, Hq = c->n_q_heads,
                  Hkv = c->n_kv_heads, G = Hq / Hkv, S = c->slots_per_partition;
-    const size_t E = B * J, U = E * Hkv, max_piece_slots = 2 * (size_t)kMaxWorkers + 2;
+    const size_t E = B * J, U = E * Hkv, max_piece_slots = max_chunks_of(c);
     size_t off = 0;
     auto take = [&](size_t bytes) {
         const size_t o = off;
@@ -79,10 +89,11 @@ Layout make_layout(const kf_config *c) {
     L.error = take(4);
     L.plan = take(sizeof(PlanHeader));
     L.units = take(U * sizeof(Unit));
-    L.spans = take((size_t)kMaxWorkers * sizeof(Span));
-    L.scratch = take((B + B + (B + 1) + E + (E + 1) + kMaxWorkers) * 4);
-    L.unit_counter = take(U * 4);
-    L.group_counter = take(B * Hkv * 4);
+    L.chunks = take(max_piece_slots * sizeof(Chunk));
+    L.sched = take(8 * 4);
+    L.scratch = take((B + B + (B + 1) + E + (E + 1) + (E + 1) + 3 * ((size_t)kMaxLevels * E + 1)) * 4);
+    L.unit_counter = take(2 * U * 4);        // double-buffered by launch parity
+    L.group_counter = take(2 * B * Hkv * 4);
     L.piece_o = take(max_piece_slots * G * kHeadDim * 4);
     L.piece_lse = take(max_piece_slots * G * 4);
     L.range_o = take(E * Hq * kHeadDim * 4);
@@ -227,9 +238,11 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     e = cudaGetDeviceProperties(&prop, dev_id);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     ctx->sm_count = prop.multiProcessorCount;
-    ctx->n_ctas = ctx->sm_count;
-    if (ctx->n_ctas * kWarpsPerCta > kMaxWorkers) ctx->n_ctas = kMaxWorkers / kWarpsPerCta;
     ctx->impl = cfg->attend_impl == KF_IMPL_AUTO ? KF_IMPL_TMA : cfg->attend_impl;
+    // the CUDA-core kernel always runs 8 warps per CTA; the TMA kernel's shape is tunable
+    const int warps = ctx->impl == KF_IMPL_SIMPLE ? kWarpsPerCta : (cfg->workers_per_sm ? cfg->workers_per_sm : kDefaultWarps);
+    ctx->n_ctas = ctx->sm_count;
+    if (ctx->n_ctas * warps > kMaxWorkers) ctx->n_ctas = kMaxWorkers / warps;
     ctx->plan_dirty = true;
 
     unsigned char *ws = (unsigned char *)workspace;
@@ -251,8 +264,13 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.B = cfg->max_requests;
     d.Jmax = cfg->max_ranges_per_request;
     d.slots = cfg->slots_per_partition;
-    d.max_workers = ctx->n_ctas * kWarpsPerCta;
+    d.max_workers = ctx->n_ctas * warps;
     d.min_tiles = cfg->min_tiles_per_worker > 0 ? cfg->min_tiles_per_worker : 4;
+    d.warps_per_cta = warps;
+    d.stages = cfg->pipeline_stages ? cfg->pipeline_stages : kDefaultStages;
+    d.max_chunks = (int32_t)max_chunks_of(cfg);
+    d.sched_first = 0.01f * (cfg->sched_first_pct ? cfg->sched_first_pct : kDefaultFirstPct);
+    d.sched_decay = 0.01f * (cfg->sched_decay_pct ? cfg->sched_decay_pct : kDefaultDecayPct);
     const float scale = cfg->softmax_scale > 0.f ? cfg->softmax_scale : 1.0f / sqrtf((float)kHeadDim);
     d.scale_log2 = scale * 1.4426950408889634f;
     d.len = (int32_t *)(ws + L.len);
@@ -266,7 +284,8 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.error = (int32_t *)(ws + L.error);
     d.plan = (PlanHeader *)(ws + L.plan);
     d.units = (Unit *)(ws + L.units);
-    d.spans = (Span *)(ws + L.spans);
+    d.chunks = (Chunk *)(ws + L.chunks);
+    d.sched = (int32_t *)(ws + L.sched);
     d.scratch = (int32_t *)(ws + L.scratch);
     d.unit_counter = (int32_t *)(ws + L.unit_counter);
     d.group_counter = (int32_t *)(ws + L.group_counter);

@@ -1,5 +1,5 @@
 // kf_attend_simple.cu -- KF_IMPL_SIMPLE: CUDA-core split-KV decode attention over token-range partitions
-// (PAPER.md:137, :145).  One warp = one worker walking its span of the work plan; 128-bit coalesced loads of
+// (PAPER.md:137, :145).  One warp = one worker taking chunks of the work plan round-robin; 128-bit coalesced loads of
 // K rows, 64-bit coalesced loads of V rows, fp32 online softmax (base-2), warp-shuffle reductions.  It is the
 // plain reference GPU kernel: the TMA / tensor-core kernel (kf_attend_tma.cu) must agree with it.
 #include "kf_merge.cuh"
@@ -10,18 +10,19 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) attend_simple_kernel(Attend
     __shared__ float q_s[kWarpsPerCta][kMaxGroup * kHeadDim];
     const Dev &d = p.d;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int w = blockIdx.x * kWarpsPerCta + warp;
-    const Span sp = d.spans[w];
-    if (sp.n_tiles == 0) return;
+    const int W = gridDim.x * kWarpsPerCta;
+    const int n_chunks = d.plan->n_pieces;
+    const Counters ctr = launch_prologue(d, blockIdx.x * kWarpsPerCta + warp, W, lane);
     const int G = d.G;
     float *qs = q_s[warp];
 
-    int u = sp.unit, t0 = sp.tile_in_unit, piece = sp.piece, remaining = sp.n_tiles;
-    while (remaining > 0) {
+    // static round-robin over the chunk list (one chunk = one piece of one unit)
+    for (int c = blockIdx.x * kWarpsPerCta + warp; c < n_chunks; c += W) {
+        const Chunk ch = d.chunks[c];
+        const int u = ch.unit, piece = ch.piece;
         const Unit un = d.units[u];
         const int g = u % d.Hkv;
-        const int ntiles = (un.cnt + kTileTokens - 1) / kTileTokens;
-        const int t1 = min(ntiles, t0 + remaining);
+        const int t0 = ch.tile_begin, t1 = ch.tile_begin + ch.n_tiles;
         if ((p.part_mask >> un.part) & 1ull) {
             const __half *qg = p.q + ((size_t)un.req * d.Hq + (size_t)g * G) * kHeadDim;
             __syncwarp();
@@ -124,13 +125,11 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) attend_simple_kernel(Attend
                     }
                 }
             }
-            if (p.fused) finish_piece(p, u, un, g, lane);
+            if (p.fused) piece_done(p, ctr, u, un, g, lane);
         }
-        remaining -= t1 - t0;
-        t0 = 0;
-        ++u;
-        ++piece;
     }
+    if (p.fused) merge_phase(p, ctr, W, lane);
+    launch_epilogue(d, W, lane);
 }
 
 int launch_attend_simple(const AttendParams &p, int n_ctas, cudaStream_t s) {

@@ -22,11 +22,10 @@
 
 namespace kf {
 
-constexpr int kStages = 3;
 constexpr int kSubTile = kTileTokens * 128;     // 16 rows x 128 B (64 halfs): one TMA box
 constexpr int kStageBytes = 4 * kSubTile;       // K lo | K hi | V lo | V hi = 8 KB
-constexpr int kWarpSmem = kStages * kStageBytes;
-constexpr int kTmaSmemBytes = kWarpsPerCta * kWarpSmem + 1024;
+constexpr int kTicketAhead = 3;                 // tiles before the end of a chunk at which the next ticket is taken
+constexpr int kRing = 8;                        // chunk descriptors in flight between the load and compute cursors
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -107,182 +106,216 @@ __device__ __forceinline__ Unit load_unit(const Unit *units, int u) {
     return un;
 }
 
-__global__ void __launch_bounds__(kWarpsPerCta * 32, 1) attend_tma_kernel(const AttendParams p) {
+
+template <int WARPS, int STAGES>
+__global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendParams p) {
+    constexpr int kWarpSmem = STAGES * kStageBytes;
     extern __shared__ unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t bars[kWarpsPerCta][kStages];
+    __shared__ __align__(8) uint64_t bars[WARPS][STAGES];
+    __shared__ int4 ring[WARPS][kRing];
     const Dev &d = p.d;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int w = blockIdx.x * kWarpsPerCta + warp;
-    const Span sp = d.spans[w];
-    const int n_tiles = sp.n_tiles;
+    const int W = gridDim.x * WARPS;
+    const int w = blockIdx.x * WARPS + warp;
+    const int n_chunks = __ldg(&d.plan->n_pieces);
     const long long t_start = global_ns();
-    long long t_first = 0;
-    if (n_tiles == 0) {  // idle worker: safe, the kernel has no CTA-wide barrier
+    long long t_first = 0, t_stream = 0;
+    const Counters ctr = launch_prologue(d, w, W, lane);
+
+    if (w < n_chunks) {
+        const uint32_t wbase = ((smem_u32(smem_raw) + 1023u) & ~1023u) + warp * kWarpSmem;
+        const uint32_t bar0 = smem_u32(&bars[warp][0]);
         if (lane == 0) {
-            d.worker_times[4 * w] = sm_id();
-            d.worker_times[4 * w + 1] = d.worker_times[4 * w + 2] = d.worker_times[4 * w + 3] = 0;
-        }
-        return;
-    }
-
-    const uint32_t wbase = ((smem_u32(smem_raw) + 1023u) & ~1023u) + warp * kWarpSmem;
-    const uint32_t bar0 = smem_u32(&bars[warp][0]);
-    if (lane == 0) {
 #pragma unroll
-        for (int s = 0; s < kStages; ++s) mbar_init(bar0 + 8 * s, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
-    __syncwarp();
-
-    const int G = d.G, Hkv = d.Hkv;
-    const int row_stride_unit = d.R;  // rows per (slot, kv head)
-    const unsigned char *tmaps = reinterpret_cast<const unsigned char *>(d.tmaps);
-
-    // ---- load cursor (runs kStages tiles ahead of the compute cursor) --------------------------------
-    int lu = sp.unit, lt = sp.tile_in_unit, l_left = n_tiles;
-    Unit lun = load_unit(d.units, lu);
-    int l_ntiles = (lun.cnt + kTileTokens - 1) / kTileTokens;
-    int l_rowbase = ((p.layer * d.slots + lun.slot) * Hkv + (lu % Hkv)) * row_stride_unit;
-    auto issue_tile = [&](int stage) {
-        if (lane == 0) {
-            const uint32_t sb = wbase + stage * kStageBytes, bar = bar0 + 8 * stage;
-            const int row = l_rowbase + lt * kTileTokens;
-            const unsigned char *tk = tmaps + (size_t)lun.part * 256;
-            mbar_expect_tx(bar, kStageBytes);
-            tma_load_2d(sb, tk, 0, row, bar);
-            tma_load_2d(sb + kSubTile, tk, 64, row, bar);
-            tma_load_2d(sb + 2 * kSubTile, tk + 128, 0, row, bar);
-            tma_load_2d(sb + 3 * kSubTile, tk + 128, 64, row, bar);
+            for (int s = 0; s < STAGES; ++s) mbar_init(bar0 + 8 * s, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         }
-        ++lt;
-        --l_left;
-        if (lt == l_ntiles && l_left > 0) {
-            ++lu;
-            lt = 0;
-            lun = load_unit(d.units, lu);
-            l_ntiles = (lun.cnt + kTileTokens - 1) / kTileTokens;
-            l_rowbase = ((p.layer * d.slots + lun.slot) * Hkv + (lu % Hkv)) * row_stride_unit;
-        }
-    };
-#pragma unroll
-    for (int s = 0; s < kStages; ++s)
-        if (s < n_tiles) issue_tile(s);
+        __syncwarp();
 
-    // ---- per-lane shared-memory offsets of the ldmatrix rows (128B hardware swizzle: chunk ^= row & 7) ----
-    const int l7 = lane & 7, mi = lane >> 3;
-    const uint32_t k_row = l7 * 128;
-    const uint32_t k_x0 = ((mi) ^ l7) << 4, k_x1 = ((4 + mi) ^ l7) << 4;
-    const uint32_t v_row = ((mi & 1) * 8 + l7) * 128;
-    const int v_c = mi >> 1;
-    const int qrow = lane >> 2, qcol = (lane & 3) * 2;
+        const int G = d.G, Hkv = d.Hkv;
+        const unsigned char *tmaps = reinterpret_cast<const unsigned char *>(d.tmaps);
 
-    // ---- compute cursor ------------------------------------------------------------------------------
-    int cu = sp.unit, ct = sp.tile_in_unit, piece = sp.piece;
-    Unit cun = load_unit(d.units, cu);
-    int c_ntiles = (cun.cnt + kTileTokens - 1) / kTileTokens;
-
-    uint32_t qa[8][2];  // A fragments of Q: [k-step][a0, a2]
-    auto load_q = [&]() {
-        const __half *qg = p.q + ((size_t)cun.req * d.Hq + (size_t)(cu % Hkv) * G + qrow) * kHeadDim + qcol;
-#pragma unroll
-        for (int ks = 0; ks < 8; ++ks) {
-            qa[ks][0] = qrow < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16)) : 0u;
-            qa[ks][1] = qrow < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16 + 8)) : 0u;
-        }
-    };
-    load_q();
-
-    float o[16][4];
-    float m_run = -INFINITY, l_run = 0.f;
-#pragma unroll
-    for (int n = 0; n < 16; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
-
-    for (int i = 0; i < n_tiles; ++i) {
-        const int stage = i % kStages;
-        const uint32_t sb = wbase + stage * kStageBytes;
-        mbar_wait(bar0 + 8 * stage, (i / kStages) & 1);
-        if (i == 0) t_first = global_ns();
-
-        const int valid = min(kTileTokens, cun.cnt - ct * kTileTokens);
-        const bool ragged = valid < kTileTokens;
-        if (ragged) {
-            // rows >= valid hold whatever the pool holds (maybe NaN patterns): zero them in V so 0 * V = 0
-            for (int idx = lane; idx < (kTileTokens - valid) * 16; idx += 32) {
-                const int row = valid + (idx >> 4), rem = idx & 15;
-                const uint32_t a = sb + 2 * kSubTile + (rem >> 3) * kSubTile + row * 128 + (rem & 7) * 16;
-                asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
+        // ---- load cursor: runs up to STAGES tiles ahead of the compute cursor, across chunk boundaries ----
+        int issued = 0, consumed = 0;
+        int l_left = 0, l_row = 0, l_part = 0;
+        int ring_w = 0, ring_r = 0;
+        int pre = 0;  // lane 0: ticket of the dynamic part of the chunk list, taken shortly before it is needed
+        bool l_first = true, l_done = false, has_pre = false;
+        auto grab = [&]() -> bool {
+            for (;;) {
+                int id;
+                if (l_first) {
+                    id = w;  // the first W chunks are handed out statically: no atomic storm at launch
+                    l_first = false;
+                } else {
+                    if (!has_pre && lane == 0) pre = atomicAdd(d.sched, 1);
+                    has_pre = false;
+                    id = W + __shfl_sync(0xffffffffu, pre, 0);
+                }
+                if (id >= n_chunks) {
+                    l_done = true;
+                    return false;
+                }
+                const int4 c4 = __ldg(reinterpret_cast<const int4 *>(d.chunks + id));
+                const Unit un = load_unit(d.units, c4.x);
+                if (!((p.part_mask >> un.part) & 1ull)) continue;  // partition not selected: nothing to load
+                l_left = c4.z;
+                l_part = un.part;
+                l_row = ((p.layer * d.slots + un.slot) * Hkv + (c4.x % Hkv)) * d.R + c4.y * kTileTokens;
+                if (lane == 0) ring[warp][ring_w & (kRing - 1)] = c4;
+                ++ring_w;
+                return true;
             }
-            __syncwarp();
-        }
+        };
+        auto try_issue = [&]() {
+            if (l_done) return;
+            if (l_left == 0 && !grab()) return;
+            if (lane == 0) {
+                const int stage = issued % STAGES;
+                const uint32_t sb = wbase + stage * kStageBytes, bar = bar0 + 8 * stage;
+                const unsigned char *tk = tmaps + (size_t)l_part * 256;
+                mbar_expect_tx(bar, kStageBytes);
+                tma_load_2d(sb, tk, 0, l_row, bar);
+                tma_load_2d(sb + kSubTile, tk, 64, l_row, bar);
+                tma_load_2d(sb + 2 * kSubTile, tk + 128, 0, l_row, bar);
+                tma_load_2d(sb + 3 * kSubTile, tk + 128, 64, l_row, bar);
+            }
+            l_row += kTileTokens;
+            --l_left;
+            ++issued;
+            // take the next ticket a few tiles before the end of this chunk: late enough that a slow worker does
+            // not reserve work long before it can start it, early enough to hide the atomic's round trip
+            if (l_left == kTicketAhead - 1 || (l_left < kTicketAhead - 1 && !has_pre && l_left >= 0)) {
+                if (!has_pre) {
+                    if (lane == 0) pre = atomicAdd(d.sched, 1);
+                    has_pre = true;
+                }
+            }
+        };
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) try_issue();
 
-        // ---- S = Q K^T : 16 (heads, padded) x 16 tokens ------------------------------------------------
-        float s[2][4];
+        // ---- per-lane shared-memory offsets of the ldmatrix rows (128B hardware swizzle: chunk ^= row & 7) ----
+        const int l7 = lane & 7, mi = lane >> 3;
+        const uint32_t k_row = l7 * 128;
+        const uint32_t k_x0 = ((mi) ^ l7) << 4, k_x1 = ((4 + mi) ^ l7) << 4;
+        const uint32_t v_row = ((mi & 1) * 8 + l7) * 128;
+        const int v_c = mi >> 1;
+        const int qrow = lane >> 2, qcol = (lane & 3) * 2;
+
+        // ---- compute cursor ------------------------------------------------------------------------------
+        int cu = 0, ct = 0, c_left = 0, piece = 0;
+        Unit cun;
+        cun.cnt = 0;
+        uint32_t qa[8][2];  // A fragments of Q: [k-step][a0, a2]
+        float o[16][4];
+        float m_run = -INFINITY, l_run = 0.f;
+
+        while (consumed < issued) {
+            if (c_left == 0) {
+                // ---- next chunk (= one piece of one unit) ----
+                __syncwarp();
+                const int4 c4 = ring[warp][ring_r & (kRing - 1)];
+                ++ring_r;
+                cu = c4.x;
+                ct = c4.y;
+                c_left = c4.z;
+                piece = c4.w;
+                cun = load_unit(d.units, cu);
+                const __half *qg = p.q + ((size_t)cun.req * d.Hq + (size_t)(cu % Hkv) * G + qrow) * kHeadDim + qcol;
 #pragma unroll
-        for (int j = 0; j < 2; ++j) s[j][0] = s[j][1] = s[j][2] = s[j][3] = 0.f;
+                for (int ks = 0; ks < 8; ++ks) {
+                    qa[ks][0] = qrow < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16)) : 0u;
+                    qa[ks][1] = qrow < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16 + 8)) : 0u;
+                }
+                m_run = -INFINITY;
+                l_run = 0.f;
 #pragma unroll
-        for (int ii = 0; ii < 4; ++ii) {
+                for (int n = 0; n < 16; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
+            }
+            const int stage = consumed % STAGES;
+            const uint32_t sb = wbase + stage * kStageBytes;
+            mbar_wait(bar0 + 8 * stage, (consumed / STAGES) & 1);
+            if (consumed == 0) t_first = global_ns();
+
+            const int valid = min(kTileTokens, cun.cnt - ct * kTileTokens);
+            const bool ragged = valid < kTileTokens;
+            if (ragged) {
+                // rows >= valid hold whatever the pool holds (maybe NaN patterns): zero them in V so 0 * V = 0
+                for (int idx = lane; idx < (kTileTokens - valid) * 16; idx += 32) {
+                    const int row = valid + (idx >> 4), rem = idx & 15;
+                    const uint32_t a = sb + 2 * kSubTile + (rem >> 3) * kSubTile + row * 128 + (rem & 7) * 16;
+                    asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
+                }
+                __syncwarp();
+            }
+
+            // ---- S = Q K^T : 16 (heads, padded) x 16 tokens ------------------------------------------------
+            float s[2][4];
+#pragma unroll
+            for (int j = 0; j < 2; ++j) s[j][0] = s[j][1] = s[j][2] = s[j][3] = 0.f;
+#pragma unroll
+            for (int ii = 0; ii < 4; ++ii) {
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    uint32_t b0, b1, b2, b3;
+                    ldsm_x4(sb + (ii >> 1) * kSubTile + j * 1024 + k_row + ((ii & 1) ? k_x1 : k_x0), b0, b1, b2, b3);
+                    mma16816(s[j], qa[2 * ii][0], qa[2 * ii][1], b0, b1);
+                    mma16816(s[j], qa[2 * ii + 1][0], qa[2 * ii + 1][1], b2, b3);
+                }
+            }
+
+            // ---- online softmax on row `qrow` (c0, c1 of each n-tile), base 2 ------------------------------
+            float mx = -INFINITY;
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const float v = s[j][e] * d.scale_log2;
+                    s[j][e] = (8 * j + qcol + e < valid) ? v : -INFINITY;
+                    mx = fmaxf(mx, s[j][e]);
+                }
+            }
+            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
+            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
+            const float m_new = fmaxf(m_run, mx);
+            const float alpha = fast_exp2(m_run - m_new);
+            const float p00 = fast_exp2(s[0][0] - m_new), p01 = fast_exp2(s[0][1] - m_new);
+            const float p10 = fast_exp2(s[1][0] - m_new), p11 = fast_exp2(s[1][1] - m_new);
+            l_run = l_run * alpha + ((p00 + p01) + (p10 + p11));
+            m_run = m_new;
+            if (__any_sync(0xffffffffu, alpha != 1.f)) {
+#pragma unroll
+                for (int n = 0; n < 16; ++n) {
+                    o[n][0] *= alpha;
+                    o[n][1] *= alpha;
+                }
+            }
+            const uint32_t pa0 = pack_half2(p00, p01), pa2 = pack_half2(p10, p11);
+
+            // ---- O += P V : 16 x 128 -----------------------------------------------------------------------
+#pragma unroll
+            for (int nd = 0; nd < 16; nd += 2) {
                 uint32_t b0, b1, b2, b3;
-                ldsm_x4(sb + (ii >> 1) * kSubTile + j * 1024 + k_row + ((ii & 1) ? k_x1 : k_x0), b0, b1, b2, b3);
-                mma16816(s[j], qa[2 * ii][0], qa[2 * ii][1], b0, b1);
-                mma16816(s[j], qa[2 * ii + 1][0], qa[2 * ii + 1][1], b2, b3);
+                ldsm_x4_trans(sb + 2 * kSubTile + (nd >> 3) * kSubTile + v_row + ((((nd & 7) + v_c) ^ l7) << 4), b0, b1,
+                              b2, b3);
+                mma16816(o[nd], pa0, pa2, b0, b1);
+                mma16816(o[nd + 1], pa0, pa2, b2, b3);
             }
-        }
 
-        // ---- online softmax on row `qrow` (c0, c1 of each n-tile), base 2 ------------------------------
-        float mx = -INFINITY;
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-#pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                const float v = s[j][e] * d.scale_log2;
-                s[j][e] = (8 * j + qcol + e < valid) ? v : -INFINITY;
-                mx = fmaxf(mx, s[j][e]);
-            }
-        }
-        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
-        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
-        const float m_new = fmaxf(m_run, mx);
-        const float alpha = fast_exp2(m_run - m_new);
-        const float p00 = fast_exp2(s[0][0] - m_new), p01 = fast_exp2(s[0][1] - m_new);
-        const float p10 = fast_exp2(s[1][0] - m_new), p11 = fast_exp2(s[1][1] - m_new);
-        l_run = l_run * alpha + ((p00 + p01) + (p10 + p11));
-        m_run = m_new;
-        if (__any_sync(0xffffffffu, alpha != 1.f)) {
-#pragma unroll
-            for (int n = 0; n < 16; ++n) {
-                o[n][0] *= alpha;
-                o[n][1] *= alpha;
-            }
-        }
-        const uint32_t pa0 = pack_half2(p00, p01), pa2 = pack_half2(p10, p11);
-
-        // ---- O += P V : 16 x 128 -----------------------------------------------------------------------
-#pragma unroll
-        for (int nd = 0; nd < 16; nd += 2) {
-            uint32_t b0, b1, b2, b3;
-            ldsm_x4_trans(sb + 2 * kSubTile + (nd >> 3) * kSubTile + v_row + ((((nd & 7) + v_c) ^ l7) << 4), b0, b1, b2,
-                          b3);
-            mma16816(o[nd], pa0, pa2, b0, b1);
-            mma16816(o[nd + 1], pa0, pa2, b2, b3);
-        }
-
-        __syncwarp();  // every lane is done reading this stage
-        if (i + kStages < n_tiles) {
+            __syncwarp();  // every lane is done reading this stage
             if (ragged && lane == 0) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            issue_tile(stage);
-        }
+            try_issue();   // refills this very stage: issued == consumed + STAGES whenever it issues
 
-        ++ct;
-        if (ct == c_ntiles || i == n_tiles - 1) {
-            // ---- end of a piece: emit its partial (o, lse) --------------------------------------------
-            const int g = cu % Hkv;
-            float lt = l_run + __shfl_xor_sync(0xffffffffu, l_run, 1);
-            lt += __shfl_xor_sync(0xffffffffu, lt, 2);
-            const bool selected = (p.part_mask >> cun.part) & 1ull;
-            if (selected) {
+            ++consumed;
+            ++ct;
+            --c_left;
+            if (c_left == 0) {
+                // ---- end of the piece: emit its partial (o, lse) -------------------------------------------
+                const int g = cu % Hkv;
+                float lt = l_run + __shfl_xor_sync(0xffffffffu, l_run, 1);
+                lt += __shfl_xor_sync(0xffffffffu, lt, 2);
                 const PieceDest pd = piece_dest(p, cun, cu, g, piece);
                 if (qrow < G) {
                     const float inv = 1.f / lt;
@@ -300,38 +333,63 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32, 1) attend_tma_kernel(const 
                         if ((lane & 3) == 0) pd.lse2[qrow] = lse;
                     }
                 }
-                if (p.fused) finish_piece(p, cu, cun, g, lane);
-            }
-            if (i + 1 < n_tiles) {
-                ++cu;
-                ct = 0;
-                ++piece;
-                cun = load_unit(d.units, cu);
-                c_ntiles = (cun.cnt + kTileTokens - 1) / kTileTokens;
-                load_q();
-                m_run = -INFINITY;
-                l_run = 0.f;
-#pragma unroll
-                for (int n = 0; n < 16; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
+                if (p.fused) piece_done(p, ctr, cu, cun, g, lane);
             }
         }
+        t_stream = global_ns();
     }
+    if (p.fused) merge_phase(p, ctr, W, lane);
+
     if (lane == 0) {
-        d.worker_times[4 * w] = sm_id();
-        d.worker_times[4 * w + 1] = t_start;
+        // diagnostics: {SM | stream-end offset << 8, start, first tile ready, end}
+        d.worker_times[4 * w] = sm_id() | ((w < n_chunks ? t_stream - t_start : 0) << 8);
+        d.worker_times[4 * w + 1] = w < n_chunks ? t_start : 0;
         d.worker_times[4 * w + 2] = t_first;
-        d.worker_times[4 * w + 3] = global_ns();
+        d.worker_times[4 * w + 3] = w < n_chunks ? global_ns() : 0;
     }
+    launch_epilogue(d, W, lane);
+}
+
+template <int WARPS, int STAGES>
+static int setup_one() {
+    const int smem = WARPS * STAGES * kStageBytes + 1024;
+    return cudaFuncSetAttribute(attend_tma_kernel<WARPS, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) ==
+                   cudaSuccess
+               ? 0
+               : KF_ECUDA;
+}
+
+template <int WARPS, int STAGES>
+static int launch_one(const AttendParams &p, int n_ctas, cudaStream_t s) {
+    const int smem = WARPS * STAGES * kStageBytes + 1024;
+    attend_tma_kernel<WARPS, STAGES><<<n_ctas, WARPS * 32, smem, s>>>(p);
+    return 1;
+}
+
+#define KF_TMA_SHAPES(X) X(4, 2) X(4, 3) X(4, 4) X(4, 5) X(4, 6) X(8, 2) X(8, 3)
+
+bool attend_tma_shape_ok(int warps, int stages) {
+#define X(Wp, St) \
+    if (warps == Wp && stages == St) return true;
+    KF_TMA_SHAPES(X)
+#undef X
+    return false;
 }
 
 int attend_tma_setup() {
-    cudaError_t e = cudaFuncSetAttribute(attend_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTmaSmemBytes);
-    return e == cudaSuccess ? 0 : KF_ECUDA;
+    int rc = 0;
+#define X(Wp, St) rc |= setup_one<Wp, St>();
+    KF_TMA_SHAPES(X)
+#undef X
+    return rc == 0 ? 0 : KF_ECUDA;
 }
 
 int launch_attend_tma(const AttendParams &p, int n_ctas, cudaStream_t s) {
-    attend_tma_kernel<<<n_ctas, kWarpsPerCta * 32, kTmaSmemBytes, s>>>(p);
-    return 1;
+#define X(Wp, St) \
+    if (p.d.warps_per_cta == Wp && p.d.stages == St) return launch_one<Wp, St>(p, n_ctas, s);
+    KF_TMA_SHAPES(X)
+#undef X
+    return KF_EINVAL;
 }
 
 }  // namespace kf

@@ -12,8 +12,11 @@ namespace kf {
 
 constexpr int kHeadDim = 128;
 constexpr int kTileTokens = 16;       // work-plan granule = one MMA k-step of tokens
-constexpr int kWarpsPerCta = 8;       // one worker = one warp
-constexpr int kMaxWorkers = 2048;     // >= SMs * kWarpsPerCta on any Blackwell part (148 * 8 = 1184)
+constexpr int kWarpsPerCta = 8;       // default workers (warps) per CTA; one worker = one warp
+constexpr int kMaxWarpsPerCta = 8;
+constexpr int kMaxWorkers = 2048;     // >= SMs * kMaxWarpsPerCta on any Blackwell part (148 * 8 = 1184)
+constexpr int kMaxLevels = 16;        // levels of the guided self-scheduling chunk list
+constexpr int kChunkSlack = 16 * kMaxWorkers;  // chunk capacity = units + kChunkSlack
 constexpr int kMaxGroup = 8;          // G = H_q / H_kv
 constexpr int kMaxPartitions = 64;
 
@@ -24,28 +27,31 @@ struct Unit {
     int32_t part;
     int32_t slot;
     int32_t cnt;         // tokens of this range attended in this step (1..R)
-    int32_t tile_begin;  // first global tile index of this unit
-    int32_t piece_begin; // first global piece index of this unit
-    int32_t n_pieces;    // pieces (worker spans intersecting this unit)
+    int32_t tile_begin;  // first global tile index of this unit (unit-major order; informational)
+    int32_t piece_begin; // first global piece index of this unit (pieces of a unit are consecutive, tile order)
+    int32_t n_pieces;    // pieces = chunks this unit is cut into
 };
 
-// Contiguous span of global tiles given to one worker (warp): stream-K style equal split.
-struct Span {
-    int32_t unit;         // unit holding the first tile
-    int32_t tile_in_unit; // index of the first tile inside that unit
-    int32_t n_tiles;      // 0 => idle worker
-    int32_t piece;        // global piece index of the first piece
+// One chunk of work = one piece: a contiguous run of 16-token tiles inside ONE unit.  The chunk list is
+// ordered by scheduling level (big chunks first, small chunks last: guided self-scheduling) and consumed
+// through an atomic counter, so fast SMs take more chunks; the cuts themselves are static, which keeps the
+// reduction order -- and therefore the result bits -- independent of which worker ran which chunk.
+struct Chunk {
+    int32_t unit;
+    int32_t tile_begin; // first tile inside the unit
+    int32_t n_tiles;    // >= 1
+    int32_t piece;      // global piece index (unit-major)
 };
 
 struct PlanHeader {
     int32_t n_units;
     int32_t n_tiles;
-    int32_t n_workers; // active workers
-    int32_t n_pieces;
+    int32_t n_workers; // workers that get at least one chunk = min(max_workers, n_chunks)
+    int32_t n_pieces;  // = number of chunks
     int32_t n_entries; // (request, range) entries = n_units / H_kv
     int32_t tile_tokens;
     int32_t max_workers;
-    int32_t pad;
+    int32_t n_levels;
 };
 
 // Device pointers into the caller's workspace + immutable config.  Passed BY VALUE to every kernel.
@@ -53,6 +59,9 @@ struct Dev {
     // config
     int32_t Hq, Hkv, G, L, R, P, B, Jmax, slots;
     int32_t max_workers, min_tiles;
+    int32_t warps_per_cta, stages;      // launch shape of the attend kernels
+    int32_t max_chunks;                 // capacity of chunks[] and of the piece buffers
+    float sched_first, sched_decay;     // GSS factor rho (chunk <= rho * remaining / workers); share of a unit's remaining tiles per level
     float scale_log2;  // softmax_scale * log2(e)
     // routing state
     int32_t *len;        // [B]   -1 = closed
@@ -67,13 +76,15 @@ struct Dev {
     // work plan
     PlanHeader *plan;
     Unit *units;            // [B*Jmax*Hkv]
-    Span *spans;            // [kMaxWorkers]
-    int32_t *scratch;       // plan scratch: [B] J, [B] S, [B+1] entry prefix, [E+1] tile prefix, [E] tiles, [W] cuts
+    Chunk *chunks;          // [max_chunks]
+    int32_t *sched;         // [0] chunk counter (dynamic part of the list), [1] finished-worker counter
+    int32_t *scratch;       // plan scratch: [B] J, [B] S, [B+1] entry prefix, [E] tiles, [E+1] tile prefix,
+                            //               [E+1] piece prefix, [kMaxLevels*E+1] chunk prefix
     int32_t *unit_counter;  // [B*Jmax*Hkv]  last-arriver counters (self-resetting)
     int32_t *group_counter; // [B*Hkv]
     // partial buffers
-    float *piece_o;   // [max_pieces][G][128]
-    float *piece_lse; // [max_pieces][G]
+    float *piece_o;   // [max_chunks][G][128]
+    float *piece_lse; // [max_chunks][G]
     float *range_o;   // [B][Jmax][Hq][128]  scratch when the caller passes no o_part
     float *range_lse; // [B][Jmax][Hq]
     // staging for kf_layer_step_host
@@ -117,6 +128,7 @@ int launch_load_context(const Dev &d, int layer, int req, int tok_begin, int n_t
 int launch_kv_append(const Dev &d, int layer, const __half *k_new, const __half *v_new, cudaStream_t s);
 int launch_attend_simple(const AttendParams &p, int n_ctas, cudaStream_t s);
 int launch_attend_tma(const AttendParams &p, int n_ctas, cudaStream_t s);
+bool attend_tma_shape_ok(int warps, int stages);
 int attend_tma_setup();  // cudaFuncSetAttribute for the dynamic shared memory; 0 or KF_ECUDA
 int launch_merge_units(const AttendParams &p, int n_ctas, cudaStream_t s);
 int launch_merge_ranges(const Dev &d, const float *o_part, const float *lse_part, float *o, float *lse,

@@ -31,12 +31,8 @@ __device__ __forceinline__ size_t range_row(const Dev &d, int req, int range, in
     return ((size_t)req * d.Jmax + range) * d.Hq + head;
 }
 
-// Pieces of a unit cut by c >= 1 span boundaries use piece-buffer slots 2*cb .. 2*cb + c, where cb = cuts before
-// the unit = piece_begin - u: slots of different units never overlap and at most 2*workers + 1 slots are used.
-__device__ __forceinline__ int piece_slot(const Unit &un, int u, int piece) {
-    return 2 * (un.piece_begin - u) + (piece - un.piece_begin);
-}
-
+// A unit cut into several pieces keeps them in the piece buffer at their global piece index (consecutive for
+// one unit, tile order); a unit that is one piece writes its range partial directly.
 __device__ __forceinline__ PieceDest piece_dest(const AttendParams &p, const Unit &un, int u, int g, int piece) {
     const Dev &d = p.d;
     PieceDest pd;
@@ -52,146 +48,225 @@ __device__ __forceinline__ PieceDest piece_dest(const AttendParams &p, const Uni
             pd.lse2 = p.lse + frow;
         }
     } else {
-        const int ps = piece_slot(un, u, piece);
-        pd.o = d.piece_o + (size_t)ps * d.G * kHeadDim;
-        pd.lse = d.piece_lse + (size_t)ps * d.G;
+        pd.o = d.piece_o + (size_t)piece * d.G * kHeadDim;
+        pd.lse = d.piece_lse + (size_t)piece * d.G;
     }
     return pd;
 }
 
-// One warp merges n partials of a head group: source partial j has o rows at src_o + j*o_stride + i*128 and
-// lse at src_lse[j*lse_stride + i], i < G.  Lane l owns columns [4l, 4l+4).  Loads bypass L1 (__ldcg): the
-// partials were written by other SMs in this same launch.  Four heads are reduced together and the inner loop
-// is unrolled so that ~16 independent 16-byte loads are in flight per lane (the merge is L2-latency bound).
-// The accumulation order is j ascending for every head, whoever calls this.
-__device__ __forceinline__ void warp_merge(const float *src_o, size_t o_stride, const float *src_lse,
-                                           size_t lse_stride, int n, int G, float *dst_o, float *dst_lse,
-                                           float *dst2_o, float *dst2_lse, int lane) {
-    for (int i0 = 0; i0 < G; i0 += 4) {
-        const int nh = min(4, G - i0);
-        float4 acc[4];
-        float lse_h[4];
+// One warp merges n partials of ONE query head: partial j has its o row at src_o + j*o_stride and its lse at
+// src_lse[j*lse_stride].  Lane l owns columns [4l, 4l+4).  Loads bypass L1 (__ldcg): the partials were written
+// by other SMs, possibly in this same launch.  The lse values and the first batch of rows are requested before
+// anything is computed, so a merge of <= 16 partials costs one L2 round trip.  The accumulation order is j
+// ascending, whoever calls this, so every path (fused tail, stand-alone kernels) produces the same bits.
+constexpr int kMergeBatch = 16;
+
+__device__ __forceinline__ void merge_rows(const float *src_o, size_t o_stride, const float *src_lse,
+                                           size_t lse_stride, int n, float *dst_o, float *dst_lse, float *dst2_o,
+                                           float *dst2_lse, int lane) {
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    float lse = -INFINITY;
+    if (n == 1) {  // exact copy
+        lse = __ldcg(src_lse);
+        acc = __ldcg(reinterpret_cast<const float4 *>(src_o) + lane);
+    } else {
+        // lse values: lane l caches partials l, l+32, l+64, l+96; beyond that they are re-read
+        float lc[4];
 #pragma unroll
-        for (int hh = 0; hh < 4; ++hh) {
-            acc[hh] = make_float4(0.f, 0.f, 0.f, 0.f);
-            lse_h[hh] = -INFINITY;
+        for (int c = 0; c < 4; ++c) {
+            const int j = lane + 32 * c;
+            lc[c] = j < n ? __ldcg(src_lse + (size_t)j * lse_stride) : -INFINITY;
         }
-        if (n == 1) {  // exact copy
+        float4 v[kMergeBatch];
 #pragma unroll
-            for (int hh = 0; hh < 4; ++hh) {
-                if (hh < nh) {
-                    lse_h[hh] = __ldcg(src_lse + i0 + hh);
-                    acc[hh] = __ldcg(reinterpret_cast<const float4 *>(src_o + (size_t)(i0 + hh) * kHeadDim) + lane);
-                }
-            }
-        } else {
+        for (int k = 0; k < kMergeBatch; ++k)
+            v[k] = k < n ? __ldcg(reinterpret_cast<const float4 *>(src_o + (size_t)k * o_stride) + lane)
+                         : make_float4(0.f, 0.f, 0.f, 0.f);
+        float M = fmaxf(fmaxf(lc[0], lc[1]), fmaxf(lc[2], lc[3]));
+        for (int j = lane + 128; j < n; j += 32) M = fmaxf(M, __ldcg(src_lse + (size_t)j * lse_stride));
+        M = warp_max(M);
+        if (M != -INFINITY) {
+            float sum = 0.f;
 #pragma unroll
-            for (int hh = 0; hh < 4; ++hh) {
-                if (hh < nh) {
-                    const float *lp = src_lse + i0 + hh;
-                    float M = -INFINITY;
-                    for (int j = lane; j < n; j += 32) M = fmaxf(M, __ldcg(lp + (size_t)j * lse_stride));
-                    M = warp_max(M);
-                    if (M != -INFINITY) {
-                        float sum = 0.f;
-                        for (int j = lane; j < n; j += 32) sum += expf(__ldcg(lp + (size_t)j * lse_stride) - M);
-                        sum = warp_sum(sum);
-                        lse_h[hh] = M + logf(sum);
-                    }
-                }
-            }
-            for (int jb = 0; jb < n; jb += 32) {
-                float wl[4];  // this lane's weights of partial jb + lane
-#pragma unroll
-                for (int hh = 0; hh < 4; ++hh) {
-                    wl[hh] = 0.f;
-                    if (hh < nh && jb + lane < n && lse_h[hh] != -INFINITY)
-                        wl[hh] = expf(__ldcg(src_lse + (size_t)(jb + lane) * lse_stride + i0 + hh) - lse_h[hh]);
-                }
-                const int cnt = min(32, n - jb);
-#pragma unroll 4
-                for (int jj = 0; jj < cnt; ++jj) {
-                    const float *row = src_o + (size_t)(jb + jj) * o_stride + (size_t)i0 * kHeadDim;
-#pragma unroll
-                    for (int hh = 0; hh < 4; ++hh) {
-                        const float w = __shfl_sync(0xffffffffu, wl[hh], jj);
-                        if (hh < nh) {
-                            float4 v = __ldcg(reinterpret_cast<const float4 *>(row + (size_t)hh * kHeadDim) + lane);
-                            if (w == 0.f) v = make_float4(0.f, 0.f, 0.f, 0.f);  // lse_j = -inf: ignore its o_j
-                            acc[hh].x = fmaf(w, v.x, acc[hh].x);
-                            acc[hh].y = fmaf(w, v.y, acc[hh].y);
-                            acc[hh].z = fmaf(w, v.z, acc[hh].z);
-                            acc[hh].w = fmaf(w, v.w, acc[hh].w);
-                        }
-                    }
-                }
-            }
+            for (int c = 0; c < 4; ++c) sum += expf(lc[c] - M);  // exp(-inf) = 0 for the padding
+            for (int j = lane + 128; j < n; j += 32) sum += expf(__ldcg(src_lse + (size_t)j * lse_stride) - M);
+            sum = warp_sum(sum);
+            lse = M + logf(sum);
         }
+        for (int jb = 0; jb < n; jb += 32) {
+            float wl = 0.f;  // this lane's weight of partial jb + lane
+            if (jb + lane < n && lse != -INFINITY) {
+                const int c = jb >> 5;
+                const float lj = c == 0 ? lc[0] : c == 1 ? lc[1] : c == 2 ? lc[2] : c == 3 ? lc[3]
+                                        : __ldcg(src_lse + (size_t)(jb + lane) * lse_stride);
+                wl = expf(lj - lse);
+            }
+            const int cnt = min(32, n - jb);
+            for (int j0 = 0; j0 < cnt; j0 += kMergeBatch) {
+                if (jb + j0 > 0) {
 #pragma unroll
-        for (int hh = 0; hh < 4; ++hh) {
-            if (hh < nh) {
-                reinterpret_cast<float4 *>(dst_o + (size_t)(i0 + hh) * kHeadDim)[lane] = acc[hh];
-                if (lane == 0) dst_lse[i0 + hh] = lse_h[hh];
-                if (dst2_o) {
-                    reinterpret_cast<float4 *>(dst2_o + (size_t)(i0 + hh) * kHeadDim)[lane] = acc[hh];
-                    if (lane == 0) dst2_lse[i0 + hh] = lse_h[hh];
+                    for (int k = 0; k < kMergeBatch; ++k)
+                        v[k] = j0 + k < cnt ? __ldcg(reinterpret_cast<const float4 *>(
+                                                         src_o + (size_t)(jb + j0 + k) * o_stride) + lane)
+                                            : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+#pragma unroll
+                for (int k = 0; k < kMergeBatch; ++k) {
+                    const float w = __shfl_sync(0xffffffffu, wl, (j0 + k) & 31);
+                    if (j0 + k < cnt && w != 0.f) {  // w == 0 (lse_j = -inf): ignore its o_j, whatever it holds
+                        acc.x = fmaf(w, v[k].x, acc.x);
+                        acc.y = fmaf(w, v[k].y, acc.y);
+                        acc.z = fmaf(w, v[k].z, acc.z);
+                        acc.w = fmaf(w, v[k].w, acc.w);
+                    }
                 }
             }
         }
     }
+    reinterpret_cast<float4 *>(dst_o)[lane] = acc;
+    if (lane == 0) *dst_lse = lse;
+    if (dst2_o) {
+        reinterpret_cast<float4 *>(dst2_o)[lane] = acc;
+        if (lane == 0) *dst2_lse = lse;
+    }
 }
 
-// merge the pieces of unit u into its range partial (and into the final output if J_r == 1 and fused)
-__device__ __forceinline__ void merge_unit_pieces(const AttendParams &p, const Unit &un, int u, int g, int lane) {
+// merge the pieces of unit u, query head i of its group, into the range partial (and into the final output if
+// the request has a single range and `to_final`)
+__device__ __forceinline__ void merge_unit_head(const AttendParams &p, const Unit &un, int g, int i, bool to_final,
+                                                int lane) {
     const Dev &d = p.d;
-    const size_t row = range_row(d, un.req, un.range, g * d.G);
+    const int head = g * d.G + i;
+    const size_t row = range_row(d, un.req, un.range, head);
     float *o2 = nullptr, *l2 = nullptr;
-    if (p.fused && d.scratch[un.req] == 1) {
-        const size_t frow = (size_t)un.req * d.Hq + g * d.G;
+    if (to_final && d.scratch[un.req] == 1) {
+        const size_t frow = (size_t)un.req * d.Hq + head;
         o2 = p.o + frow * kHeadDim;
         l2 = p.lse + frow;
     }
-    const int ps = piece_slot(un, u, un.piece_begin);
-    warp_merge(d.piece_o + (size_t)ps * d.G * kHeadDim, (size_t)d.G * kHeadDim,
-               d.piece_lse + (size_t)ps * d.G, d.G, un.n_pieces, d.G, p.o_part + row * kHeadDim,
+    merge_rows(d.piece_o + ((size_t)un.piece_begin * d.G + i) * kHeadDim, (size_t)d.G * kHeadDim,
+               d.piece_lse + (size_t)un.piece_begin * d.G + i, d.G, un.n_pieces, p.o_part + row * kHeadDim,
                p.lse_part + row, o2, l2, lane);
 }
 
-// merge the J range partials of (req, kv head g) into the final output
-__device__ __forceinline__ void merge_request_ranges(const Dev &d, const float *o_part, const float *lse_part,
-                                                     float *o, float *lse, int req, int g, int J, int lane) {
-    const size_t row = range_row(d, req, 0, g * d.G);
-    const size_t frow = (size_t)req * d.Hq + g * d.G;
-    warp_merge(o_part + row * kHeadDim, (size_t)d.Hq * kHeadDim, lse_part + row, d.Hq, J, d.G,
-               o + frow * kHeadDim, lse + frow, nullptr, nullptr, lane);
+// merge the J range partials of (req, query head h) into the final output
+__device__ __forceinline__ void merge_request_head(const Dev &d, const float *o_part, const float *lse_part,
+                                                   float *o, float *lse, int req, int h, int J, int lane) {
+    const size_t row = range_row(d, req, 0, h);
+    const size_t frow = (size_t)req * d.Hq + h;
+    merge_rows(o_part + row * kHeadDim, (size_t)d.Hq * kHeadDim, lse_part + row, d.Hq, J, o + frow * kHeadDim,
+               lse + frow, nullptr, nullptr, lane);
 }
 
-// Fused tail: called by the whole warp after it has written the partial of one piece of unit u.
-// The last piece of a unit merges the unit; the last unit of a (request, kv head) merges the request.
-__device__ __forceinline__ void finish_piece(const AttendParams &p, int u, const Unit &un, int g, int lane) {
-    const Dev &d = p.d;
-    if (un.n_pieces > 1) {
+// ---- scheduler words and completion counters of one attend launch -----------------------------------------
+// sched[0] chunk ticket, [1] finished workers, [2] unit-merge ticket, [3] request-merge ticket, [4] epoch.
+// The completion counters are double-buffered by launch parity: a launch counts in buffer (epoch & 1) and
+// zeroes the other one for the next launch, so nothing has to be reset on the critical path.
+struct Counters {
+    int32_t *unit;   // [U]      pieces of unit u finished
+    int32_t *group;  // [B*Hkv]  range partials of (request, kv head) finished, counted per query head
+};
+
+__device__ __forceinline__ Counters launch_prologue(const Dev &d, int w, int W, int lane) {
+    const int epoch = *reinterpret_cast<volatile int32_t *>(d.sched + 4);
+    const int Ucap = d.B * d.Jmax * d.Hkv, Gcap = d.B * d.Hkv;
+    Counters c, o;
+    c.unit = d.unit_counter + (size_t)(epoch & 1) * Ucap;
+    c.group = d.group_counter + (size_t)(epoch & 1) * Gcap;
+    o.unit = d.unit_counter + (size_t)((epoch + 1) & 1) * Ucap;
+    o.group = d.group_counter + (size_t)((epoch + 1) & 1) * Gcap;
+    for (int i = w * 32 + lane; i < Ucap; i += W * 32) o.unit[i] = 0;
+    for (int i = w * 32 + lane; i < Gcap; i += W * 32) o.group[i] = 0;
+    return c;
+}
+
+// the last worker to finish rewinds the tickets and flips the epoch for the next launch
+__device__ __forceinline__ void launch_epilogue(const Dev &d, int W, int lane) {
+    if (lane == 0) {
         __threadfence();
-        __syncwarp();
-        int old = 0;
-        if (lane == 0) old = atomicAdd(&d.unit_counter[u], 1);
-        old = __shfl_sync(0xffffffffu, old, 0);
-        if (old != un.n_pieces - 1) return;
-        __threadfence();
-        merge_unit_pieces(p, un, u, g, lane);
-        if (lane == 0) d.unit_counter[u] = 0;
+        const int old = atomicAdd(d.sched + 1, 1);
+        if (old == W - 1) {
+            d.sched[0] = 0;
+            d.sched[1] = 0;
+            d.sched[2] = 0;
+            d.sched[3] = 0;
+            d.sched[4] = d.sched[4] + 1;
+        }
     }
-    const int J = d.scratch[un.req];
-    if (J <= 1) return;  // piece_dest / merge_unit_pieces already wrote the final rows
+}
+
+// called by the whole warp after it has written the partial of one piece of unit u (fused mode)
+__device__ __forceinline__ void piece_done(const AttendParams &p, const Counters &c, int u, const Unit &un, int g,
+                                           int lane) {
+    const Dev &d = p.d;
     __threadfence();
     __syncwarp();
-    int old = 0;
-    if (lane == 0) old = atomicAdd(&d.group_counter[un.req * d.Hkv + g], 1);
-    old = __shfl_sync(0xffffffffu, old, 0);
-    if (old != J - 1) return;
+    if (lane == 0) {
+        if (un.n_pieces > 1)
+            atomicAdd(&c.unit[u], 1);
+        else if (d.scratch[un.req] > 1)
+            atomicAdd(&c.group[un.req * d.Hkv + g], d.G);  // the range partial of all G heads is complete
+    }
+}
+
+__device__ __forceinline__ void wait_counter(const int32_t *ctr, int target, int lane) {
+    if (lane == 0) {
+        int v;
+        for (;;) {
+            asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+            if (v >= target) break;
+            __nanosleep(64);
+        }
+    }
+    __syncwarp();
     __threadfence();
-    merge_request_ranges(d, p.o_part, p.lse_part, p.o, p.lse, un.req, g, J, lane);
-    if (lane == 0) d.group_counter[un.req * d.Hkv + g] = 0;
+}
+
+// Fused tail: once the chunk list is exhausted every worker turns into a merge worker.
+// Phase A tasks = (unit, head of its group): pieces -> range partial; phase B tasks = (request, query head):
+// range partials -> output.  A task waits until its inputs are complete (the producers are resident workers of
+// this same launch: the grid never exceeds the SM count).  Tickets are taken in batches to bound atomic traffic.
+__device__ __forceinline__ void merge_phase(const AttendParams &p, const Counters &c, int W, int lane) {
+    const Dev &d = p.d;
+    const int G = d.G, Hkv = d.Hkv;
+    const int nA = __ldg(&d.plan->n_units) * G;
+    const int batchA = max(1, nA / (4 * W));
+    for (;;) {
+        int t0 = 0;
+        if (lane == 0) t0 = atomicAdd(d.sched + 2, batchA);
+        t0 = __shfl_sync(0xffffffffu, t0, 0);
+        if (t0 >= nA) break;
+        const int t1 = min(nA, t0 + batchA);
+        for (int t = t0; t < t1; ++t) {
+            const int u = t / G, i = t - u * G;
+            const Unit un = d.units[u];
+            if (un.n_pieces <= 1) continue;
+            const int g = u % Hkv;
+            wait_counter(&c.unit[u], un.n_pieces, lane);
+            merge_unit_head(p, un, g, i, true, lane);
+            if (d.scratch[un.req] > 1) {
+                __threadfence();
+                __syncwarp();
+                if (lane == 0) atomicAdd(&c.group[un.req * Hkv + g], 1);
+            }
+        }
+    }
+    const int nB = d.B * d.Hq;
+    const int batchB = max(1, nB / (4 * W));
+    for (;;) {
+        int t0 = 0;
+        if (lane == 0) t0 = atomicAdd(d.sched + 3, batchB);
+        t0 = __shfl_sync(0xffffffffu, t0, 0);
+        if (t0 >= nB) break;
+        const int t1 = min(nB, t0 + batchB);
+        for (int t = t0; t < t1; ++t) {
+            const int req = t / d.Hq, h = t - req * d.Hq;
+            const int J = d.scratch[req];  // 0 for closed requests
+            if (J <= 1) continue;          // a single range: its partial was also written to the output
+            wait_counter(&c.group[req * Hkv + h / G], J * G, lane);
+            merge_request_head(d, p.o_part, p.lse_part, p.o, p.lse, req, h, J, lane);
+        }
+    }
 }
 
 }  // namespace kf

@@ -152,16 +152,60 @@ __device__ __forceinline__ int last_le(const int *a, int n, int x) {
     return lo;
 }
 
-// scratch layout (ints): J[B] | S[B] | epre[B+1] | etiles[Emax] | tpre[Emax+1] | cuts[kMaxWorkers]
+// ---- guided self-scheduling ----------------------------------------------------------------------------
+// Chunk sizes follow guided self-scheduling: a chunk that starts at position `pos` of the step's tile sequence
+// (Nt tiles, W workers) holds at most  rho * (Nt - pos) / W  tiles, never fewer than min_tiles -- so whichever
+// worker takes it, and however slow its SM, it finishes before the rest of the work can run out.
+// The tile sequence is LEVEL-major: every unit (n tiles) is cut at the same relative positions -- level 0 takes
+// the first `decay` of its tiles, every later level `decay` of what is left, the last level the rest -- and
+// the sequence visits the level-0 portions of all units, then the level-1 portions, ...  So the small chunks at
+// the end of the launch are spread over all units (each unit ends up with a few pieces per level) instead of
+// shredding the last units into hundreds of pieces.
+struct Levels {
+    int K;
+    int end16[kMaxLevels];  // cumulative fraction at the end of level k, 16-bit fixed point (last = 65536)
+};
+
+__device__ void make_levels(Levels &lv, long long Nt, int W, int m, float f) {
+    const double base = (double)Nt / (double)W;
+    double cum = 0.0;
+    int K = 0;
+    for (;;) {
+        const double phi = (1.0 - cum) * f;
+        // stop when what is left per worker is about two minimum chunks
+        if ((1.0 - cum) * base <= 2.0 * m || K == kMaxLevels - 1 || f > 0.9995f) {
+            lv.end16[K++] = 65536;
+            break;
+        }
+        cum += phi;
+        lv.end16[K++] = (int)(cum * 65536.0);
+    }
+    lv.K = K;
+}
+
+// tiles [b0, b0 + len) of a unit with n tiles belong to level k
+__device__ __forceinline__ void level_span(const Levels &lv, int n, int k, int &b0, int &len) {
+    b0 = k == 0 ? 0 : (int)(((long long)n * lv.end16[k - 1]) >> 16);
+    const int b1 = (int)(((long long)n * lv.end16[k]) >> 16);
+    len = b1 - b0;
+}
+
+// scratch layout (ints): J[B] | S[B] | epre[B+1] | etiles[Emax] | tpre[Emax+1] | ppre[Emax+1] |
+//                        pos[kMaxLevels*Emax+1] | ccnt[kMaxLevels*Emax] | lpre[kMaxLevels*Emax+1]
 __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d) {
+    __shared__ Levels lv;
+    __shared__ int s_m;
     const int tid = threadIdx.x, nt = blockDim.x;
-    const int B = d.B, Emax = d.B * d.Jmax, T = kTileTokens;
+    const int B = d.B, Emax = d.B * d.Jmax, T = kTileTokens, Hkv = d.Hkv;
     int *Jr = d.scratch;
     int *Sr = Jr + B;
     int *epre = Sr + B;
     int *etiles = epre + (B + 1);
     int *tpre = etiles + Emax;
-    int *cuts = tpre + (Emax + 1);
+    int *ppre = tpre + (Emax + 1);
+    int *pos = ppre + (Emax + 1);
+    int *ccnt = pos + ((size_t)kMaxLevels * Emax + 1);
+    int *lpre = ccnt + (size_t)kMaxLevels * Emax;
 
     // 1. per request: tokens attended this step S = len + 1, ranges J = ceil(S / R)
     for (int r = tid; r < B; r += nt) {
@@ -183,82 +227,127 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d) {
     if (tid == 0) epre[B] = E;
     __syncthreads();
 
-    // 2. per (request, range) entry: token count and tiles
+    // 2. per (request, range) entry: token count and tiles (identical for the H_kv units of the entry)
     for (int e = tid; e < E; e += nt) {
         const int r = last_le(epre, B + 1, e);
         const int j = e - epre[r];
         const int cnt = min(d.R, Sr[r] - j * d.R);
         const int tiles = (cnt + T - 1) / T;
         etiles[e] = tiles;
-        tpre[e] = tiles * d.Hkv;
+        tpre[e] = tiles * Hkv;
     }
     __syncthreads();
     const int Nt = block_exclusive_scan(tpre, E);
-    if (tid == 0) tpre[E] = Nt;
+    if (tid == 0) {
+        tpre[E] = Nt;
+        s_m = d.min_tiles;
+    }
     __syncthreads();
 
-    // 3. equal split of the global tile sequence over A workers
-    int A = 0;
-    if (Nt > 0) A = max(1, min(d.max_workers, Nt / d.min_tiles));
-    for (int w = tid; w < d.max_workers; w += nt) {
-        Span sp = {0, 0, 0, 0};
-        int cut = 0;
-        if (w < A) {
-            const int start = (int)(((int64_t)w * Nt) / A);
-            const int end = (int)(((int64_t)(w + 1) * Nt) / A);
-            const int e = last_le(tpre, E + 1, start);
-            const int rel = start - tpre[e];
-            const int g = rel / etiles[e];
-            sp.unit = e * d.Hkv + g;
-            sp.tile_in_unit = rel - g * etiles[e];
-            sp.n_tiles = end - start;
-            cut = sp.tile_in_unit != 0;
+    // 3. levels, positions in the level-major tile sequence, chunk counts per (level, entry);
+    //    coarsen (double min_tiles) until the chunk list fits its buffer
+    const int W = d.max_workers;
+    const float rho = d.sched_first;
+    int n_chunks = 0;
+    for (int iter = 0; iter < 32; ++iter) {
+        if (tid == 0) make_levels(lv, Nt, W, s_m, d.sched_decay);
+        __syncthreads();
+        const int KE = lv.K * E, m = s_m;
+        for (int idx = tid; idx < KE; idx += nt) {
+            const int k = idx / E, e = idx - k * E;
+            int b0, len;
+            level_span(lv, etiles[e], k, b0, len);
+            pos[idx] = len * Hkv;
         }
-        d.spans[w] = sp;
-        cuts[w] = cut;
+        __syncthreads();
+        block_exclusive_scan(pos, KE);
+        __syncthreads();
+        for (int idx = tid; idx < KE; idx += nt) {
+            const int k = idx / E, e = idx - k * E;
+            int b0, len;
+            level_span(lv, etiles[e], k, b0, len);
+            const float left = (float)(Nt - pos[idx]);
+            const int size = max(m, (int)ceilf(rho * left / (float)W));
+            const int c = (len + size - 1) / size;
+            ccnt[idx] = c;
+            lpre[idx] = c * Hkv;
+        }
+        __syncthreads();
+        n_chunks = block_exclusive_scan(lpre, KE);
+        if (tid == 0) lpre[KE] = n_chunks;
+        __syncthreads();
+        if (n_chunks <= d.max_chunks) break;
+        if (tid == 0) s_m = s_m >= (1 << 28) ? s_m : s_m * 2;
+        __syncthreads();
+    }
+    const int K = lv.K;
+
+    // 4. pieces per entry (per kv head) -> piece prefix
+    for (int e = tid; e < E; e += nt) {
+        int pu = 0;
+        for (int k = 0; k < K; ++k) pu += ccnt[k * E + e];
+        ppre[e] = pu;
     }
     __syncthreads();
-    const int total_cuts = block_exclusive_scan(cuts, A);
-    for (int w = tid; w < A; w += nt) {
-        const int own = d.spans[w].tile_in_unit != 0;
-        d.spans[w].piece = d.spans[w].unit + cuts[w] + own;
-    }
+    const int pieces_per_head = block_exclusive_scan(ppre, E);
+    if (tid == 0) ppre[E] = pieces_per_head;
     __syncthreads();
 
-    // 4. units, with the pieces (worker spans) that intersect them
-    const int U = E * d.Hkv;
+    // 5. chunk descriptors in level-major order; piece index = unit-major, tile order inside the unit
+    const int items = K * E * Hkv;
+    for (int idx = tid; idx < items; idx += nt) {
+        const int k = idx / (E * Hkv);
+        const int rem = idx - k * (E * Hkv);
+        const int e = rem / Hkv, g = rem - e * Hkv;
+        const int c = ccnt[k * E + e];
+        if (c == 0) continue;
+        int b0, len;
+        level_span(lv, etiles[e], k, b0, len);
+        int before = 0;
+        for (int kk = 0; kk < k; ++kk) before += ccnt[kk * E + e];
+        const int pu = ppre[e + 1] - ppre[e];
+        const int piece0 = ppre[e] * Hkv + g * pu + before;
+        const int chunk0 = lpre[k * E + e] + g * c;
+        for (int i = 0; i < c; ++i) {
+            const int t0 = b0 + (int)(((long long)i * len) / c);
+            const int t1 = b0 + (int)(((long long)(i + 1) * len) / c);
+            Chunk ch;
+            ch.unit = e * Hkv + g;
+            ch.tile_begin = t0;
+            ch.n_tiles = t1 - t0;
+            ch.piece = piece0 + i;
+            d.chunks[chunk0 + i] = ch;
+        }
+    }
+
+    // 6. units
+    const int U = E * Hkv;
     for (int u = tid; u < U; u += nt) {
-        const int e = u / d.Hkv, g = u - e * d.Hkv;
+        const int e = u / Hkv, g = u - e * Hkv;
         const int r = last_le(epre, B + 1, e);
         const int j = e - epre[r];
-        const int tb = tpre[e] + g * etiles[e];
-        const int te = tb + etiles[e];
-        // number of workers whose span starts before tile x: ceil(x * A / Nt)
-        const int wb = (int)(((int64_t)tb * A + Nt - 1) / Nt);
-        const int we = (int)(((int64_t)te * A + Nt - 1) / Nt);
-        const int cb = wb > 0 ? cuts[wb - 1] + (d.spans[wb - 1].tile_in_unit != 0) : 0;
-        const int ce = we > 0 ? cuts[we - 1] + (d.spans[we - 1].tile_in_unit != 0) : 0;
+        const int pu = ppre[e + 1] - ppre[e];
         Unit un;
         un.req = r;
         un.range = j;
         un.part = d.route_part[(size_t)r * d.Jmax + j];
         un.slot = d.route_slot[(size_t)r * d.Jmax + j];
         un.cnt = min(d.R, Sr[r] - j * d.R);
-        un.tile_begin = tb;
-        un.piece_begin = u + cb;
-        un.n_pieces = (u + 1 + ce) - (u + cb);
+        un.tile_begin = tpre[e] + g * etiles[e];
+        un.piece_begin = ppre[e] * Hkv + g * pu;
+        un.n_pieces = pu;
         d.units[u] = un;
     }
     if (tid == 0) {
         PlanHeader h;
         h.n_units = U;
         h.n_tiles = Nt;
-        h.n_workers = A;
-        h.n_pieces = U + total_cuts;
+        h.n_workers = min(W, n_chunks);
+        h.n_pieces = n_chunks;
         h.n_entries = E;
         h.tile_tokens = T;
-        h.max_workers = d.max_workers;
-        h.pad = 0;
+        h.max_workers = W;
+        h.n_levels = K;
         *d.plan = h;
     }
 }

@@ -17,7 +17,7 @@ from .binding import KF_IMPL_AUTO, KFlume, make_config
 class Session:
     def __init__(self, wl: Workload, impl: int = KF_IMPL_AUTO, n_layers_phys: Optional[int] = None,
                  steps: Optional[int] = None, min_tiles: int = 0, device: str = "cuda:0", softmax_scale: float = 0.0,
-                 slack_slots: int = 0):
+                 slack_slots: int = 0, **tuning):
         import torch
         self.torch = torch
         self.wl = wl
@@ -27,7 +27,7 @@ class Session:
         cfg = make_config(wl.n_q_heads, wl.n_kv_heads, wl.range_tokens, wl.n_partitions, wl.batch,
                           wl.max_ranges(self.steps), wl.slots_per_partition(self.steps) + slack_slots,
                           n_layers=self.L_phys, softmax_scale=softmax_scale, attend_impl=impl,
-                          min_tiles_per_worker=min_tiles)
+                          min_tiles_per_worker=min_tiles, **tuning)
         self.kf = KFlume(cfg, device)
         self.device = self.kf.device
         B, Hq, Hkv = wl.batch, wl.n_q_heads, wl.n_kv_heads
