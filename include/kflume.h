@@ -185,8 +185,8 @@ int kf_status(kf_ctx *ctx, kf_stream stream);
 int kf_plan_info(kf_ctx *ctx, int32_t *out, kf_stream stream);
 int64_t kf_launch_count(const kf_ctx *ctx);
 /* kf_worker_times (diagnostics): per-worker timestamps of the LAST attend launch, out[max_workers][4] [host] =
- *   {SM id, t_start, t_first_tile_ready, t_end} in globaltimer nanoseconds (all 0 for idle workers);
- *   *n_workers = max_workers.  Synchronises `stream`. */
+ *   {SM id | (time spent streaming chunks, ns) << 8, t_start, t_first_tile_ready (0: took no chunk), t_end} in
+ *   globaltimer nanoseconds; *n_workers = max_workers.  Synchronises `stream`. */
 int kf_worker_times(kf_ctx *ctx, int64_t *out, int32_t *n_workers, kf_stream stream);
 
 #ifdef __cplusplus

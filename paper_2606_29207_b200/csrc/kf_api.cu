@@ -3,6 +3,7 @@
 #include <cuda.h>
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -26,7 +27,7 @@ namespace {
 
 constexpr size_t kAlign = 256;
 constexpr int kDefaultWarps = 8, kDefaultStages = 3;
-constexpr int kDefaultFirstPct = 50, kDefaultDecayPct = 50;
+constexpr int kDefaultFirstPct = 80, kDefaultDecayPct = 50;
 
 size_t max_chunks_of(const kf_config *c) {
     return (size_t)c->max_requests * c->max_ranges_per_request * c->n_kv_heads + kChunkSlack;
@@ -269,6 +270,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.warps_per_cta = warps;
     d.stages = cfg->pipeline_stages ? cfg->pipeline_stages : kDefaultStages;
     d.max_chunks = (int32_t)max_chunks_of(cfg);
+    d.l2_hint = getenv("KF_L2_HINT") ? atoi(getenv("KF_L2_HINT")) : 0;  // experiment knob
     d.sched_first = 0.01f * (cfg->sched_first_pct ? cfg->sched_first_pct : kDefaultFirstPct);
     d.sched_decay = 0.01f * (cfg->sched_decay_pct ? cfg->sched_decay_pct : kDefaultDecayPct);
     const float scale = cfg->softmax_scale > 0.f ? cfg->softmax_scale : 1.0f / sqrtf((float)kHeadDim);

@@ -12,12 +12,13 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) attend_simple_kernel(Attend
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = gridDim.x * kWarpsPerCta;
     const int n_chunks = d.plan->n_pieces;
-    const Counters ctr = launch_prologue(d, blockIdx.x * kWarpsPerCta + warp, W, lane);
+    const int w = warp * gridDim.x + blockIdx.x;  // warp-major: small launches spread over all SMs
+    const Counters ctr = launch_prologue(d, w, W, lane);
     const int G = d.G;
     float *qs = q_s[warp];
 
     // static round-robin over the chunk list (one chunk = one piece of one unit)
-    for (int c = blockIdx.x * kWarpsPerCta + warp; c < n_chunks; c += W) {
+    for (int c = w; c < n_chunks; c += W) {
         const Chunk ch = d.chunks[c];
         const int u = ch.unit, piece = ch.piece;
         const Unit un = d.units[u];

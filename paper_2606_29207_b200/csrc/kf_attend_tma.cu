@@ -54,6 +54,14 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void *tmap, int 
         "l"(tmap), "r"(bar), "r"(x), "r"(y)
         : "memory");
 }
+__device__ __forceinline__ void tma_load_2d_hint(uint32_t dst, const void *tmap, int x, int y, uint32_t bar,
+                                                 uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4}], "
+        "[%2], %5;" ::"r"(dst),
+        "l"(tmap), "r"(bar), "r"(x), "r"(y), "l"(policy)
+        : "memory");
+}
 __device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t &r0, uint32_t &r1, uint32_t &r2, uint32_t &r3) {
     asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
                  : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
@@ -116,7 +124,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
     const Dev &d = p.d;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = gridDim.x * WARPS;
-    const int w = blockIdx.x * WARPS + warp;
+    const int w = warp * gridDim.x + blockIdx.x;  // warp-major: the first chunks of a small launch spread over all SMs
     const int n_chunks = __ldg(&d.plan->n_pieces);
     const long long t_start = global_ns();
     long long t_first = 0, t_stream = 0;
@@ -134,6 +142,8 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
         __syncwarp();
 
         const int G = d.G, Hkv = d.Hkv;
+        uint64_t policy = 0;  // K/V is read once per launch: evict-first keeps the partials resident in L2
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
         const unsigned char *tmaps = reinterpret_cast<const unsigned char *>(d.tmaps);
 
         // ---- load cursor: runs up to STAGES tiles ahead of the compute cursor, across chunk boundaries ----
@@ -176,10 +186,17 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
                 const uint32_t sb = wbase + stage * kStageBytes, bar = bar0 + 8 * stage;
                 const unsigned char *tk = tmaps + (size_t)l_part * 256;
                 mbar_expect_tx(bar, kStageBytes);
-                tma_load_2d(sb, tk, 0, l_row, bar);
-                tma_load_2d(sb + kSubTile, tk, 64, l_row, bar);
-                tma_load_2d(sb + 2 * kSubTile, tk + 128, 0, l_row, bar);
-                tma_load_2d(sb + 3 * kSubTile, tk + 128, 64, l_row, bar);
+                if (d.l2_hint) {
+                    tma_load_2d_hint(sb, tk, 0, l_row, bar, policy);
+                    tma_load_2d_hint(sb + kSubTile, tk, 64, l_row, bar, policy);
+                    tma_load_2d_hint(sb + 2 * kSubTile, tk + 128, 0, l_row, bar, policy);
+                    tma_load_2d_hint(sb + 3 * kSubTile, tk + 128, 64, l_row, bar, policy);
+                } else {
+                    tma_load_2d(sb, tk, 0, l_row, bar);
+                    tma_load_2d(sb + kSubTile, tk, 64, l_row, bar);
+                    tma_load_2d(sb + 2 * kSubTile, tk + 128, 0, l_row, bar);
+                    tma_load_2d(sb + 3 * kSubTile, tk + 128, 64, l_row, bar);
+                }
             }
             l_row += kTileTokens;
             --l_left;
@@ -341,11 +358,11 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
     if (p.fused) merge_phase(p, ctr, W, lane);
 
     if (lane == 0) {
-        // diagnostics: {SM | stream-end offset << 8, start, first tile ready, end}
+        // diagnostics: {SM | stream-end offset << 8, start, first tile ready (0 = no chunk), end}
         d.worker_times[4 * w] = sm_id() | ((w < n_chunks ? t_stream - t_start : 0) << 8);
-        d.worker_times[4 * w + 1] = w < n_chunks ? t_start : 0;
+        d.worker_times[4 * w + 1] = t_start;
         d.worker_times[4 * w + 2] = t_first;
-        d.worker_times[4 * w + 3] = w < n_chunks ? global_ns() : 0;
+        d.worker_times[4 * w + 3] = global_ns();
     }
     launch_epilogue(d, W, lane);
 }

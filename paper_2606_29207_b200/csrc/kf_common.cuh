@@ -60,6 +60,7 @@ struct Dev {
     int32_t Hq, Hkv, G, L, R, P, B, Jmax, slots;
     int32_t max_workers, min_tiles;
     int32_t warps_per_cta, stages;      // launch shape of the attend kernels
+    int32_t l2_hint;                    // 1: K/V tiles are loaded with an L2 evict-first policy
     int32_t max_chunks;                 // capacity of chunks[] and of the piece buffers
     float sched_first, sched_decay;     // GSS factor rho (chunk <= rho * remaining / workers); share of a unit's remaining tiles per level
     float scale_log2;  // softmax_scale * log2(e)
