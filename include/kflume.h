@@ -78,6 +78,8 @@ typedef struct kf_config {
     int32_t pipeline_stages;        /* 8 KB TMA stages in flight per worker: 2..6 (2..3 for 8 workers) */
     int32_t sched_first_pct;        /* 1..100: guided self-scheduling factor: chunk <= pct% of (remaining tiles / workers) */
     int32_t sched_decay_pct;        /* 1..99: share of a unit's remaining tiles that each scheduling level takes */
+    int32_t plan_refresh_steps;     /* the work plan is rebuilt when a route changes or after this many token boundaries
+                                     * (0 => 128; 1 => every step); in between, tail ranges grow inside the kept plan */
 } kf_config;
 
 typedef struct kf_ctx kf_ctx;

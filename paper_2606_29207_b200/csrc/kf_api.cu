@@ -18,7 +18,8 @@ struct kf_ctx {
     int sm_count;
     int n_ctas;
     int impl;
-    bool plan_dirty;
+    bool plan_dirty;    // lengths moved (step commit) or routes were edited since the plan kernel last ran
+    bool routes_dirty;  // routes were edited from the host side (open / close / create): the next plan must be rebuilt
     int64_t launches;
     char cuda_err[256];
 };
@@ -28,6 +29,7 @@ namespace {
 constexpr size_t kAlign = 256;
 constexpr int kDefaultWarps = 8, kDefaultStages = 3;
 constexpr int kDefaultFirstPct = 80, kDefaultDecayPct = 50;
+constexpr int kDefaultPlanRefresh = 128;
 
 size_t max_chunks_of(const kf_config *c) {
     return (size_t)c->max_requests * c->max_ranges_per_request * c->n_kv_heads + kChunkSlack;
@@ -35,7 +37,7 @@ size_t max_chunks_of(const kf_config *c) {
 inline size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t len, n_ranges, route_part, route_slot, rr_cursor, free_head, free_cnt, free_stack, error, plan, units, chunks, sched,
+    size_t len, n_ranges, route_part, route_slot, rr_cursor, free_head, free_cnt, free_stack, error, plan, units, chunks, plan_age, sched,
         scratch, unit_counter, group_counter, piece_o, piece_lse, range_o, range_lse, stage_q, stage_k, stage_v,
         stage_o, stage_lse, tmaps, worker_times, total;
 };
@@ -61,6 +63,7 @@ bool valid_config(const kf_config *c) {
         return false;
     if (c->sched_first_pct < 0 || c->sched_first_pct > 100) return false;
     if (c->sched_decay_pct < 0 || c->sched_decay_pct > 99) return false;
+    if (c->plan_refresh_steps < 0) return false;
     // rows of one K (or V) half-pool must fit the int32 TMA coordinate
     const double rows = (double)c->n_layers * c->slots_per_partition * c->n_kv_heads * c->range_tokens;
     if (rows >= 2147483647.0) return false;
@@ -91,6 +94,7 @@ Layout make_layout(const kf_config *c) {
     L.plan = take(sizeof(PlanHeader));
     L.units = take(U * sizeof(Unit));
     L.chunks = take(max_piece_slots * sizeof(Chunk));
+    L.plan_age = take(4);
     L.sched = take(8 * 4);
     L.scratch = take((B + B + (B + 1) + E + (E + 1) + (E + 1) + 3 * ((size_t)kMaxLevels * E + 1)) * 4);
     L.unit_counter = take(2 * U * 4);        // double-buffered by launch parity
@@ -174,8 +178,8 @@ int encode_tmaps(kf_ctx *ctx, void *const *pools) {
 
 int ensure_plan(kf_ctx *ctx, cudaStream_t s) {
     if (!ctx->plan_dirty) return KF_OK;
-    const int rc = after_launch(ctx, launch_plan(ctx->dev, s));
-    if (rc == KF_OK) ctx->plan_dirty = false;
+    const int rc = after_launch(ctx, launch_plan(ctx->dev, 0, s));
+    if (rc == KF_OK) ctx->plan_dirty = ctx->routes_dirty = false;
     return rc;
 }
 
@@ -244,7 +248,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     const int warps = ctx->impl == KF_IMPL_SIMPLE ? kWarpsPerCta : (cfg->workers_per_sm ? cfg->workers_per_sm : kDefaultWarps);
     ctx->n_ctas = ctx->sm_count;
     if (ctx->n_ctas * warps > kMaxWorkers) ctx->n_ctas = kMaxWorkers / warps;
-    ctx->plan_dirty = true;
+    ctx->plan_dirty = ctx->routes_dirty = true;
 
     unsigned char *ws = (unsigned char *)workspace;
     e = cudaMemset(ws, 0, L.total);
@@ -271,6 +275,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.stages = cfg->pipeline_stages ? cfg->pipeline_stages : kDefaultStages;
     d.max_chunks = (int32_t)max_chunks_of(cfg);
     d.l2_hint = getenv("KF_L2_HINT") ? atoi(getenv("KF_L2_HINT")) : 0;  // experiment knob
+    d.plan_refresh = cfg->plan_refresh_steps > 0 ? cfg->plan_refresh_steps : kDefaultPlanRefresh;
     d.sched_first = 0.01f * (cfg->sched_first_pct ? cfg->sched_first_pct : kDefaultFirstPct);
     d.sched_decay = 0.01f * (cfg->sched_decay_pct ? cfg->sched_decay_pct : kDefaultDecayPct);
     const float scale = cfg->softmax_scale > 0.f ? cfg->softmax_scale : 1.0f / sqrtf((float)kHeadDim);
@@ -287,6 +292,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.plan = (PlanHeader *)(ws + L.plan);
     d.units = (Unit *)(ws + L.units);
     d.chunks = (Chunk *)(ws + L.chunks);
+    d.plan_age = (int32_t *)(ws + L.plan_age);
     d.sched = (int32_t *)(ws + L.sched);
     d.scratch = (int32_t *)(ws + L.scratch);
     d.unit_counter = (int32_t *)(ws + L.unit_counter);
@@ -305,6 +311,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.v_off = half_pool_bytes(cfg);
     for (int p = 0; p < cfg->n_partitions; ++p) d.pool[p] = (unsigned char *)pool_ptrs[p];
 
+    if (plan_setup() != 0) return cuda_fail(ctx, cudaGetLastError());
     if (ctx->impl == KF_IMPL_TMA) {
         int rc = encode_tmaps(ctx, pool_ptrs);
         if (rc != KF_OK) return rc;
@@ -323,13 +330,13 @@ int kf_destroy(kf_ctx *ctx) {
 
 int kf_open_request(kf_ctx *ctx, int32_t req, int32_t n_tokens, kf_stream stream) {
     if (!ctx || req < 0 || req >= ctx->cfg.max_requests || n_tokens < 0) return KF_EINVAL;
-    ctx->plan_dirty = true;
+    ctx->plan_dirty = ctx->routes_dirty = true;
     return after_launch(ctx, launch_open_request(ctx->dev, req, n_tokens, (cudaStream_t)stream));
 }
 
 int kf_close_request(kf_ctx *ctx, int32_t req, kf_stream stream) {
     if (!ctx || req < 0 || req >= ctx->cfg.max_requests) return KF_EINVAL;
-    ctx->plan_dirty = true;
+    ctx->plan_dirty = ctx->routes_dirty = true;
     return after_launch(ctx, launch_close_request(ctx->dev, req, (cudaStream_t)stream));
 }
 
@@ -346,10 +353,11 @@ int kf_load_context(kf_ctx *ctx, int32_t layer, int32_t req, int32_t tok_begin, 
 
 int kf_token_boundary(kf_ctx *ctx, kf_stream stream) {
     if (!ctx) return KF_EINVAL;
-    int rc = after_launch(ctx, launch_token_boundary(ctx->dev, (cudaStream_t)stream));
-    if (rc != KF_OK) return rc;
-    ctx->plan_dirty = true;
-    return ensure_plan(ctx, (cudaStream_t)stream);
+    // route update and work plan in ONE launch (the plan depends on the routes the update appends)
+    // (the plan is kept when no route changed and it is younger than plan_refresh_steps boundaries)
+    const int rc = after_launch(ctx, launch_plan(ctx->dev, ctx->routes_dirty ? 2 : 1, (cudaStream_t)stream));
+    if (rc == KF_OK) ctx->plan_dirty = ctx->routes_dirty = false;
+    return rc;
 }
 
 int kf_kv_append(kf_ctx *ctx, int32_t layer, const void *k_new, const void *v_new, kf_stream stream) {

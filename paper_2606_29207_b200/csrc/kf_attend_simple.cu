@@ -23,7 +23,8 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) attend_simple_kernel(Attend
         const int u = ch.unit, piece = ch.piece;
         const Unit un = d.units[u];
         const int g = u % d.Hkv;
-        const int t0 = ch.tile_begin, t1 = ch.tile_begin + ch.n_tiles;
+        const int cnt = live_cnt(d, un);  // the plan may be older than this step (kf_common.cuh)
+        const int t0 = ch.tile_begin, t1 = ch.tile_begin + live_tiles(un, cnt, ch.tile_begin, ch.n_tiles);
         if ((p.part_mask >> un.part) & 1ull) {
             const __half *qg = p.q + ((size_t)un.req * d.Hq + (size_t)g * G) * kHeadDim;
             __syncwarp();
@@ -43,7 +44,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) attend_simple_kernel(Attend
 
             for (int tile = t0; tile < t1; ++tile) {
                 const int tok = tile * kTileTokens + (lane & 15);
-                const bool valid = tok < un.cnt;
+                const bool valid = tok < cnt;
                 float s[kMaxGroup];
 #pragma unroll
                 for (int i = 0; i < kMaxGroup; ++i) s[i] = 0.f;
@@ -91,7 +92,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) attend_simple_kernel(Attend
                         m[i] = m_new;
                     }
                 }
-                const int nvalid = min(kTileTokens, un.cnt - tile * kTileTokens);
+                const int nvalid = min(kTileTokens, cnt - tile * kTileTokens);
                 for (int tt = 0; tt < nvalid; ++tt) {
                     const uint2 vv = __ldg(reinterpret_cast<const uint2 *>(
                         Vb + (size_t)(tile * kTileTokens + tt) * 256 + lane * 8));

@@ -108,7 +108,7 @@ __device__ __forceinline__ Unit load_unit(const Unit *units, int u) {
     un.part = a.z;
     un.slot = a.w;
     un.cnt = b.x;
-    un.tile_begin = b.y;
+    un.tail = b.y;
     un.piece_begin = b.z;
     un.n_pieces = b.w;
     return un;
@@ -129,6 +129,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
     const long long t_start = global_ns();
     long long t_first = 0, t_stream = 0;
     const Counters ctr = launch_prologue(d, w, W, lane);
+    int m_first = -1;  // lane 0: pre-taken first merge ticket
 
     if (w < n_chunks) {
         const uint32_t wbase = ((smem_u32(smem_raw) + 1023u) & ~1023u) + warp * kWarpSmem;
@@ -165,11 +166,14 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
                 }
                 if (id >= n_chunks) {
                     l_done = true;
+                    // nothing left to load: reserve the first merge tasks now, STAGES tiles before they are needed
+                    if (p.fused && lane == 0) m_first = merge_first_ticket(d, W);
                     return false;
                 }
-                const int4 c4 = __ldg(reinterpret_cast<const int4 *>(d.chunks + id));
+                int4 c4 = __ldg(reinterpret_cast<const int4 *>(d.chunks + id));
                 const Unit un = load_unit(d.units, c4.x);
                 if (!((p.part_mask >> un.part) & 1ull)) continue;  // partition not selected: nothing to load
+                if (un.tail) c4.z = live_tiles(un, live_cnt(d, un), c4.y, c4.z);  // the plan may be older than this step
                 l_left = c4.z;
                 l_part = un.part;
                 l_row = ((p.layer * d.slots + un.slot) * Hkv + (c4.x % Hkv)) * d.R + c4.y * kTileTokens;
@@ -222,7 +226,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
         const int qrow = lane >> 2, qcol = (lane & 3) * 2;
 
         // ---- compute cursor ------------------------------------------------------------------------------
-        int cu = 0, ct = 0, c_left = 0, piece = 0;
+        int cu = 0, ct = 0, c_left = 0, piece = 0, c_cnt = 0;
         Unit cun;
         cun.cnt = 0;
         uint32_t qa[8][2];  // A fragments of Q: [k-step][a0, a2]
@@ -240,6 +244,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
                 c_left = c4.z;
                 piece = c4.w;
                 cun = load_unit(d.units, cu);
+                c_cnt = live_cnt(d, cun);
                 const __half *qg = p.q + ((size_t)cun.req * d.Hq + (size_t)(cu % Hkv) * G + qrow) * kHeadDim + qcol;
 #pragma unroll
                 for (int ks = 0; ks < 8; ++ks) {
@@ -256,7 +261,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
             mbar_wait(bar0 + 8 * stage, (consumed / STAGES) & 1);
             if (consumed == 0) t_first = global_ns();
 
-            const int valid = min(kTileTokens, cun.cnt - ct * kTileTokens);
+            const int valid = min(kTileTokens, c_cnt - ct * kTileTokens);
             const bool ragged = valid < kTileTokens;
             if (ragged) {
                 // rows >= valid hold whatever the pool holds (maybe NaN patterns): zero them in V so 0 * V = 0
@@ -355,7 +360,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
         }
         t_stream = global_ns();
     }
-    if (p.fused) merge_phase(p, ctr, W, lane);
+    if (p.fused) merge_phase(p, ctr, W, lane, m_first);
 
     if (lane == 0) {
         // diagnostics: {SM | stream-end offset << 8, start, first tile ready (0 = no chunk), end}

@@ -26,8 +26,8 @@ struct Unit {
     int32_t range;
     int32_t part;
     int32_t slot;
-    int32_t cnt;         // tokens of this range attended in this step (1..R)
-    int32_t tile_begin;  // first global tile index of this unit (unit-major order; informational)
+    int32_t cnt;         // tokens of this range when the plan was built (1..R); see live_extent() for tail units
+    int32_t tail;        // 1: this is the request's LAST range: it grows by one token per step
     int32_t piece_begin; // first global piece index of this unit (pieces of a unit are consecutive, tile order)
     int32_t n_pieces;    // pieces = chunks this unit is cut into
 };
@@ -62,6 +62,7 @@ struct Dev {
     int32_t warps_per_cta, stages;      // launch shape of the attend kernels
     int32_t l2_hint;                    // 1: K/V tiles are loaded with an L2 evict-first policy
     int32_t max_chunks;                 // capacity of chunks[] and of the piece buffers
+    int32_t plan_refresh;               // a plan is rebuilt after this many token boundaries (or when routes change)
     float sched_first, sched_decay;     // GSS factor rho (chunk <= rho * remaining / workers); share of a unit's remaining tiles per level
     float scale_log2;  // softmax_scale * log2(e)
     // routing state
@@ -78,6 +79,7 @@ struct Dev {
     PlanHeader *plan;
     Unit *units;            // [B*Jmax*Hkv]
     Chunk *chunks;          // [max_chunks]
+    int32_t *plan_age;      // [0] token boundaries served by the current plan
     int32_t *sched;         // [0] chunk counter (dynamic part of the list), [1] finished-worker counter
     int32_t *scratch;       // plan scratch: [B] J, [B] S, [B+1] entry prefix, [E] tiles, [E+1] tile prefix,
                             //               [E+1] piece prefix, [kMaxLevels*E+1] chunk prefix
@@ -112,6 +114,20 @@ struct AttendParams {
 
 __device__ __forceinline__ void set_error(const Dev &d, int code) { atomicCAS(d.error, 0, code); }
 
+// A work plan outlives the step it was built in (it is rebuilt when a route changes or after plan_refresh
+// boundaries): the only thing that moves in between is the length of each request's TAIL range, +1 token per step.
+// So the token count of a tail unit is re-derived from len at run time, and the chunk that covers the planned end
+// of a tail unit (always the last chunk of scheduling level 0: one of the first and largest chunks) is stretched
+// to the live end.  Every other chunk is exactly as planned.
+__device__ __forceinline__ int live_cnt(const Dev &d, const Unit &un) {
+    return un.tail ? min(d.R, __ldg(d.len + un.req) + 1 - un.range * d.R) : un.cnt;
+}
+__device__ __forceinline__ int live_tiles(const Unit &un, int cnt_live, int tile_begin, int n_tiles) {
+    const int planned = (un.cnt + kTileTokens - 1) / kTileTokens;
+    return (un.tail && tile_begin + n_tiles == planned) ? (cnt_live + kTileTokens - 1) / kTileTokens - tile_begin
+                                                        : n_tiles;
+}
+
 // byte offset (within a partition pool) of K row (layer, slot, g, t)
 __device__ __forceinline__ size_t row_offset(const Dev &d, int layer, int slot, int g, int t) {
     return ((((size_t)layer * d.slots + slot) * d.Hkv + g) * d.R + t) * (size_t)(kHeadDim * 2);
@@ -121,8 +137,8 @@ __device__ __forceinline__ size_t row_offset(const Dev &d, int layer, int slot, 
 // or a negative KF_E* code.
 int launch_open_request(const Dev &d, int req, int n_tokens, cudaStream_t s);
 int launch_close_request(const Dev &d, int req, cudaStream_t s);
-int launch_token_boundary(const Dev &d, cudaStream_t s);
-int launch_plan(const Dev &d, cudaStream_t s);
+int launch_plan(const Dev &d, int do_boundary, cudaStream_t s);  // (a1, optional) + work plan, one launch
+int plan_setup();        // cudaFuncSetAttribute for the plan kernel's dynamic shared memory; 0 or KF_ECUDA
 int launch_step_commit(const Dev &d, cudaStream_t s);
 int launch_load_context(const Dev &d, int layer, int req, int tok_begin, int n_tokens, const __half *k,
                         const __half *v, cudaStream_t s);

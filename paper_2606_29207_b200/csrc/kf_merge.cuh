@@ -61,7 +61,9 @@ __device__ __forceinline__ PieceDest piece_dest(const AttendParams &p, const Uni
 // ascending, whoever calls this, so every path (fused tail, stand-alone kernels) produces the same bits.
 constexpr int kMergeBatch = 16;
 
-__device__ __forceinline__ void merge_rows(const float *src_o, size_t o_stride, const float *src_lse,
+// __noinline__: this code runs once or twice per worker at the very end of a launch, with a cold instruction
+// cache -- one shared copy of it costs far fewer instruction-fetch misses than an inlined copy per call site.
+static __device__ __noinline__ void merge_rows(const float *src_o, size_t o_stride, const float *src_lse,
                                            size_t lse_stride, int n, float *dst_o, float *dst_lse, float *dst2_o,
                                            float *dst2_lse, int lane) {
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -159,7 +161,7 @@ __device__ __forceinline__ void merge_request_head(const Dev &d, const float *o_
 }
 
 // ---- scheduler words and completion counters of one attend launch -----------------------------------------
-// sched[0] chunk ticket, [1] finished workers, [2] unit-merge ticket, [3] request-merge ticket, [4] epoch.
+// sched[0] chunk ticket, [1] finished workers, [2] merge-task ticket, [3] unused, [4] epoch.
 // The completion counters are double-buffered by launch parity: a launch counts in buffer (epoch & 1) and
 // zeroes the other one for the next launch, so nothing has to be reset on the critical path.
 struct Counters {
@@ -223,48 +225,55 @@ __device__ __forceinline__ void wait_counter(const int32_t *ctr, int target, int
 }
 
 // Fused tail: once the chunk list is exhausted every worker turns into a merge worker.
-// Phase A tasks = (unit, head of its group): pieces -> range partial; phase B tasks = (request, query head):
-// range partials -> output.  A task waits until its inputs are complete (the producers are resident workers of
-// this same launch: the grid never exceeds the SM count).  Tickets are taken in batches to bound atomic traffic.
-__device__ __forceinline__ void merge_phase(const AttendParams &p, const Counters &c, int W, int lane) {
+// One ticket stream covers both levels: tasks [0, nA) = (unit, head of its group): pieces -> range partial;
+// tasks [nA, nA + nB) = (request, query head): range partials -> output.  A task waits until its inputs are
+// complete; its producers are either chunks (taken by resident workers of this launch: the grid never exceeds
+// the SM count) or tasks with a LOWER ticket, and every worker serves its tickets in ascending order, so the
+// waits cannot deadlock.  Tickets are taken in batches (bounded atomic traffic on one word) and the next batch
+// is requested before the current one is processed, which keeps the atomic's round trip off the critical path.
+// `first` is lane 0's pre-taken first ticket (merge_first_ticket) or -1.
+__device__ __forceinline__ int merge_batch(const Dev &d, int W) {
+    const int total = __ldg(&d.plan->n_units) * d.G + d.B * d.Hq;
+    return max(1, total / (4 * W));
+}
+__device__ __forceinline__ int merge_first_ticket(const Dev &d, int W) {  // call from ONE lane
+    return atomicAdd(d.sched + 2, merge_batch(d, W));
+}
+
+__device__ __forceinline__ void merge_phase(const AttendParams &p, const Counters &c, int W, int lane, int first = -1) {
     const Dev &d = p.d;
     const int G = d.G, Hkv = d.Hkv;
     const int nA = __ldg(&d.plan->n_units) * G;
-    const int batchA = max(1, nA / (4 * W));
+    const int total = nA + d.B * d.Hq;
+    const int batch = merge_batch(d, W);
+    int next = first;
+    if (lane == 0 && next < 0) next = atomicAdd(d.sched + 2, batch);
     for (;;) {
-        int t0 = 0;
-        if (lane == 0) t0 = atomicAdd(d.sched + 2, batchA);
-        t0 = __shfl_sync(0xffffffffu, t0, 0);
-        if (t0 >= nA) break;
-        const int t1 = min(nA, t0 + batchA);
+        const int t0 = __shfl_sync(0xffffffffu, next, 0);
+        if (t0 >= total) break;
+        if (lane == 0) next = atomicAdd(d.sched + 2, batch);  // in flight while this batch is processed
+        const int t1 = min(total, t0 + batch);
         for (int t = t0; t < t1; ++t) {
-            const int u = t / G, i = t - u * G;
-            const Unit un = d.units[u];
-            if (un.n_pieces <= 1) continue;
-            const int g = u % Hkv;
-            wait_counter(&c.unit[u], un.n_pieces, lane);
-            merge_unit_head(p, un, g, i, true, lane);
-            if (d.scratch[un.req] > 1) {
-                __threadfence();
-                __syncwarp();
-                if (lane == 0) atomicAdd(&c.group[un.req * Hkv + g], 1);
+            if (t < nA) {
+                const int u = t / G, i = t - u * G;
+                const Unit un = d.units[u];
+                if (un.n_pieces <= 1) continue;
+                const int g = u % Hkv;
+                wait_counter(&c.unit[u], un.n_pieces, lane);
+                merge_unit_head(p, un, g, i, true, lane);
+                if (d.scratch[un.req] > 1) {
+                    __threadfence();
+                    __syncwarp();
+                    if (lane == 0) atomicAdd(&c.group[un.req * Hkv + g], 1);
+                }
+            } else {
+                const int tb = t - nA;
+                const int req = tb / d.Hq, h = tb - req * d.Hq;
+                const int J = d.scratch[req];  // 0 for closed requests
+                if (J <= 1) continue;          // a single range: its partial was also written to the output
+                wait_counter(&c.group[req * Hkv + h / G], J * G, lane);
+                merge_request_head(d, p.o_part, p.lse_part, p.o, p.lse, req, h, J, lane);
             }
-        }
-    }
-    const int nB = d.B * d.Hq;
-    const int batchB = max(1, nB / (4 * W));
-    for (;;) {
-        int t0 = 0;
-        if (lane == 0) t0 = atomicAdd(d.sched + 3, batchB);
-        t0 = __shfl_sync(0xffffffffu, t0, 0);
-        if (t0 >= nB) break;
-        const int t1 = min(nB, t0 + batchB);
-        for (int t = t0; t < t1; ++t) {
-            const int req = t / d.Hq, h = t - req * d.Hq;
-            const int J = d.scratch[req];  // 0 for closed requests
-            if (J <= 1) continue;          // a single range: its partial was also written to the output
-            wait_counter(&c.group[req * Hkv + h / G], J * G, lane);
-            merge_request_head(d, p.o_part, p.lse_part, p.o, p.lse, req, h, J, lane);
         }
     }
 }

@@ -72,8 +72,9 @@ __global__ void close_request_kernel(Dev d, int req) {
 }
 
 // (a1) route update: one warp scans the requests 32 at a time; lane 0 allocates in ascending order.
-__global__ void token_boundary_kernel(Dev d) {
-    const int lane = threadIdx.x;
+// returns (in every lane) the number of ranges opened
+__device__ int token_boundary_warp(const Dev &d, int lane) {
+    int opened = 0;
     for (int base = 0; base < d.B; base += 32) {
         const int r = base + lane;
         bool need = false;
@@ -82,6 +83,7 @@ __global__ void token_boundary_kernel(Dev d) {
             need = len >= 0 && (len % d.R) == 0 && d.n_ranges[r] == len / d.R;
         }
         unsigned m = __ballot_sync(0xffffffffu, need);
+        opened += __popc(m);
         if (lane == 0) {
             while (m) {
                 const int b = __ffs(m) - 1;
@@ -91,6 +93,7 @@ __global__ void token_boundary_kernel(Dev d) {
         }
         __syncwarp();
     }
+    return opened;
 }
 
 __global__ void step_commit_kernel(Dev d) {
@@ -183,29 +186,62 @@ __device__ void make_levels(Levels &lv, long long Nt, int W, int m, float f) {
     lv.K = K;
 }
 
-// tiles [b0, b0 + len) of a unit with n tiles belong to level k
+// tiles [b0, b0 + len) of a unit with n tiles belong to level k.  Levels run from the END of the unit towards its
+// start and round up, so level 0 -- the first and largest chunks of the launch -- always holds the unit's last
+// tile: the one place where a tail unit grows between plan rebuilds (live_tiles(), kf_common.cuh).
 __device__ __forceinline__ void level_span(const Levels &lv, int n, int k, int &b0, int &len) {
-    b0 = k == 0 ? 0 : (int)(((long long)n * lv.end16[k - 1]) >> 16);
-    const int b1 = (int)(((long long)n * lv.end16[k]) >> 16);
-    len = b1 - b0;
+    const int lo = k == 0 ? 0 : (int)(((long long)n * lv.end16[k - 1] + 65535) >> 16);
+    const int hi = (int)(((long long)n * lv.end16[k] + 65535) >> 16);
+    b0 = n - hi;
+    len = hi - lo;
 }
 
-// scratch layout (ints): J[B] | S[B] | epre[B+1] | etiles[Emax] | tpre[Emax+1] | ppre[Emax+1] |
-//                        pos[kMaxLevels*Emax+1] | ccnt[kMaxLevels*Emax] | lpre[kMaxLevels*Emax+1]
-__global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d) {
+// scratch (ints): J[B] (always global: the attend kernels read it) | S[B] | epre[B+1] | etiles[E] | tpre[E+1] |
+//                 ppre[E+1] | pos[K*E+1] | ccnt[K*E] | lpre[K*E+1]
+// Every array other than J lives in shared memory when it fits (it does for all BASELINE configs) and in the
+// global scratch area otherwise: the plan is a chain of ~15 dependent phases, and a global round trip per phase
+// is what made this kernel cost 30 us.  With do_boundary != 0 the kernel first performs the route update (a1).
+constexpr int kPlanSmemInts = 48 * 1024;  // 192 KB of dynamic shared memory
+
+__global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
+    extern __shared__ int plan_smem[];
     __shared__ Levels lv;
-    __shared__ int s_m;
+    __shared__ int s_m, s_keep;
     const int tid = threadIdx.x, nt = blockDim.x;
     const int B = d.B, Emax = d.B * d.Jmax, T = kTileTokens, Hkv = d.Hkv;
+    if (do_boundary) {
+        // do_boundary == 1: keep the current plan if no range was opened and it is younger than plan_refresh
+        // boundaries; do_boundary == 2: routes were edited from the host side (open / close): always rebuild
+        if (tid < 32) {
+            const int opened = token_boundary_warp(d, tid);
+            if (tid == 0) {
+                const int age = *d.plan_age;
+                const bool keep = do_boundary == 1 && opened == 0 && age + 1 < d.plan_refresh;
+                *d.plan_age = keep ? age + 1 : 0;
+                s_keep = keep ? 1 : 0;
+            }
+        }
+        __syncthreads();
+        if (s_keep) return;
+    } else if (tid == 0) {
+        *d.plan_age = 0;
+    }
+    int used = 0;
+    auto take = [&](int n, int *fallback) -> int * {
+        if (used + n <= kPlanSmemInts) {
+            int *p = plan_smem + used;
+            used += n;
+            return p;
+        }
+        return fallback;
+    };
     int *Jr = d.scratch;
-    int *Sr = Jr + B;
-    int *epre = Sr + B;
-    int *etiles = epre + (B + 1);
-    int *tpre = etiles + Emax;
-    int *ppre = tpre + (Emax + 1);
-    int *pos = ppre + (Emax + 1);
-    int *ccnt = pos + ((size_t)kMaxLevels * Emax + 1);
-    int *lpre = ccnt + (size_t)kMaxLevels * Emax;
+    int *g_Sr = Jr + B, *g_epre = g_Sr + B, *g_etiles = g_epre + (B + 1), *g_tpre = g_etiles + Emax;
+    int *g_ppre = g_tpre + (Emax + 1), *g_pos = g_ppre + (Emax + 1);
+    int *g_ccnt = g_pos + ((size_t)kMaxLevels * Emax + 1), *g_lpre = g_ccnt + (size_t)kMaxLevels * Emax;
+    int *Sr = take(B, g_Sr);
+    int *epre = take(B + 1, g_epre);
+    int *etiles = nullptr, *tpre = nullptr, *ppre = nullptr, *pos = nullptr, *ccnt = nullptr, *lpre = nullptr;
 
     // 1. per request: tokens attended this step S = len + 1, ranges J = ceil(S / R)
     for (int r = tid; r < B; r += nt) {
@@ -225,6 +261,9 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d) {
     __syncthreads();
     const int E = block_exclusive_scan(epre, B);
     if (tid == 0) epre[B] = E;
+    etiles = take(E, g_etiles);
+    tpre = take(E + 1, g_tpre);
+    ppre = take(E + 1, g_ppre);
     __syncthreads();
 
     // 2. per (request, range) entry: token count and tiles (identical for the H_kv units of the entry)
@@ -253,6 +292,11 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d) {
         if (tid == 0) make_levels(lv, Nt, W, s_m, d.sched_decay);
         __syncthreads();
         const int KE = lv.K * E, m = s_m;
+        if (iter == 0) {  // K only shrinks when min_tiles is coarsened
+            pos = take(KE + 1, g_pos);
+            ccnt = take(KE, g_ccnt);
+            lpre = take(KE + 1, g_lpre);
+        }
         for (int idx = tid; idx < KE; idx += nt) {
             const int k = idx / E, e = idx - k * E;
             int b0, len;
@@ -293,7 +337,7 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d) {
     if (tid == 0) ppre[E] = pieces_per_head;
     __syncthreads();
 
-    // 5. chunk descriptors in level-major order; piece index = unit-major, tile order inside the unit
+    // 5. chunk descriptors in level-major order; piece index = unit-major, (level, tile) order inside the unit
     const int items = K * E * Hkv;
     for (int idx = tid; idx < items; idx += nt) {
         const int k = idx / (E * Hkv);
@@ -308,9 +352,10 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d) {
         const int pu = ppre[e + 1] - ppre[e];
         const int piece0 = ppre[e] * Hkv + g * pu + before;
         const int chunk0 = lpre[k * E + e] + g * c;
+        const int cq = len / c, cr = len - cq * c;  // the first cr chunks hold cq + 1 tiles
         for (int i = 0; i < c; ++i) {
-            const int t0 = b0 + (int)(((long long)i * len) / c);
-            const int t1 = b0 + (int)(((long long)(i + 1) * len) / c);
+            const int t0 = b0 + i * cq + min(i, cr);
+            const int t1 = b0 + (i + 1) * cq + min(i + 1, cr);
             Chunk ch;
             ch.unit = e * Hkv + g;
             ch.tile_begin = t0;
@@ -333,7 +378,7 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d) {
         un.part = d.route_part[(size_t)r * d.Jmax + j];
         un.slot = d.route_slot[(size_t)r * d.Jmax + j];
         un.cnt = min(d.R, Sr[r] - j * d.R);
-        un.tile_begin = tpre[e] + g * etiles[e];
+        un.tail = j == Jr[r] - 1 ? 1 : 0;
         un.piece_begin = ppre[e] * Hkv + g * pu;
         un.n_pieces = pu;
         d.units[u] = un;
@@ -361,13 +406,16 @@ int launch_close_request(const Dev &d, int req, cudaStream_t s) {
     close_request_kernel<<<1, 32, 0, s>>>(d, req);
     return 1;
 }
-int launch_token_boundary(const Dev &d, cudaStream_t s) {
-    token_boundary_kernel<<<1, 32, 0, s>>>(d);
+// do_boundary != 0: route update (a1) followed by the work plan, in one launch
+int launch_plan(const Dev &d, int do_boundary, cudaStream_t s) {
+    plan_kernel<<<1, 1024, kPlanSmemInts * sizeof(int), s>>>(d, do_boundary);
     return 1;
 }
-int launch_plan(const Dev &d, cudaStream_t s) {
-    plan_kernel<<<1, 1024, 0, s>>>(d);
-    return 1;
+int plan_setup() {
+    return cudaFuncSetAttribute(plan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)(kPlanSmemInts * sizeof(int))) == cudaSuccess
+               ? 0
+               : KF_ECUDA;
 }
 int launch_step_commit(const Dev &d, cudaStream_t s) {
     step_commit_kernel<<<(d.B + 255) / 256, 256, 0, s>>>(d);
