@@ -1,0 +1,94 @@
+"""GPU parity of the decode LOOP when the device work plan is kept across steps:
+between rebuilds only the tail range of every request grows, and the attend kernels re-derive its extent from
+`len` at run time.  Every step is checked against the fp64 oracle; routes against the integer model."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from kf_inputs.workloads import Workload  # noqa: E402
+from kf_testlib import check_close, oracle_request  # noqa: E402
+from oracle.routing import RoutingModel  # noqa: E402
+from paper_2606_29207_b200 import KF_ESTATE, KF_IMPL_SIMPLE, KF_IMPL_TMA, KF_OK  # noqa: E402
+from paper_2606_29207_b200.workload import Session  # noqa: E402
+
+IMPLS = [KF_IMPL_SIMPLE, KF_IMPL_TMA]
+
+
+def _decode_loop(wl, impl, steps, refresh, fused=True, min_tiles=0, check_every=1):
+    ses = Session(wl, impl=impl, steps=steps, min_tiles=min_tiles, plan_refresh_steps=refresh)
+    ses.prepare()
+    kf = ses.kf
+    model = RoutingModel(wl.n_partitions, wl.range_tokens, wl.batch, kf.Jmax, kf.cfg.slots_per_partition)
+    for r, n in enumerate(ses.len0):
+        model.open_request(r, n)
+    outs = []
+    for step in range(steps):
+        kf.token_boundary()
+        model.token_boundary()
+        q = ses.q_for(0, step)
+        k_new, v_new = ses.kv_new_for(0, step)
+        ses.o.fill_(float("nan"))
+        ses.lse.fill_(float("nan"))
+        ses.layer_step(0, q, k_new, v_new, fused=fused)
+        kf.step_commit()
+        model.step_commit()
+        assert kf.status() == KF_OK
+        o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+        outs.append((o.copy(), lse.copy()))
+        if step % check_every == 0 or step == steps - 1:
+            for r, S0 in enumerate(wl.contexts):
+                o_ref, lse_ref = oracle_request(wl, 0, r, step, S0 + step)
+                check_close(o[r], lse[r], o_ref, lse_ref, f"{wl.name} step{step} r{r} impl{impl} refresh{refresh}")
+    snap, ms = kf.route_snapshot(), model.snapshot()
+    for key in ("len", "n_ranges", "part", "slot", "free_head", "rr_cursor"):
+        assert snap[key] == ms[key], key
+    ses.close()
+    return outs
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+@pytest.mark.parametrize("refresh", [0, 1, 5])
+def test_kept_plan_decode_loop_matches_oracle(impl, refresh):
+    # contexts chosen so that within 40 steps: tails cross 16-token tile edges many times, request 1 fills its
+    # range at step 3 (128 -> new range, forces a rebuild), request 3 starts with a 1-token tail range, request 4
+    # sits one token before a tile edge, and the plan ages past `refresh` (0 = default 128: never, 1: every step)
+    wl = Workload("kept_plan", 32, 8, 64, 3, [200, 125, 33, 65, 16, 1])
+    _decode_loop(wl, impl, steps=40, refresh=refresh)
+
+
+def test_kept_plan_many_pieces_and_unfused():
+    # min_tiles = 1: every tile its own piece, so the stretched level-0 chunk sits among many small pieces
+    wl = Workload("kept_plan_pieces", 64, 8, 512, 2, [1500, 700, 511])
+    a = _decode_loop(wl, KF_IMPL_TMA, steps=36, refresh=0, fused=True, min_tiles=1, check_every=5)
+    b = _decode_loop(wl, KF_IMPL_TMA, steps=36, refresh=0, fused=False, min_tiles=1, check_every=5)
+    for (oa, la), (ob, lb) in zip(a, b):     # same plan history => same cuts => bit-identical
+        assert np.array_equal(oa, ob) and np.array_equal(la, lb)
+
+
+def test_attend_after_commit_without_boundary():
+    # a commit invalidates the plan on the host side: an attend that follows it without kf_token_boundary rebuilds
+    # the plan; if the new position has no route (tail range full) the device reports ESTATE, as before
+    wl = Workload("no_boundary", 32, 8, 64, 2, [63, 10])
+    ses = Session(wl, steps=4)
+    ses.prepare()
+    kf = ses.kf
+    kf.token_boundary()
+    q = ses.q_for(0, 0)
+    k_new, v_new = ses.kv_new_for(0, 0)
+    ses.layer_step(0, q, k_new, v_new)
+    kf.step_commit()                      # len = 63, 10: position 63 still has a route
+    q = ses.q_for(0, 1)
+    k_new, v_new = ses.kv_new_for(0, 1)
+    ses.layer_step(0, q, k_new, v_new)    # no boundary call
+    assert kf.status() == KF_OK
+    o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+    for r, S0 in enumerate(wl.contexts):
+        o_ref, lse_ref = oracle_request(wl, 0, r, 1, S0 + 1)
+        check_close(o[r], lse[r], o_ref, lse_ref, f"no_boundary r{r}")
+    kf.step_commit()                      # len = 64: request 0 needs a new range, none was opened
+    ses.layer_step(0, q, k_new, v_new)
+    assert kf.status() == KF_ESTATE
+    ses.close()
