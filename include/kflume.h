@@ -172,6 +172,32 @@ int kf_step_commit(kf_ctx *ctx, kf_stream stream);
 int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host,
                        const void *v_new_host, float *o_host, float *lse_host, kf_stream stream);
 
+/* ---- one decode step as a static CUDA graph ----------------------------------------------------------
+ * The paper keeps the W-node computation in one static CUDA Graph and confines elasticity to a routing table the
+ * graph never sees (PAPER.md:127 requirement R1, :165-179).  The same holds here: every hot kernel launches a
+ * fixed grid and reads lengths, routes and the work plan from device memory, so ONE captured graph of
+ *     kf_token_boundary -> for i < n: { kf_kv_append(layers[i], k_new[i], v_new[i]);
+ *                                       kf_attend(layers[i], q[i], o[i], lse[i]) } -> kf_step_commit
+ * is replayed for every decode step, across range fills, route updates and kf_open/close_request, without
+ * re-capture.  A replay also removes the submission latency between the small kernels of a step.
+ * kf_step_graph_create: captures on `stream` (must not be the legacy default stream; nothing executes) and
+ *   instantiates.  layers: [host] int32[n], physical layer of each layer-step.  q, k_new, v_new, o, lse: [host]
+ *   arrays of n pointers, shapes as in kf_kv_append / kf_attend.  host_io == 0: they are [device] pointers and may
+ *   be re-bound at every launch.  host_io != 0: they are PINNED [host] buffers (the end-to-end path: each
+ *   layer-step copies q / k_new / v_new to device staging and o / lse back); they are bound for the graph's
+ *   lifetime -- the caller rewrites their contents between launches (pre-registered buffers).
+ * kf_step_graph_launch: one decode step.  q .. lse: all NULL = keep the bound pointers; else all five arrays
+ *   [host, n pointers each] re-bind the device pointers (host-side node update; no re-instantiation).
+ *   Asynchronous on `stream`.  Errors as the calls it contains (device errors via kf_status).
+ * kf_step_graph_destroy: frees the graph; the ctx must still be alive. */
+typedef struct kf_graph kf_graph;
+int kf_step_graph_create(kf_ctx *ctx, int32_t n_layer_steps, const int32_t *layers, int32_t host_io,
+                         const void *const *q, const void *const *k_new, const void *const *v_new, float *const *o,
+                         float *const *lse, kf_stream stream, kf_graph **out);
+int kf_step_graph_launch(kf_graph *graph, const void *const *q, const void *const *k_new, const void *const *v_new,
+                         float *const *o, float *const *lse, kf_stream stream);
+int kf_step_graph_destroy(kf_graph *graph);
+
 /* ---- inspection (tests, tools) -------------------------------------------------------------------
  * kf_route_snapshot: downloads the routing state into [host] arrays (any may be NULL):
  *   len[B] (-1 = closed), n_ranges[B], part[B][Jmax], slot[B][Jmax] (-1 where unused), free_head[P],

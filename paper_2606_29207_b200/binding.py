@@ -18,6 +18,7 @@ EXPORTS = [
     "kf_create", "kf_destroy", "kf_open_request", "kf_close_request", "kf_load_context", "kf_token_boundary",
     "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_step_commit", "kf_layer_step_host",
     "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count", "kf_worker_times",
+    "kf_step_graph_create", "kf_step_graph_launch", "kf_step_graph_destroy",
 ]
 
 
@@ -74,6 +75,10 @@ def load_library():
     L.kf_plan_info.argtypes = [vp, ctypes.POINTER(i32), vp]
     L.kf_launch_count.argtypes, L.kf_launch_count.restype = [vp], i64
     L.kf_worker_times.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i32), vp]
+    pp = ctypes.POINTER(vp)
+    L.kf_step_graph_create.argtypes = [vp, i32, ctypes.POINTER(i32), i32, pp, pp, pp, pp, pp, vp, ctypes.POINTER(vp)]
+    L.kf_step_graph_launch.argtypes = [vp, pp, pp, pp, pp, pp, vp]
+    L.kf_step_graph_destroy.argtypes = [vp]
     for name in EXPORTS:
         if getattr(L, name).restype is None:
             getattr(L, name).restype = ctypes.c_int
@@ -229,6 +234,10 @@ class KFlume:
                                                 _ptr(o_host), _ptr(lse_host), self._stream(stream)),
                     "kf_layer_step_host")
 
+    def step_graph_create(self, layers: Sequence[int], q, k_new, v_new, o, lse, host_io: bool = False, stream=None):
+        """kf_step_graph_create: q .. lse are lists (one tensor per layer-step).  Returns a StepGraph."""
+        return StepGraph(self, layers, q, k_new, v_new, o, lse, host_io, stream)
+
     def route_snapshot(self, stream=None) -> dict:
         i32 = ctypes.c_int32
         ln, nr = (i32 * self.B)(), (i32 * self.B)()
@@ -263,3 +272,44 @@ class KFlume:
 
     def pool_offset(self, layer: int, slot: int, kv_head: int, token: int, is_v: bool) -> int:
         return int(self.lib.kf_pool_offset(ctypes.byref(self.cfg), layer, slot, kv_head, token, 1 if is_v else 0))
+
+
+class StepGraph:
+    """kf_graph handle: one decode step (token boundary, n x (append, attend), commit) as a static CUDA graph."""
+
+    def __init__(self, kf: KFlume, layers, q, k_new, v_new, o, lse, host_io=False, stream=None):
+        self.kf, self.n, self.host_io = kf, len(layers), bool(host_io)
+        for lst in (q, k_new, v_new, o, lse):
+            assert len(lst) == self.n
+            for t in lst:
+                assert t.is_contiguous() and t.is_cuda != self.host_io
+        self._keep = (list(q), list(k_new), list(v_new), list(o), list(lse))  # bound buffers stay alive
+        arr = (ctypes.c_int32 * self.n)(*layers)
+        h = ctypes.c_void_p()
+        kf._check(kf.lib.kf_step_graph_create(kf.h, self.n, arr, 1 if host_io else 0, *self._arrays(*self._keep),
+                                              kf._stream(stream), ctypes.byref(h)), "kf_step_graph_create")
+        self.h = h
+
+    def _arrays(self, q, k_new, v_new, o, lse):
+        return [(ctypes.c_void_p * self.n)(*[t.data_ptr() for t in lst]) for lst in (q, k_new, v_new, o, lse)]
+
+    def launch(self, q=None, k_new=None, v_new=None, o=None, lse=None, stream=None):
+        """One decode step.  Pass all five lists to re-bind the device pointers, or none to keep them."""
+        if q is None:
+            args = [None] * 5
+        else:
+            self._keep = (list(q), list(k_new), list(v_new), list(o), list(lse))
+            args = self._arrays(*self._keep)
+        self.kf._check(self.kf.lib.kf_step_graph_launch(self.h, *args, self.kf._stream(stream)), "kf_step_graph_launch")
+
+    def destroy(self):
+        if getattr(self, "h", None) and self.kf.h:
+            self.kf.torch.cuda.synchronize(self.kf.device)
+            self.kf.lib.kf_step_graph_destroy(self.h)
+        self.h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -8,21 +8,16 @@
 
 #include <new>
 
-#include "kf_common.cuh"
+#include "kf_ctx.h"
 
 using namespace kf;
 
-struct kf_ctx {
-    kf_config cfg;
-    Dev dev;
-    int sm_count;
-    int n_ctas;
-    int impl;
-    bool plan_dirty;    // lengths moved (step commit) or routes were edited since the plan kernel last ran
-    bool routes_dirty;  // routes were edited from the host side (open / close / create): the next plan must be rebuilt
-    int64_t launches;
-    char cuda_err[256];
-};
+namespace kf {
+int cuda_fail(kf_ctx *ctx, cudaError_t e) {
+    if (ctx) snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+    return KF_ECUDA;
+}
+}  // namespace kf
 
 namespace {
 
@@ -118,10 +113,6 @@ size_t half_pool_bytes(const kf_config *c) {
     return (size_t)c->n_layers * c->slots_per_partition * c->n_kv_heads * c->range_tokens * (size_t)(kHeadDim * 2);
 }
 
-int cuda_fail(kf_ctx *ctx, cudaError_t e) {
-    if (ctx) snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
-    return KF_ECUDA;
-}
 
 // after a launch: count it, surface launch errors
 int after_launch(kf_ctx *ctx, int n) {
@@ -179,7 +170,7 @@ int encode_tmaps(kf_ctx *ctx, void *const *pools) {
 int ensure_plan(kf_ctx *ctx, cudaStream_t s) {
     if (!ctx->plan_dirty) return KF_OK;
     const int rc = after_launch(ctx, launch_plan(ctx->dev, 0, s));
-    if (rc == KF_OK) ctx->plan_dirty = ctx->routes_dirty = false;
+    if (rc == KF_OK) ctx->plan_dirty = false;
     return rc;
 }
 
@@ -248,7 +239,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     const int warps = ctx->impl == KF_IMPL_SIMPLE ? kWarpsPerCta : (cfg->workers_per_sm ? cfg->workers_per_sm : kDefaultWarps);
     ctx->n_ctas = ctx->sm_count;
     if (ctx->n_ctas * warps > kMaxWorkers) ctx->n_ctas = kMaxWorkers / warps;
-    ctx->plan_dirty = ctx->routes_dirty = true;
+    ctx->plan_dirty = true;
 
     unsigned char *ws = (unsigned char *)workspace;
     e = cudaMemset(ws, 0, L.total);
@@ -257,6 +248,9 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     e = cudaMemset(ws + L.len, 0xFF, (size_t)cfg->max_requests * 4);
     if (e == cudaSuccess) e = cudaMemset(ws + L.route_part, 0xFF, (size_t)cfg->max_requests * cfg->max_ranges_per_request * 4);
     if (e == cudaSuccess) e = cudaMemset(ws + L.route_slot, 0xFF, (size_t)cfg->max_requests * cfg->max_ranges_per_request * 4);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    const int32_t stale = kPlanStale;  // no plan yet: the first plan kernel builds one
+    e = cudaMemcpy(ws + L.plan_age, &stale, 4, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
 
     Dev &d = ctx->dev;
@@ -330,13 +324,13 @@ int kf_destroy(kf_ctx *ctx) {
 
 int kf_open_request(kf_ctx *ctx, int32_t req, int32_t n_tokens, kf_stream stream) {
     if (!ctx || req < 0 || req >= ctx->cfg.max_requests || n_tokens < 0) return KF_EINVAL;
-    ctx->plan_dirty = ctx->routes_dirty = true;
+    ctx->plan_dirty = true;
     return after_launch(ctx, launch_open_request(ctx->dev, req, n_tokens, (cudaStream_t)stream));
 }
 
 int kf_close_request(kf_ctx *ctx, int32_t req, kf_stream stream) {
     if (!ctx || req < 0 || req >= ctx->cfg.max_requests) return KF_EINVAL;
-    ctx->plan_dirty = ctx->routes_dirty = true;
+    ctx->plan_dirty = true;
     return after_launch(ctx, launch_close_request(ctx->dev, req, (cudaStream_t)stream));
 }
 
@@ -355,8 +349,10 @@ int kf_token_boundary(kf_ctx *ctx, kf_stream stream) {
     if (!ctx) return KF_EINVAL;
     // route update and work plan in ONE launch (the plan depends on the routes the update appends)
     // (the plan is kept when no route changed and it is younger than plan_refresh_steps boundaries)
-    const int rc = after_launch(ctx, launch_plan(ctx->dev, ctx->routes_dirty ? 2 : 1, (cudaStream_t)stream));
-    if (rc == KF_OK) ctx->plan_dirty = ctx->routes_dirty = false;
+    // open / close / create invalidate the plan on the DEVICE (plan_age), so this launch is the same whatever
+    // happened before it -- a CUDA graph that contains it stays valid (kf_step_graph_*).
+    const int rc = after_launch(ctx, launch_plan(ctx->dev, 1, (cudaStream_t)stream));
+    if (rc == KF_OK) ctx->plan_dirty = false;
     return rc;
 }
 

@@ -19,6 +19,7 @@ constexpr int kMaxLevels = 16;        // levels of the guided self-scheduling ch
 constexpr int kChunkSlack = 16 * kMaxWorkers;  // chunk capacity = units + kChunkSlack
 constexpr int kMaxGroup = 8;          // G = H_q / H_kv
 constexpr int kMaxPartitions = 64;
+constexpr int kPlanStale = 1 << 30;    // plan_age value that forces a rebuild at the next token boundary
 
 // One unit of attention work: (request, token range, kv head).  Built by the plan kernel.
 struct Unit {

@@ -45,6 +45,7 @@ __global__ void open_request_kernel(Dev d, int req, int n_tokens) {
         set_error(d, KF_ESTATE);
         return;
     }
+    *d.plan_age = kPlanStale;  // routes edited: the next plan kernel must rebuild
     d.len[req] = n_tokens;
     d.n_ranges[req] = 0;
     const int J = (int)(((int64_t)n_tokens + d.R - 1) / d.R);
@@ -58,6 +59,7 @@ __global__ void close_request_kernel(Dev d, int req) {
         set_error(d, KF_ESTATE);
         return;
     }
+    *d.plan_age = kPlanStale;
     const int J = d.n_ranges[req];
     for (int j = 0; j < J; ++j) {
         const int p = d.route_part[(size_t)req * d.Jmax + j];
@@ -210,13 +212,13 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
     const int tid = threadIdx.x, nt = blockDim.x;
     const int B = d.B, Emax = d.B * d.Jmax, T = kTileTokens, Hkv = d.Hkv;
     if (do_boundary) {
-        // do_boundary == 1: keep the current plan if no range was opened and it is younger than plan_refresh
-        // boundaries; do_boundary == 2: routes were edited from the host side (open / close): always rebuild
+        // keep the current plan if no range was opened and it is younger than plan_refresh boundaries
+        // (kf_open_request / kf_close_request / kf_create age it to kPlanStale: always rebuilt)
         if (tid < 32) {
             const int opened = token_boundary_warp(d, tid);
             if (tid == 0) {
                 const int age = *d.plan_age;
-                const bool keep = do_boundary == 1 && opened == 0 && age + 1 < d.plan_refresh;
+                const bool keep = opened == 0 && age + 1 < d.plan_refresh;
                 *d.plan_age = keep ? age + 1 : 0;
                 s_keep = keep ? 1 : 0;
             }
