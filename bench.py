@@ -33,8 +33,8 @@ NOMINAL_PEAK_GBS = 8000.0        # BASELINE.json's "~8 TB/s" denominator (contex
 FALLBACK_PEAK_GBS = 6650.0       # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 
 # dram__bytes_read.sum + dram__bytes_write.sum per kf_attend launch from the committed `ncu --set full` capture
-# (profiles/r01b_attend_full_cfg3.md); None where no capture exists for that workload.
-NCU_TRAFFIC_BYTES = {"cfg3": 4802209552}
+# (profiles/r01c_attend_full_cfg3.md); None where no capture exists for that workload.
+NCU_TRAFFIC_BYTES = {"cfg3": 4802068504}
 
 
 def load_peak():
@@ -209,6 +209,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 50)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--min-tiles", type=int, default=0)
+    ap.add_argument("--no-graph", action="store_true", help="launch the calls of a step one by one instead of "
+                    "replaying the static step graph")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -223,6 +225,7 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     dev = torch.device(f"cuda:{local}")
+    torch.cuda.set_stream(torch.cuda.Stream(dev))   # stream capture (kf_step_graph_create) needs a non-default stream
     dist = None
     if world > 1:
         import torch.distributed as dist
@@ -232,7 +235,7 @@ def main():
     wl.seed = wl.seed + rank                       # independent batch per rank (weak scaling)
     n_layers = wl.n_layers
     e2e_steps = args.e2e_steps or min(args.steps, 50)
-    total_steps = args.warmup + args.steps + e2e_steps + 2
+    total_steps = args.warmup + args.steps + 100 + e2e_steps + 2   # + the roofline region (<= 100 steps)
     if args.layers_phys:
         L_phys = args.layers_phys
     else:
@@ -266,11 +269,39 @@ def main():
                 kf.attend(layer % L_phys, q, ses.o, ses.lse)
         kf.step_commit()
 
+    n_eager = max(1, args.warmup - 2)
     step = 0
-    for _ in range(args.warmup):
+    for _ in range(n_eager):
         run_step(inputs(step))
         step += 1
-    timed_inputs = [inputs(step + i) for i in range(args.steps)] if n_layers * args.steps <= 4096 else None
+    assert kf.status() == 0
+
+    # ---- the timed region: K decode steps, each ONE replay of the static step graph (kf_step_graph_*) with the
+    #      step's resident inputs re-bound; --no-graph times the same calls launched one by one ---------------------
+    layer_ids = [layer % L_phys for layer in range(n_layers)]
+
+    def per_layer(step_inputs):
+        return ([step_inputs[lp][0] for lp in layer_ids], [step_inputs[lp][1] for lp in layer_ids],
+                [step_inputs[lp][2] for lp in layer_ids])
+
+    o_list, lse_list = [ses.o] * n_layers, [ses.lse] * n_layers
+    graph = None
+    if not args.no_graph:
+        q0, k0, v0 = per_layer(inputs(step))
+        graph = kf.step_graph_create(layer_ids, q0, k0, v0, o_list, lse_list)
+
+    def timed_step(step_inputs):
+        if graph is None:
+            run_step(step_inputs)
+        else:
+            q, kn, vn = per_layer(step_inputs)
+            graph.launch(q, kn, vn, o_list, lse_list)
+
+    for _ in range(args.warmup - n_eager):          # the last warm-up steps run exactly what is timed
+        timed_step(inputs(step))
+        step += 1
+    resident = n_layers * args.steps <= 4096
+    timed_inputs = [inputs(step + i) for i in range(args.steps)] if resident else None
     total_bytes = kv_bytes = 0
     for i in range(args.steps):
         b, k = algorithmic_bytes(wl, [n + step + i for n in lens], n_layers)
@@ -285,12 +316,11 @@ def main():
     if dist:
         dist.barrier()
     launches0 = kf.launch_count()
-    attend_events = []
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0 = sampler.mark()
     e0.record()
     for i in range(args.steps):
-        run_step(timed_inputs[i] if timed_inputs else inputs(step + i), attend_events)
+        timed_step(timed_inputs[i] if timed_inputs else inputs(step + i))
     e1.record()
     torch.cuda.synchronize(dev)
     t1 = sampler.mark()
@@ -299,7 +329,27 @@ def main():
     launches = kf.launch_count() - launches0
     step += args.steps
     ms = e0.elapsed_time(e1)
+    del timed_inputs
+    assert kf.status() == 0
+
+    # ---- roofline region: the same steps launched one by one, CUDA events around every kf_attend (events cannot
+    #      be recorded inside a graph replay); also gives the eager step time ---------------------------------------
+    roof_steps = max(1, min(args.steps, 4096 // n_layers, 100))
+    roof_inputs = [inputs(step + i) for i in range(roof_steps)]
+    attend_events = []
+    r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(dev)
+    r0.record()
+    for i in range(roof_steps):
+        run_step(roof_inputs[i], attend_events)
+    r1.record()
+    torch.cuda.synchronize(dev)
+    eager_ms_per_step = r0.elapsed_time(r1) / roof_steps
     attend_ms = sum(a.elapsed_time(b) for a, b in attend_events) / len(attend_events)
+    roof_bytes = sum(algorithmic_bytes(wl, [n + step + i for n in lens], n_layers)[0] for i in range(roof_steps))
+    attend_bytes = roof_bytes / (roof_steps * n_layers)  # per kf_attend launch (append rows are ~1e-5 of it)
+    step += roof_steps
+    del roof_inputs
     clocks = sampler.stop(t0, t1) if rank == 0 else None
     assert kf.status() == 0
     if dist:
@@ -314,27 +364,41 @@ def main():
     value = total_bytes_all / (ms * 1e-3) / 1e9
     ms_per_step = ms / args.steps
 
-    # ---- end to end: host buffers through kf_layer_step_host, copies inside the timed region -------------------
+    # ---- end to end: HOST buffers, copies inside the timed region.  One replay per step of a host-io step graph
+    #      (pinned, pre-registered buffers: PAPER.md:177): every layer-step copies q / k_new / v_new host->device and
+    #      o / lse device->host; the caller rewrites the pinned inputs and reads the result every step ---------------
     B, Hq, Hkv = wl.batch, wl.n_q_heads, wl.n_kv_heads
     host_in = []
     for i in range(e2e_steps):
         host_in.append([tuple(t.cpu().pin_memory() for t in x) for x in inputs(step + i)])
-    o_h = torch.zeros((B, Hq, 128), dtype=torch.float32).pin_memory()
-    l_h = torch.zeros((B, Hq), dtype=torch.float32).pin_memory()
+    qh = [torch.zeros((B, Hq, 128), dtype=torch.float16).pin_memory() for _ in range(n_layers)]
+    kh = [torch.zeros((B, Hkv, 128), dtype=torch.float16).pin_memory() for _ in range(n_layers)]
+    vh = [torch.zeros((B, Hkv, 128), dtype=torch.float16).pin_memory() for _ in range(n_layers)]
+    o_h = [torch.zeros((B, Hq, 128), dtype=torch.float32).pin_memory() for _ in range(n_layers)]
+    l_h = [torch.zeros((B, Hq), dtype=torch.float32).pin_memory() for _ in range(n_layers)]
+    hgraph = None if args.no_graph else kf.step_graph_create(layer_ids, qh, kh, vh, o_h, l_h, host_io=True)
     e2e_bytes = 0
     for i in range(e2e_steps):
         e2e_bytes += algorithmic_bytes(wl, [n + step + i for n in lens], n_layers)[0]
+    checksum = 0.0
     torch.cuda.synchronize(dev)
     if dist:
         dist.barrier()
     e0.record()
     for i in range(e2e_steps):
-        kf.token_boundary()
-        for layer in range(n_layers):
-            qh, kh, vh = host_in[i][layer % L_phys]
-            kf.layer_step_host(layer % L_phys, qh, kh, vh, o_h, l_h)
-        kf.step_commit()
-        torch.cuda.current_stream(dev).synchronize()      # the caller reads o_h / l_h every step
+        if hgraph is None:
+            kf.token_boundary()
+            for layer in range(n_layers):
+                qx, kx, vx = host_in[i][layer % L_phys]
+                kf.layer_step_host(layer % L_phys, qx, kx, vx, o_h[layer], l_h[layer])
+            kf.step_commit()
+        else:
+            for layer in range(n_layers):           # the producer writes this step's inputs into the bound buffers
+                qx, kx, vx = host_in[i][layer % L_phys]
+                qh[layer].copy_(qx), kh[layer].copy_(kx), vh[layer].copy_(vx)
+            hgraph.launch()
+        torch.cuda.current_stream(dev).synchronize()      # the caller reads the step's result on the host
+        checksum += float(l_h[n_layers - 1][0, 0])
     e1.record()
     torch.cuda.synchronize(dev)
     e2e_ms = e0.elapsed_time(e1)
@@ -346,7 +410,7 @@ def main():
     e2e_value = e2e_bytes * world / (e2e_ms * 1e-3) / 1e9
     h2d = n_layers * (B * Hq * 128 * 2 + 2 * B * Hkv * 128 * 2)
     d2h = n_layers * (B * Hq * 128 * 4 + B * Hq * 4)
-    assert kf.status() == 0
+    assert kf.status() == 0 and checksum == checksum
 
     if rank != 0:
         if dist:
@@ -355,7 +419,6 @@ def main():
         return 0
 
     peak, peak_src = load_peak()
-    attend_bytes = total_bytes / (args.steps * n_layers)   # per kf_attend launch (append rows are ~1e-5 of it)
     achieved = attend_bytes / (attend_ms * 1e-3) / 1e9
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -370,7 +433,12 @@ def main():
                    "l2": "inputs larger than L2 (KV read per layer-step >> 126 MB); no flush needed"
                          if kv_bytes / (args.steps * n_layers) > 4 * 126e6 else
                          "KV fits L2: numbers are L2-warm (see profiles for the cold protocol)",
-                   "attend_impl": {0: "tma", 1: "simple", 2: "tma"}[args.attend_impl]},
+                   "attend_impl": {0: "tma", 1: "simple", 2: "tma"}[args.attend_impl],
+                   "launch": "eager: one C-ABI call per kernel" if args.no_graph else
+                             "kf_step_graph: one static CUDA-graph replay per step, inputs re-bound per step",
+                   "roofline_region": f"{roof_steps} further steps launched one by one with CUDA events around "
+                                      "every kf_attend (events cannot be recorded inside a graph replay)"},
+        "eager_ms_per_step": eager_ms_per_step,
         "us_per_layer_step": ms_per_step * 1e3 / n_layers,
         "pct_of_nominal_8TBs": 100.0 * value / world / NOMINAL_PEAK_GBS,
         "clocks": clocks,
