@@ -133,6 +133,27 @@ def tiny_t0() -> Workload:
     return Workload("t0", 8, 2, 4, 2, [5], note="tiny: ranges [0,4) and [4,5)")
 
 
+FIG10_HEADS = [(32, 8), (48, 8), (64, 8), (32, 32), (40, 40), (48, 48)]   # PAPER.md:322 (Fig. 10)
+
+
+def fig10(n_q_heads: int, n_kv_heads: int, batch: int, seq: int, range_tokens: int = 8 * K,
+          n_partitions: int = 4) -> Workload:
+    """Head-shape sweep of the paper's Fig. 10: six head configurations (GQA Q32:KV8, Q48:KV8,
+    Q64:KV8; MHA Q32:KV32, Q40:KV40, Q48:KV48), batch 8-128, sequence 2K-32K; every request at context `seq`, KV cut
+    into 8K-token ranges routed round-robin over 4 emulated attention nodes."""
+    assert (n_q_heads, n_kv_heads) in FIG10_HEADS and 8 <= batch <= 128 and 2 * K <= seq <= 32 * K
+    return Workload(f"fig10_q{n_q_heads}kv{n_kv_heads}_b{batch}_s{seq // K}k", n_q_heads, n_kv_heads, range_tokens,
+                    n_partitions, [seq] * batch,
+                    note=f"Fig. 10 shape Q{n_q_heads}:KV{n_kv_heads}, batch {batch}, every request at context {seq}, "
+                         f"{range_tokens // K}K ranges over {n_partitions} partitions")
+
+
 def by_name(name: str) -> Workload:
+    if name.startswith("fig10_"):      # fig10_q<Hq>kv<Hkv>_b<batch>_s<seq in K>k
+        import re
+        m = re.fullmatch(r"fig10_q(\d+)kv(\d+)_b(\d+)_s(\d+)k", name)
+        if not m:
+            raise KeyError(name)
+        return fig10(int(m.group(1)), int(m.group(2)), int(m.group(3)), int(m.group(4)) * K)
     return {"cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4, "cfg5": cfg5,
             "cfg5_twin": cfg5_twin, "t0": tiny_t0}[name]()

@@ -203,3 +203,23 @@ def test_cfg5_full_size_aliased_layers():
     assert [[p, s] for p, s in zip(snap["part"][0], snap["slot"][0]) if p >= 0] == g["request0_final_route"]
     assert [[p, s] for p, s in zip(snap["part"][120], snap["slot"][120]) if p >= 0] == g["request120_final_route"]
     ses.close()
+
+
+# ---- the head shapes of the paper's Fig. 10, at bench sizes ----------------
+@pytest.mark.parametrize("name,reqs,heads", [
+    ("fig10_q32kv32_b8_s8k", (0, 7), [0, 13, 31]),        # MHA, G = 1
+    ("fig10_q40kv40_b8_s2k", (3,), [0, 39]),              # MHA, 40 KV heads
+    ("fig10_q48kv8_b8_s32k", (0, 5), [0, 17, 47]),        # GQA, G = 6: rows 6, 7 of the MMA tile are padding
+    ("fig10_q64kv8_b16_s8k", (15,), [7, 8, 63]),          # GQA, G = 8
+])
+def test_fig10_head_shapes_sampled(name, reqs, heads):
+    wl = workloads.by_name(name)
+    ses = _static_run(wl)
+    o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+    op, lp = ses.o_part.cpu().numpy(), ses.lse_part.cpu().numpy()
+    assert np.isfinite(o).all() and np.isfinite(lse).all()
+    for r in reqs:
+        _check_request(wl, (o, lse), 0, r, 0, wl.contexts[r], heads, op, lp, name)
+    # all requests see different q/K/V but the same context length: lse ~ ln S + scale^2 |q|^2 / 2 (loose sanity)
+    assert np.all(np.abs(lse - (np.log(wl.contexts[0]) + 0.5)) < 1.0)
+    ses.close()

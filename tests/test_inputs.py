@@ -78,3 +78,16 @@ def test_workload_shapes():
     assert workloads.cfg3().max_ranges() == 6
     w5 = workloads.cfg5()
     assert w5.batch == 128 and w5.max_ranges() == 9 and w5.total_ranges() == 625
+
+
+def test_fig10_workload_names_parse_to_the_papers_head_shapes():
+    # PAPER.md:322 (Fig. 10): GQA Q32:KV8, Q48:KV8, Q64:KV8; MHA Q32:KV32, Q40:KV40, Q48:KV48; batch 8-128; seq 2K-32K
+    from kf_inputs import workloads
+    for hq, hkv in workloads.FIG10_HEADS:
+        wl = workloads.by_name(f"fig10_q{hq}kv{hkv}_b16_s32k")
+        assert (wl.n_q_heads, wl.n_kv_heads, wl.batch, wl.contexts[0]) == (hq, hkv, 16, 32768)
+        assert wl.kv_bytes_per_token() == 2 * hkv * 128 * 2            # PAPER.md:234, per layer
+        assert wl.max_ranges(1) == 4 and wl.slots_per_partition(1) == 16
+    import pytest
+    with pytest.raises((KeyError, AssertionError)):
+        workloads.by_name("fig10_q33kv8_b16_s32k")
