@@ -71,12 +71,13 @@ typedef struct kf_config {
     int32_t slots_per_partition;    /* token-range slots in each partition pool                   */
     float softmax_scale;            /* 0 => 1/sqrt(head_dim); scores are scale * q.k              */
     int32_t attend_impl;            /* KF_IMPL_*                                                  */
-    int32_t min_tiles_per_worker;   /* 0 => default (4); smallest chunk of the work plan, in 16-token tiles */
+    int32_t min_tiles_per_worker;   /* smallest chunk of the work plan, in 16-token tiles; 0 => 8 when the step has at
+                                     * least 16 tiles per worker, else 4 */
     /* tuning of the attend kernel and its work plan; 0 => default.  Results are bit-identical for a given
      * (min_tiles_per_worker, workers_per_sm, sched_*) because the plan's cuts depend only on these. */
     int32_t workers_per_sm;         /* warps (independent workers) per SM: 4 or 8                  */
     int32_t pipeline_stages;        /* 8 KB TMA stages in flight per worker: 2..6 (2..3 for 8 workers) */
-    int32_t sched_first_pct;        /* 1..100: guided self-scheduling factor: chunk <= pct% of (remaining tiles / workers) */
+    int32_t sched_first_pct;        /* 1..100 (0 => 100): guided self-scheduling factor: chunk <= pct% of (remaining tiles / workers) */
     int32_t sched_decay_pct;        /* 1..99: share of a unit's remaining tiles that each scheduling level takes */
     int32_t plan_refresh_steps;     /* the work plan is rebuilt when a route changes or after this many token boundaries
                                      * (0 => 128; 1 => every step); in between, tail ranges grow inside the kept plan */

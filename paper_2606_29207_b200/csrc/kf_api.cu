@@ -23,7 +23,7 @@ namespace {
 
 constexpr size_t kAlign = 256;
 constexpr int kDefaultWarps = 8, kDefaultStages = 3;
-constexpr int kDefaultFirstPct = 80, kDefaultDecayPct = 50;
+constexpr int kDefaultFirstPct = 100, kDefaultDecayPct = 50;
 constexpr int kDefaultPlanRefresh = 128;
 
 size_t max_chunks_of(const kf_config *c) {
@@ -264,7 +264,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.Jmax = cfg->max_ranges_per_request;
     d.slots = cfg->slots_per_partition;
     d.max_workers = ctx->n_ctas * warps;
-    d.min_tiles = cfg->min_tiles_per_worker > 0 ? cfg->min_tiles_per_worker : 4;
+    d.min_tiles = cfg->min_tiles_per_worker;  // 0 = chosen by the plan kernel from the amount of work
     d.warps_per_cta = warps;
     d.stages = cfg->pipeline_stages ? cfg->pipeline_stages : kDefaultStages;
     d.max_chunks = (int32_t)max_chunks_of(cfg);
