@@ -167,9 +167,11 @@ int kf_attend(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, f
 /* (a5) kf_step_commit -- len_r += 1 for every open request (the step boundary). */
 int kf_step_commit(kf_ctx *ctx, kf_stream stream);
 
-/* One layer-step with HOST buffers (end-to-end path): copies q / k_new / v_new [host, fp16, shapes as above]
- * to device staging, runs kf_kv_append + kf_attend, copies o [B][H_q][128] and lse [B][H_q] (fp32) back to
- * [host].  Asynchronous on `stream` (use pinned host memory); the caller synchronises the stream. */
+/* One layer-step with HOST buffers (end-to-end path): q / k_new / v_new [host, fp16, shapes as above] in,
+ * o [B][H_q][128] and lse [B][H_q] (fp32) out [host].  With PINNED host memory (16-byte aligned) nothing is copied
+ * by a copy engine: the append kernel reads k_new / v_new over the bus and stages q, kf_attend writes o / lse
+ * straight into the host buffers.  Otherwise the buffers go through device staging with cudaMemcpyAsync.
+ * Asynchronous on `stream`; the caller synchronises the stream before reading o / lse or rewriting the inputs. */
 int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host,
                        const void *v_new_host, float *o_host, float *lse_host, kf_stream stream);
 

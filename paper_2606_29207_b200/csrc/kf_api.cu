@@ -421,11 +421,31 @@ int kf_step_commit(kf_ctx *ctx, kf_stream stream) {
     return after_launch(ctx, launch_step_commit(ctx->dev, (cudaStream_t)stream));
 }
 
+// true if the GPU can dereference this host pointer as it is (pinned memory under unified addressing)
+static bool device_can_read(const void *host_ptr) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, host_ptr) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeHost && a.devicePointer == host_ptr;
+}
+
 int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host, const void *v_new_host,
                        float *o_host, float *lse_host, kf_stream stream) {
     if (!ctx || bad_layer(ctx, layer) || !q_host || !k_new_host || !v_new_host || !o_host || !lse_host) return KF_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
     const Dev &d = ctx->dev;
+    const bool aligned = !(((uintptr_t)q_host | (uintptr_t)k_new_host | (uintptr_t)v_new_host | (uintptr_t)o_host) & 15);
+    if (aligned && device_can_read(q_host) && device_can_read(k_new_host) && device_can_read(v_new_host) &&
+        device_can_read(o_host) && device_can_read(lse_host)) {
+        // zero-copy: the append kernel reads k_new / v_new over the bus and stages q; the attend kernel's merge
+        // tail writes o / lse straight into the host buffers.  No copy engine work at all.
+        int rc = after_launch(ctx, launch_kv_append_stage(d, layer, (const __half *)k_new_host, (const __half *)v_new_host,
+                                                          (const __half *)q_host, d.stage_q, s));
+        if (rc != KF_OK) return rc;
+        return kf_attend(ctx, layer, d.stage_q, o_host, lse_host, nullptr, nullptr, stream);
+    }
     const size_t qb = (size_t)d.B * d.Hq * kHeadDim * 2, kb = (size_t)d.B * d.Hkv * kHeadDim * 2;
     cudaError_t e = cudaMemcpyAsync(d.stage_q, q_host, qb, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d.stage_k, k_new_host, kb, cudaMemcpyHostToDevice, s);

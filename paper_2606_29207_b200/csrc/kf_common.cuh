@@ -144,6 +144,8 @@ int launch_step_commit(const Dev &d, cudaStream_t s);
 int launch_load_context(const Dev &d, int layer, int req, int tok_begin, int n_tokens, const __half *k,
                         const __half *v, cudaStream_t s);
 int launch_kv_append(const Dev &d, int layer, const __half *k_new, const __half *v_new, cudaStream_t s);
+int launch_kv_append_stage(const Dev &d, int layer, const __half *k_new, const __half *v_new, const __half *q_src,
+                           __half *q_dst, cudaStream_t s);
 int launch_attend_simple(const AttendParams &p, int n_ctas, cudaStream_t s);
 int launch_attend_tma(const AttendParams &p, int n_ctas, cudaStream_t s);
 bool attend_tma_shape_ok(int warps, int stages);

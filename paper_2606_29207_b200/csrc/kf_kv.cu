@@ -47,6 +47,36 @@ __global__ void __launch_bounds__(256) kv_append_kernel(Dev d, int layer, const 
     }
 }
 
+// (a2) for the end-to-end path: k_new / v_new / q_src are PINNED HOST buffers read straight over the bus (zero-copy,
+// uncached loads: the host rewrites them between launches); the q rows are staged into device memory for the attend
+// kernel in the same launch.  Replaces three host->device copies by one kernel.
+__global__ void __launch_bounds__(256) kv_append_stage_kernel(Dev d, int layer, const __half *k_new,
+                                                              const __half *v_new, const __half *q_src,
+                                                              __half *q_dst) {
+    const int r = blockIdx.x;
+    const int q_chunks = d.Hq * 16;  // 16-byte chunks of this request's q rows
+    for (int i = threadIdx.x; i < q_chunks; i += blockDim.x) {
+        const size_t off = (size_t)r * q_chunks + i;
+        reinterpret_cast<int4 *>(q_dst)[off] = __ldcv(reinterpret_cast<const int4 *>(q_src) + off);
+    }
+    const int len = d.len[r];
+    if (len < 0) return;
+    const int j = len / d.R, off = len - j * d.R;
+    if (j >= d.n_ranges[r]) {
+        if (threadIdx.x == 0) set_error(d, KF_ESTATE);
+        return;
+    }
+    const int p = d.route_part[(size_t)r * d.Jmax + j];
+    const int slot = d.route_slot[(size_t)r * d.Jmax + j];
+    const int chunks = 2 * d.Hkv * 16;
+    for (int i = threadIdx.x; i < chunks; i += blockDim.x) {
+        const int c = i & 15, g = (i >> 4) % d.Hkv, is_v = (i >> 4) / d.Hkv;
+        const __half *src = (is_v ? v_new : k_new) + ((size_t)r * d.Hkv + g) * kHeadDim + c * 8;
+        unsigned char *dst = d.pool[p] + (is_v ? d.v_off : 0) + row_offset(d, layer, slot, g, off) + c * 16;
+        *reinterpret_cast<int4 *>(dst) = __ldcv(reinterpret_cast<const int4 *>(src));
+    }
+}
+
 int launch_load_context(const Dev &d, int layer, int req, int tok_begin, int n_tokens, const __half *k,
                         const __half *v, cudaStream_t s) {
     if (n_tokens <= 0) return 0;
@@ -58,6 +88,12 @@ int launch_load_context(const Dev &d, int layer, int req, int tok_begin, int n_t
 
 int launch_kv_append(const Dev &d, int layer, const __half *k_new, const __half *v_new, cudaStream_t s) {
     kv_append_kernel<<<d.B, 256, 0, s>>>(d, layer, k_new, v_new);
+    return 1;
+}
+
+int launch_kv_append_stage(const Dev &d, int layer, const __half *k_new, const __half *v_new, const __half *q_src,
+                           __half *q_dst, cudaStream_t s) {
+    kv_append_stage_kernel<<<d.B, 256, 0, s>>>(d, layer, k_new, v_new, q_src, q_dst);
     return 1;
 }
 
