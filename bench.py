@@ -218,6 +218,7 @@ def main():
 
     import torch
     from kf_inputs import workloads
+    from paper_2606_29207_b200 import sharding
     from paper_2606_29207_b200.workload import Session
 
     rank = int(os.environ.get("RANK", "0"))
@@ -232,7 +233,7 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     wl = workloads.by_name(args.workload)
-    wl.seed = wl.seed + rank                       # independent batch per rank (weak scaling)
+    wl.seed = sharding.rank_seed(wl.seed, rank)    # independent batch per rank (weak scaling)
     n_layers = wl.n_layers
     e2e_steps = args.e2e_steps or min(args.steps, 50)
     total_steps = args.warmup + args.steps + 100 + e2e_steps + 2   # + the roofline region (<= 100 steps)
@@ -352,16 +353,8 @@ def main():
     del roof_inputs
     clocks = sampler.stop(t0, t1) if rank == 0 else None
     assert kf.status() == 0
-    if dist:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-        tb = torch.tensor([float(total_bytes), float(launches)], dtype=torch.float64, device=dev)
-        dist.all_reduce(tb, op=dist.ReduceOp.SUM)
-        total_bytes_all, launches_all = float(tb[0].item()), int(tb[1].item())
-    else:
-        total_bytes_all, launches_all = float(total_bytes), launches
-    value = total_bytes_all / (ms * 1e-3) / 1e9
+    ms, total_bytes_all, launches_all = sharding.aggregate(ms, total_bytes, launches, dist, dev)
+    value = sharding.throughput_gbs(total_bytes_all, ms)
     ms_per_step = ms / args.steps
 
     # ---- end to end: HOST buffers, copies inside the timed region.  One replay per step of a host-io step graph
@@ -402,12 +395,9 @@ def main():
     e1.record()
     torch.cuda.synchronize(dev)
     e2e_ms = e0.elapsed_time(e1)
-    if dist:
-        t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms, e2e_bytes_all, _ = sharding.aggregate(e2e_ms, e2e_bytes, 0, dist, dev)
     step += e2e_steps
-    e2e_value = e2e_bytes * world / (e2e_ms * 1e-3) / 1e9
+    e2e_value = sharding.throughput_gbs(e2e_bytes_all, e2e_ms)
     h2d = n_layers * (B * Hq * 128 * 2 + 2 * B * Hkv * 128 * 2)
     d2h = n_layers * (B * Hq * 128 * 4 + B * Hq * 4)
     assert kf.status() == 0 and checksum == checksum
