@@ -353,6 +353,22 @@ def main():
     del roof_inputs
     clocks = sampler.stop(t0, t1) if rank == 0 else None
     assert kf.status() == 0
+
+    # ---- read-only bandwidth probe over the same KV pools (third denominator; MEASURED_PEAKS' figure is a copy) ----
+    probe_gbs = None
+    pool_bytes = sum(p.numel() for p in kf.pools)
+    if rank == 0 and pool_bytes > 8 * 126e6:
+        sink = torch.zeros(1, dtype=torch.int32, device=dev)
+        best = None
+        for _ in range(4):
+            p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            p0.record()
+            pool_bytes = kf.probe_read(sink)
+            p1.record()
+            torch.cuda.synchronize(dev)
+            t = p0.elapsed_time(p1)
+            best = t if best is None else min(best, t)
+        probe_gbs = pool_bytes / (best * 1e-3) / 1e9
     ms, total_bytes_all, launches_all = sharding.aggregate(ms, total_bytes, launches, dist, dev)
     value = sharding.throughput_gbs(total_bytes_all, ms)
     ms_per_step = ms / args.steps
@@ -439,7 +455,8 @@ def main():
                      "achieved": achieved, "peak": peak, "unit": UNIT, "frac": achieved / peak,
                      "traffic": NCU_TRAFFIC_BYTES.get(wl.name), "algorithmic_bytes_per_launch": attend_bytes,
                      "avg_launch_ms": attend_ms, "peak_source": peak_src,
-                     "frac_of_nominal_8000": achieved / NOMINAL_PEAK_GBS},
+                     "frac_of_nominal_8000": achieved / NOMINAL_PEAK_GBS,
+                     "read_probe_gbs": probe_gbs, "frac_of_read_probe": achieved / probe_gbs if probe_gbs else None},
         "cpu_baseline": cpu,
     }
     print(json.dumps(line))

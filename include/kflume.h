@@ -220,6 +220,13 @@ int64_t kf_launch_count(const kf_ctx *ctx);
  *   globaltimer nanoseconds; *n_workers = max_workers.  Synchronises `stream`. */
 int kf_worker_times(kf_ctx *ctx, int64_t *out, int32_t *n_workers, kf_stream stream);
 
+/* kf_probe_read (measurement aid): streams all P KV pools of the ctx once, in one launch, with plain 128-bit loads on
+ * a persistent grid and discards the data -- the read-only HBM bandwidth this box delivers to a trivial kernel, the
+ * third roofline denominator next to the nominal 8 TB/s and the measured copy bandwidth.
+ * sink: [device] 4 bytes, scratch.  *bytes_read [host, may be NULL] = P * kf_pool_bytes().  Asynchronous on `stream`;
+ * time it with events.  Not counted in kf_launch_count. */
+int kf_probe_read(kf_ctx *ctx, void *sink, size_t *bytes_read, kf_stream stream);
+
 #ifdef __cplusplus
 }
 #endif

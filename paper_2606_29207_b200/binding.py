@@ -18,7 +18,7 @@ EXPORTS = [
     "kf_create", "kf_destroy", "kf_open_request", "kf_close_request", "kf_load_context", "kf_token_boundary",
     "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_step_commit", "kf_layer_step_host",
     "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count", "kf_worker_times",
-    "kf_step_graph_create", "kf_step_graph_launch", "kf_step_graph_destroy",
+    "kf_step_graph_create", "kf_step_graph_launch", "kf_step_graph_destroy", "kf_probe_read",
 ]
 
 
@@ -79,6 +79,7 @@ def load_library():
     L.kf_step_graph_create.argtypes = [vp, i32, ctypes.POINTER(i32), i32, pp, pp, pp, pp, pp, vp, ctypes.POINTER(vp)]
     L.kf_step_graph_launch.argtypes = [vp, pp, pp, pp, pp, pp, vp]
     L.kf_step_graph_destroy.argtypes = [vp]
+    L.kf_probe_read.argtypes = [vp, vp, ctypes.POINTER(sz), vp]
     for name in EXPORTS:
         if getattr(L, name).restype is None:
             getattr(L, name).restype = ctypes.c_int
@@ -237,6 +238,12 @@ class KFlume:
     def step_graph_create(self, layers: Sequence[int], q, k_new, v_new, o, lse, host_io: bool = False, stream=None):
         """kf_step_graph_create: q .. lse are lists (one tensor per layer-step).  Returns a StepGraph."""
         return StepGraph(self, layers, q, k_new, v_new, o, lse, host_io, stream)
+
+    def probe_read(self, sink, stream=None) -> int:
+        """kf_probe_read: stream all KV pools once (measurement aid); sink: 4-byte CUDA tensor.  Returns bytes read."""
+        n = ctypes.c_size_t(0)
+        self._check(self.lib.kf_probe_read(self.h, _ptr(sink), ctypes.byref(n), self._stream(stream)), "kf_probe_read")
+        return int(n.value)
 
     def route_snapshot(self, stream=None) -> dict:
         i32 = ctypes.c_int32
