@@ -191,9 +191,13 @@ __device__ void make_levels(Levels &lv, long long Nt, int W, int m, float f) {
 // tiles [b0, b0 + len) of a unit with n tiles belong to level k.  Levels run from the END of the unit towards its
 // start and round up, so level 0 -- the first and largest chunks of the launch -- always holds the unit's last
 // tile: the one place where a tail unit grows between plan rebuilds (live_tiles(), kf_common.cuh).
-__device__ __forceinline__ void level_span(const Levels &lv, int n, int k, int &b0, int &len) {
-    const int lo = k == 0 ? 0 : (int)(((long long)n * lv.end16[k - 1] + 65535) >> 16);
-    const int hi = (int)(((long long)n * lv.end16[k] + 65535) >> 16);
+__device__ __forceinline__ void level_span(const Levels &lv, int n, int k, int m, int &b0, int &len) {
+    // a level that would leave fewer than m (the smallest chunk) tiles to the later ones takes them too: small
+    // units end up as one or two pieces instead of one sliver per level
+    int lo = k == 0 ? 0 : (int)(((long long)n * lv.end16[k - 1] + 65535) >> 16);
+    int hi = (int)(((long long)n * lv.end16[k] + 65535) >> 16);
+    if (k > 0 && n - lo < m) lo = n;
+    if (n - hi < m) hi = n;
     b0 = n - hi;
     len = hi - lo;
 }
@@ -304,7 +308,7 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
         for (int idx = tid; idx < KE; idx += nt) {
             const int k = idx / E, e = idx - k * E;
             int b0, len;
-            level_span(lv, etiles[e], k, b0, len);
+            level_span(lv, etiles[e], k, m, b0, len);
             pos[idx] = len * Hkv;
         }
         __syncthreads();
@@ -313,7 +317,7 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
         for (int idx = tid; idx < KE; idx += nt) {
             const int k = idx / E, e = idx - k * E;
             int b0, len;
-            level_span(lv, etiles[e], k, b0, len);
+            level_span(lv, etiles[e], k, m, b0, len);
             const float left = (float)(Nt - pos[idx]);
             const int size = max(m, (int)ceilf(rho * left / (float)W));
             const int c = (len + size - 1) / size;
@@ -350,7 +354,7 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
         const int c = ccnt[k * E + e];
         if (c == 0) continue;
         int b0, len;
-        level_span(lv, etiles[e], k, b0, len);
+        level_span(lv, etiles[e], k, s_m, b0, len);
         int before = 0;
         for (int kk = 0; kk < k; ++kk) before += ccnt[kk * E + e];
         const int pu = ppre[e + 1] - ppre[e];
