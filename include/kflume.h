@@ -114,12 +114,27 @@ int kf_destroy(kf_ctx *ctx);
 /* ---- routing table --------------------------------------------------------------
  * kf_open_request: "post-prefill initialisation": marks request `req` open with
  *   len = n_tokens and allocates ceil(n_tokens/R) ranges j = 0.. in order.  The k-th range ever allocated
- *   goes to partition k mod P (one global round-robin cursor); the slot comes from that partition's LIFO
+ *   goes to partition k mod P (one global round-robin cursor over the active set, see
+ *   kf_set_active_partitions); the slot comes from that partition's LIFO
  *   free list if non-empty, else from its bump allocator.  Routes are layer-independent: an attention
  *   node holds all L layers of a range.  Device errors: ESTATE (already open), ENOSPC.
  * kf_close_request: returns the request's slots to the free lists (ascending j) and marks it closed. */
 int kf_open_request(kf_ctx *ctx, int32_t req, int32_t n_tokens, kf_stream stream);
 int kf_close_request(kf_ctx *ctx, int32_t req, kf_stream stream);
+
+/* kf_set_active_partitions -- publish a new ACTIVE SET of attention nodes (a scale-up or scale-down event of the
+ *   paper's policy: PAPER.md:216-219 "at the next token boundary, publish the route", :240 "future appends use the
+ *   new A node, while existing KV ranges remain in place").  active: [host] uint8[P], non-zero = the partition
+ *   receives new ranges; at least one must be set.  Takes effect for every range allocated after this call in stream
+ *   order (kf_token_boundary, kf_open_request); existing routes never change, partitions that leave the set keep
+ *   serving the ranges they hold.  Allocation order: the first active partition after the one used last, cyclically
+ *   (with all P active: the k-th range ever allocated goes to partition k mod P).  All partitions start active.
+ *   This call IS the critical-path "route install" (paper: 7.2 us on the CPU): one tiny kernel.
+ * kf_partition_state -- occupancy that the policy monitors (Algorithm 1, l.6-9): [host] active[P] (0/1),
+ *   tokens[P] = committed tokens resident on each partition (x 2*H_kv*d*2 B*L = KV bytes),
+ *   tails[P] = open requests whose tail range lives there.  Any pointer may be NULL.  Synchronises `stream`. */
+int kf_set_active_partitions(kf_ctx *ctx, const uint8_t *active, kf_stream stream);
+int kf_partition_state(kf_ctx *ctx, int32_t *active, int64_t *tokens, int32_t *tails, kf_stream stream);
 
 /* kf_load_context: copies tokens [tok_begin, tok_begin + n_tokens) of request `req`, layer `layer`, into the
  * routed slots.  k, v: [device] fp16 [H_kv][n_tokens][128].  Every position must already have a route

@@ -10,6 +10,9 @@ attending).  Where the paper is silent the readings of DESIGN.md apply:
   reading 8: at the boundary BEFORE appending, a request with len % R == 0 opens range len / R
   reading 9: one global round-robin cursor: the k-th range ever allocated goes to partition k % P;
              allocation order = ranges ascending within a request; requests ascending at a boundary;
+             with an ACTIVE SET of partitions (the published routes of PAPER.md:216-219; "future appends use
+             the new A node, while existing KV ranges remain in place", :240) the next range goes to the
+             first active partition after the one used last, cyclically -- which is k % P when all are active;
              slot = per-partition LIFO free list if non-empty, else bump allocator free_head[p]++
   reading 10: exhaustion (slot >= slots_per_partition, or range index >= max_ranges) -> error ENOSPC
 
@@ -34,7 +37,9 @@ class RoutingModel:
         self.slots = slots_per_partition
         self.len: List[int] = [-1] * max_requests          # -1 = request closed
         self.route: List[List[Tuple[int, int]]] = [[] for _ in range(max_requests)]
-        self.rr_cursor = 0
+        self.rr_cursor = 0                                  # ranges allocated so far
+        self.rr_last = -1                                   # partition of the last allocation
+        self.active = [True] * n_partitions                 # partitions that receive new ranges
         self.free_head = [0] * n_partitions                 # bump allocator
         self.free_list: List[List[int]] = [[] for _ in range(n_partitions)]  # LIFO of released slots
 
@@ -42,7 +47,14 @@ class RoutingModel:
     def _alloc(self, req: int) -> Tuple[int, int]:
         if len(self.route[req]) >= self.Jmax:
             raise RoutingError("ENOSPC: max_ranges_per_request")
-        p = self.rr_cursor % self.P
+        p = None
+        for i in range(1, self.P + 1):                      # first active partition after the last one used
+            c = (self.rr_last + i) % self.P
+            if self.active[c]:
+                p = c
+                break
+        if p is None:
+            raise RoutingError("ENOSPC: no active partition")
         if self.free_list[p]:
             slot = self.free_list[p][-1]
         else:
@@ -51,6 +63,7 @@ class RoutingModel:
                 raise RoutingError("ENOSPC: partition full")
         # commit
         self.rr_cursor += 1
+        self.rr_last = p
         if self.free_list[p]:
             self.free_list[p].pop()
         else:
@@ -104,6 +117,24 @@ class RoutingModel:
             self.free_list[p].append(s)
         self.route[req] = []
         self.len[req] = -1
+
+    def set_active(self, active) -> None:
+        """Publish a new active set (scale event): future ranges only; existing routes never change."""
+        if len(active) != self.P or not any(active):
+            raise RoutingError("EINVAL")
+        self.active = [bool(a) for a in active]
+
+    def partition_state(self) -> Dict[str, object]:
+        """What the scaling policy monitors (Algorithm 1, l.6-9): committed tokens per partition, tails per partition."""
+        tokens, tails = [0] * self.P, [0] * self.P
+        for r in range(self.B):
+            if self.len[r] < 0:
+                continue
+            for j, (p, _) in enumerate(self.route[r]):
+                tokens[p] += max(0, min(self.R, self.len[r] - j * self.R))
+                if j == len(self.route[r]) - 1:
+                    tails[p] += 1
+        return {"active": [1 if a else 0 for a in self.active], "tokens": tokens, "tails": tails}
 
     # -- inspection -----------------------------------------------------------------------------
     def n_ranges(self, req: int) -> int:

@@ -19,6 +19,7 @@ EXPORTS = [
     "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_step_commit", "kf_layer_step_host",
     "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count", "kf_worker_times",
     "kf_step_graph_create", "kf_step_graph_launch", "kf_step_graph_destroy", "kf_probe_read",
+    "kf_set_active_partitions", "kf_partition_state",
 ]
 
 
@@ -79,6 +80,8 @@ def load_library():
     L.kf_step_graph_create.argtypes = [vp, i32, ctypes.POINTER(i32), i32, pp, pp, pp, pp, pp, vp, ctypes.POINTER(vp)]
     L.kf_step_graph_launch.argtypes = [vp, pp, pp, pp, pp, pp, vp]
     L.kf_step_graph_destroy.argtypes = [vp]
+    L.kf_set_active_partitions.argtypes = [vp, ctypes.POINTER(ctypes.c_uint8), vp]
+    L.kf_partition_state.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32), vp]
     L.kf_probe_read.argtypes = [vp, vp, ctypes.POINTER(sz), vp]
     for name in EXPORTS:
         if getattr(L, name).restype is None:
@@ -244,6 +247,16 @@ class KFlume:
         n = ctypes.c_size_t(0)
         self._check(self.lib.kf_probe_read(self.h, _ptr(sink), ctypes.byref(n), self._stream(stream)), "kf_probe_read")
         return int(n.value)
+
+    def set_active_partitions(self, active: Sequence[int], stream=None):
+        assert len(active) == self.P
+        arr = (ctypes.c_uint8 * self.P)(*[1 if x else 0 for x in active])
+        self._check(self.lib.kf_set_active_partitions(self.h, arr, self._stream(stream)), "kf_set_active_partitions")
+
+    def partition_state(self, stream=None) -> dict:
+        act, tok, tails = (ctypes.c_int32 * self.P)(), (ctypes.c_int64 * self.P)(), (ctypes.c_int32 * self.P)()
+        self._check(self.lib.kf_partition_state(self.h, act, tok, tails, self._stream(stream)), "kf_partition_state")
+        return {"active": list(act), "tokens": list(tok), "tails": list(tails)}
 
     def route_snapshot(self, stream=None) -> dict:
         i32 = ctypes.c_int32

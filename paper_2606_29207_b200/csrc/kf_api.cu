@@ -32,7 +32,7 @@ size_t max_chunks_of(const kf_config *c) {
 inline size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t len, n_ranges, route_part, route_slot, rr_cursor, free_head, free_cnt, free_stack, error, plan, units, chunks, plan_age, sched,
+    size_t len, n_ranges, route_part, route_slot, rr_cursor, rr_last, active, part_tokens, part_tails, free_head, free_cnt, free_stack, error, plan, units, chunks, plan_age, sched,
         scratch, unit_counter, group_counter, piece_o, piece_lse, range_o, range_lse, stage_q, stage_k, stage_v,
         stage_o, stage_lse, tmaps, worker_times, total;
 };
@@ -82,6 +82,10 @@ Layout make_layout(const kf_config *c) {
     L.route_part = take(E * 4);
     L.route_slot = take(E * 4);
     L.rr_cursor = take(4);
+    L.rr_last = take(4);
+    L.active = take(P * 4);
+    L.part_tokens = take(P * 8);
+    L.part_tails = take(P * 4);
     L.free_head = take(P * 4);
     L.free_cnt = take(P * 4);
     L.free_stack = take(P * S * 4);
@@ -249,6 +253,13 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     if (e == cudaSuccess) e = cudaMemset(ws + L.route_part, 0xFF, (size_t)cfg->max_requests * cfg->max_ranges_per_request * 4);
     if (e == cudaSuccess) e = cudaMemset(ws + L.route_slot, 0xFF, (size_t)cfg->max_requests * cfg->max_ranges_per_request * 4);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
+    e = cudaMemset(ws + L.rr_last, 0xFF, 4);  // -1: nothing allocated yet
+    if (e == cudaSuccess) {
+        int32_t ones[kMaxPartitions];
+        for (int p = 0; p < kMaxPartitions; ++p) ones[p] = 1;  // every partition starts active
+        e = cudaMemcpy(ws + L.active, ones, (size_t)cfg->n_partitions * 4, cudaMemcpyHostToDevice);
+    }
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
     const int32_t stale = kPlanStale;  // no plan yet: the first plan kernel builds one
     e = cudaMemcpy(ws + L.plan_age, &stale, 4, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
@@ -279,6 +290,10 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.route_part = (int32_t *)(ws + L.route_part);
     d.route_slot = (int32_t *)(ws + L.route_slot);
     d.rr_cursor = (int32_t *)(ws + L.rr_cursor);
+    d.rr_last = (int32_t *)(ws + L.rr_last);
+    d.active = (int32_t *)(ws + L.active);
+    d.part_tokens = (long long *)(ws + L.part_tokens);
+    d.part_tails = (int32_t *)(ws + L.part_tails);
     d.free_head = (int32_t *)(ws + L.free_head);
     d.free_cnt = (int32_t *)(ws + L.free_cnt);
     d.free_stack = (int32_t *)(ws + L.free_stack);
@@ -474,6 +489,33 @@ int kf_route_snapshot(kf_ctx *ctx, int32_t *len, int32_t *n_ranges, int32_t *par
     if (slot && e == cudaSuccess) e = cudaMemcpyAsync(slot, d.route_slot, E * 4, cudaMemcpyDeviceToHost, s);
     if (free_head && e == cudaSuccess) e = cudaMemcpyAsync(free_head, d.free_head, (size_t)d.P * 4, cudaMemcpyDeviceToHost, s);
     if (rr_cursor && e == cudaSuccess) e = cudaMemcpyAsync(rr_cursor, d.rr_cursor, 4, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return KF_OK;
+}
+
+int kf_set_active_partitions(kf_ctx *ctx, const uint8_t *active, kf_stream stream) {
+    if (!ctx || !active) return KF_EINVAL;
+    unsigned long long mask = 0;
+    for (int p = 0; p < ctx->cfg.n_partitions; ++p)
+        if (active[p]) mask |= 1ull << p;
+    if (mask == 0) return KF_EINVAL;
+    return after_launch(ctx, launch_set_active(ctx->dev, mask, (cudaStream_t)stream));
+}
+
+int kf_partition_state(kf_ctx *ctx, int32_t *active, int64_t *tokens, int32_t *tails, kf_stream stream) {
+    if (!ctx) return KF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const Dev &d = ctx->dev;
+    const size_t P = d.P;
+    cudaError_t e = cudaMemsetAsync(d.part_tokens, 0, P * 8, s);
+    if (e == cudaSuccess) e = cudaMemsetAsync(d.part_tails, 0, P * 4, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    const int rc = after_launch(ctx, launch_partition_state(d, d.part_tokens, d.part_tails, s));
+    if (rc != KF_OK) return rc;
+    if (active && e == cudaSuccess) e = cudaMemcpyAsync(active, d.active, P * 4, cudaMemcpyDeviceToHost, s);
+    if (tokens && e == cudaSuccess) e = cudaMemcpyAsync(tokens, d.part_tokens, P * 8, cudaMemcpyDeviceToHost, s);
+    if (tails && e == cudaSuccess) e = cudaMemcpyAsync(tails, d.part_tails, P * 4, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     return KF_OK;

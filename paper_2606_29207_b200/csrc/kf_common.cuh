@@ -71,7 +71,11 @@ struct Dev {
     int32_t *n_ranges;   // [B]
     int32_t *route_part; // [B][Jmax]
     int32_t *route_slot; // [B][Jmax]
-    int32_t *rr_cursor;  // [1]
+    int32_t *rr_cursor;  // [1]   ranges allocated so far
+    int32_t *rr_last;    // [1]   partition of the last allocation (-1: none yet)
+    int32_t *active;     // [P]   1: partition receives new ranges (the published active set)
+    long long *part_tokens;  // [P] scratch of kf_partition_state
+    int32_t *part_tails;     // [P]
     int32_t *free_head;  // [P]
     int32_t *free_cnt;   // [P]
     int32_t *free_stack; // [P][slots]
@@ -141,6 +145,8 @@ int launch_close_request(const Dev &d, int req, cudaStream_t s);
 int launch_plan(const Dev &d, int do_boundary, cudaStream_t s);  // (a1, optional) + work plan, one launch
 int plan_setup();        // cudaFuncSetAttribute for the plan kernel's dynamic shared memory; 0 or KF_ECUDA
 int launch_step_commit(const Dev &d, cudaStream_t s);
+int launch_set_active(const Dev &d, unsigned long long mask, cudaStream_t s);
+int launch_partition_state(const Dev &d, long long *tokens, int *tails, cudaStream_t s);
 int launch_load_context(const Dev &d, int layer, int req, int tok_begin, int n_tokens, const __half *k,
                         const __half *v, cudaStream_t s);
 int launch_kv_append(const Dev &d, int layer, const __half *k_new, const __half *v_new, cudaStream_t s);

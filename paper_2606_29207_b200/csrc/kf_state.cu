@@ -15,8 +15,22 @@ __device__ bool alloc_range(const Dev &d, int req) {
         set_error(d, KF_ENOSPC);
         return false;
     }
+    // round-robin over the ACTIVE partitions: the first active one after the partition used last, cyclically
+    // (with every partition active this is "the k-th range ever allocated goes to partition k mod P")
     const int k = *d.rr_cursor;
-    const int p = k % d.P;
+    const int last = *d.rr_last;
+    int p = -1;
+    for (int i = 1; i <= d.P; ++i) {
+        const int c = (last + i) % d.P;
+        if (d.active[c]) {
+            p = c;
+            break;
+        }
+    }
+    if (p < 0) {
+        set_error(d, KF_ENOSPC);
+        return false;
+    }
     const int nfree = d.free_cnt[p];
     int slot;
     if (nfree > 0) {
@@ -29,6 +43,7 @@ __device__ bool alloc_range(const Dev &d, int req) {
         }
     }
     *d.rr_cursor = k + 1;
+    *d.rr_last = p;
     if (nfree > 0)
         d.free_cnt[p] = nfree - 1;
     else
@@ -96,6 +111,28 @@ __device__ int token_boundary_warp(const Dev &d, int lane) {
         __syncwarp();
     }
     return opened;
+}
+
+// publish a new active set (scale-up / scale-down event): affects FUTURE ranges only
+__global__ void set_active_kernel(Dev d, unsigned long long mask) {
+    const int p = threadIdx.x;
+    if (p < d.P) d.active[p] = (int)((mask >> p) & 1ull);
+}
+
+// per-partition occupancy for the scaling policy (Algorithm 1, l.6-9): committed tokens resident on partition p
+// and the number of open requests whose tail range lives there.  One thread per request, atomics on [P] words.
+__global__ void partition_state_kernel(Dev d, long long *tokens, int *tails) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= d.B) return;
+    const int len = d.len[r];
+    if (len < 0) return;
+    const int J = d.n_ranges[r];
+    for (int j = 0; j < J; ++j) {
+        const int p = d.route_part[(size_t)r * d.Jmax + j];
+        const long long cnt = max(0, min(d.R, len - j * d.R));
+        atomicAdd(reinterpret_cast<unsigned long long *>(tokens + p), (unsigned long long)cnt);
+        if (j == J - 1) atomicAdd(tails + p, 1);
+    }
 }
 
 __global__ void step_commit_kernel(Dev d) {
@@ -424,6 +461,14 @@ int plan_setup() {
                                 (int)(kPlanSmemInts * sizeof(int))) == cudaSuccess
                ? 0
                : KF_ECUDA;
+}
+int launch_set_active(const Dev &d, unsigned long long mask, cudaStream_t s) {
+    set_active_kernel<<<1, kMaxPartitions, 0, s>>>(d, mask);
+    return 1;
+}
+int launch_partition_state(const Dev &d, long long *tokens, int *tails, cudaStream_t s) {
+    partition_state_kernel<<<(d.B + 127) / 128, 128, 0, s>>>(d, tokens, tails);
+    return 1;
 }
 int launch_step_commit(const Dev &d, cudaStream_t s) {
     step_commit_kernel<<<(d.B + 255) / 256, 256, 0, s>>>(d);

@@ -141,3 +141,61 @@ def test_kv_byte_formula():
     per_token = 2 * 8 * 128 * 32 * 2
     assert per_token == 128 * 1024
     assert 64 * 4096 * per_token == 32 * 2 ** 30
+
+
+# ---- active sets: scale-up / scale-down events (Fig. 5 at :173) -------------------------
+def test_fig5_scale_up_appends_route_on_the_new_node_only():
+    # Fig. 5 caption: [0,T/2) -> A0, [T/2,T) -> A1, then A2 is published and [T,...) -> A2; nothing else changes
+    R = 8
+    m = RoutingModel(3, R, 1, 4, 4)
+    m.set_active([1, 1, 0])
+    m.open_request(0, 2 * R)                         # T = 2R tokens after prefill
+    assert m.route[0] == [(0, 0), (1, 0)]
+    before = list(m.route[0])
+    m.set_active([1, 1, 1])                          # the prewarmed node's route is published
+    ev = m.token_boundary()                          # len % R == 0: the tail range is full -> a new range opens
+    assert ev == [(0, 2, 2, 0)]
+    assert m.route[0][:2] == before and m.route[0][2] == (2, 0)
+    assert m.append_position(0) == (2, 0, 0)
+
+
+def test_all_partitions_active_is_k_mod_p():
+    import random
+    rnd = random.Random(7)
+    P, R = 5, 4
+    m = RoutingModel(P, R, 6, 64, 64)
+    k = 0
+    for r in range(6):
+        n = rnd.randrange(0, 40)
+        m.open_request(r, n)
+        for j in range(-(-n // R)):
+            assert m.route[r][j][0] == k % P
+            k += 1
+    for _ in range(30):
+        for (_, _, p, _) in m.token_boundary():
+            assert p == k % P
+            k += 1
+        m.step_commit()
+    assert m.rr_cursor == k
+
+
+def test_scale_down_keeps_existing_ranges_and_starves_the_retired_node():
+    P, R = 3, 4
+    m = RoutingModel(P, R, 3, 32, 32)
+    for r, n in enumerate([9, 4, 6]):
+        m.open_request(r, n)
+    frozen = [list(x) for x in m.route]
+    m.set_active([1, 0, 1])                          # node 1 leaves the active set
+    for _ in range(24):
+        m.token_boundary()
+        m.step_commit()
+    for r in range(3):
+        assert m.route[r][:len(frozen[r])] == frozen[r]              # entries never change once written
+        assert all(p != 1 for (p, _) in m.route[r][len(frozen[r]):])  # no new range on the retired node
+    st = m.partition_state()
+    assert sum(st["tokens"]) == sum(m.len) and sum(st["tails"]) == 3 and st["active"] == [1, 0, 1]
+    assert st["tails"][1] == 0                        # every tail has moved on since
+    # bytes the policy sees: tokens x 2 * H_kv * d_h * L * 2 B
+    assert st["tokens"][0] * 2 * 8 * 128 * 32 * 2 == st["tokens"][0] * 131072
+    with pytest.raises(RoutingError):
+        m.set_active([0, 0, 0])
