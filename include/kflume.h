@@ -235,6 +235,37 @@ int64_t kf_launch_count(const kf_ctx *ctx);
  *   globaltimer nanoseconds; *n_workers = max_workers.  Synchronises `stream`. */
 int kf_worker_times(kf_ctx *ctx, int64_t *out, int32_t *n_workers, kf_stream stream);
 
+/* ---- Algorithm 1: the A-node scaling policy, host-side controller ----------------------------
+ * Pure host arithmetic (double), no GPU work.  Feed it kf_partition_state(); act on it with
+ * kf_set_active_partitions().  The paper gives no values for beta_mem, beta_slo, gamma: they are inputs.
+ *   kf_policy_bytes_per_token: 2 * H_kv * d_h * L * 2 B.
+ *   kf_policy_threshold:       Eq. (1)  C_thresh = min(beta_mem * C_kv_cap, beta_slo * T_A^max * BW_HBM).
+ *   kf_policy_initial_nodes:   l.2-3    N_A = ceil(sum_i s_i * bytes_per_token / C_thresh); s: [host] int64[n]; -1 on bad input.
+ *   kf_policy_step:            l.6-19   for every node i holding at least one tail (tails[i] > 0):
+ *        g_i = tails[i] * bytes_per_token;  b_i = tokens[i] * bytes_per_token;
+ *        tau_fill = (C_thresh - b_i) / g_i                                   (Eq. 2; +inf for nodes without tails)
+ *        want_prewarm = tau_fill * T_step < T_prewarm and no prewarm pending or ready for i
+ *        want_publish = b_i >= gamma * C_thresh and the prewarm for i is ready
+ *      tokens, tails: [host] [P] as kf_partition_state returns them; prewarm_pending / prewarm_ready: [host] uint8[P]
+ *      kept by the caller (a prewarm is the background bring-up of a fresh node); out: [host] [P]. */
+typedef struct kf_policy_config {
+    double beta_mem, beta_slo, gamma; /* in (0, 1] */
+    double t_a_max_s;                 /* largest admissible routed-attention time per layer, seconds (from the TPOT SLO) */
+    double bw_hbm;                    /* effective HBM bandwidth of one attention node, bytes / s */
+    double c_kv_cap;                  /* usable KV capacity of one attention node, bytes */
+    double t_step_s, t_prewarm_s;     /* predicted decode-step time; measured time to prepare a new route */
+    int32_t n_kv_heads, head_dim, n_layers;
+} kf_policy_config;
+typedef struct kf_policy_decision {
+    double tau_fill;
+    int32_t want_prewarm, want_publish;
+} kf_policy_decision;
+double kf_policy_bytes_per_token(const kf_policy_config *cfg);
+double kf_policy_threshold(const kf_policy_config *cfg);
+int64_t kf_policy_initial_nodes(const kf_policy_config *cfg, const int64_t *s, int32_t n_requests);
+int kf_policy_step(const kf_policy_config *cfg, int32_t n_partitions, const int64_t *tokens, const int32_t *tails,
+                   const uint8_t *prewarm_pending, const uint8_t *prewarm_ready, kf_policy_decision *out);
+
 /* kf_probe_read (measurement aid): streams all P KV pools of the ctx once, in one launch, with plain 128-bit loads on
  * a persistent grid and discards the data -- the read-only HBM bandwidth this box delivers to a trivial kernel, the
  * third roofline denominator next to the nominal 8 TB/s and the measured copy bandwidth.

@@ -20,6 +20,7 @@ EXPORTS = [
     "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count", "kf_worker_times",
     "kf_step_graph_create", "kf_step_graph_launch", "kf_step_graph_destroy", "kf_probe_read",
     "kf_set_active_partitions", "kf_partition_state",
+    "kf_policy_bytes_per_token", "kf_policy_threshold", "kf_policy_initial_nodes", "kf_policy_step",
 ]
 
 
@@ -34,6 +35,17 @@ class kf_config(ctypes.Structure):
         ("sched_first_pct", ctypes.c_int32), ("sched_decay_pct", ctypes.c_int32),
         ("plan_refresh_steps", ctypes.c_int32),
     ]
+
+
+class kf_policy_config(ctypes.Structure):
+    _fields_ = [("beta_mem", ctypes.c_double), ("beta_slo", ctypes.c_double), ("gamma", ctypes.c_double),
+                ("t_a_max_s", ctypes.c_double), ("bw_hbm", ctypes.c_double), ("c_kv_cap", ctypes.c_double),
+                ("t_step_s", ctypes.c_double), ("t_prewarm_s", ctypes.c_double),
+                ("n_kv_heads", ctypes.c_int32), ("head_dim", ctypes.c_int32), ("n_layers", ctypes.c_int32)]
+
+
+class kf_policy_decision(ctypes.Structure):
+    _fields_ = [("tau_fill", ctypes.c_double), ("want_prewarm", ctypes.c_int32), ("want_publish", ctypes.c_int32)]
 
 
 class KFlumeError(RuntimeError):
@@ -82,6 +94,13 @@ def load_library():
     L.kf_step_graph_destroy.argtypes = [vp]
     L.kf_set_active_partitions.argtypes = [vp, ctypes.POINTER(ctypes.c_uint8), vp]
     L.kf_partition_state.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32), vp]
+    pcp = ctypes.POINTER(kf_policy_config)
+    u8p = ctypes.POINTER(ctypes.c_uint8)
+    L.kf_policy_bytes_per_token.argtypes, L.kf_policy_bytes_per_token.restype = [pcp], ctypes.c_double
+    L.kf_policy_threshold.argtypes, L.kf_policy_threshold.restype = [pcp], ctypes.c_double
+    L.kf_policy_initial_nodes.argtypes, L.kf_policy_initial_nodes.restype = [pcp, ctypes.POINTER(i64), i32], i64
+    L.kf_policy_step.argtypes = [pcp, i32, ctypes.POINTER(i64), ctypes.POINTER(i32), u8p, u8p,
+                                 ctypes.POINTER(kf_policy_decision)]
     L.kf_probe_read.argtypes = [vp, vp, ctypes.POINTER(sz), vp]
     for name in EXPORTS:
         if getattr(L, name).restype is None:
@@ -333,3 +352,31 @@ class StepGraph:
             self.destroy()
         except Exception:
             pass
+
+
+class Policy:
+    """Algorithm 1 of the paper (kf_policy_*): host-side arithmetic only, usable without a GPU."""
+
+    def __init__(self, **kw):
+        self.lib = load_library()
+        self.cfg = kf_policy_config(**kw)
+
+    def bytes_per_token(self) -> float:
+        return self.lib.kf_policy_bytes_per_token(ctypes.byref(self.cfg))
+
+    def threshold(self) -> float:
+        return self.lib.kf_policy_threshold(ctypes.byref(self.cfg))
+
+    def initial_nodes(self, lengths: Sequence[int]) -> int:
+        arr = (ctypes.c_int64 * len(lengths))(*lengths)
+        return int(self.lib.kf_policy_initial_nodes(ctypes.byref(self.cfg), arr, len(lengths)))
+
+    def step(self, tokens: Sequence[int], tails: Sequence[int], pending: Sequence[int], ready: Sequence[int]):
+        P = len(tokens)
+        out = (kf_policy_decision * P)()
+        rc = self.lib.kf_policy_step(ctypes.byref(self.cfg), P, (ctypes.c_int64 * P)(*tokens),
+                                     (ctypes.c_int32 * P)(*tails), (ctypes.c_uint8 * P)(*[1 if x else 0 for x in pending]),
+                                     (ctypes.c_uint8 * P)(*[1 if x else 0 for x in ready]), out)
+        if rc != KF_OK:
+            raise KFlumeError(rc, "kf_policy_step: invalid argument")
+        return [(d.tau_fill, bool(d.want_prewarm), bool(d.want_publish)) for d in out]

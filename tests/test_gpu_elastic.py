@@ -91,3 +91,88 @@ def test_scale_up_and_down_during_graph_replay_matches_model_and_oracle():
     st = kf.partition_state()
     assert st["active"] == [0, 1, 1, 1] and st["tokens"][3] > 0 and sum(st["tails"]) == wl.batch
     ses.close()
+
+
+# ---- Algorithm 1 closed loop: the library's controller drives the device routing table -----------------------------
+def _controller_loop(steps, P, state_fn, decide_fn, publish_fn, step_fn, prewarm_steps=3):
+    """The per-step monitor of Algorithm 1 around an abstract backend.  A node that reaches its watermark with a ready
+    prewarm leaves the active set and the lowest-numbered idle node joins it: "redirect active tails on i to
+    prewarm[i]" (l.17) under the fixed-R reading -- the tails move as their current ranges fill.  The joining node is a
+    FRESH one (never provisioned before), as in the paper; with none left the event is skipped."""
+    active = [1] + [0] * (P - 1)
+    fresh = list(range(1, P))                     # nodes never provisioned so far, in bring-up order
+    pending, ready, countdown = [False] * P, [False] * P, [0] * P
+    history = []
+    publish_fn(active)
+    for t in range(steps):
+        st = state_fn()
+        dec = decide_fn(st["tokens"], st["tails"], pending, ready)
+        for i, (_, spawn, publish) in enumerate(dec):
+            if not active[i]:
+                continue          # already published away: it only drains its tails' current ranges (<= R tokens each)
+            if spawn:
+                pending[i], countdown[i] = True, prewarm_steps
+            if publish and fresh:
+                active[fresh.pop(0)] = 1
+                active[i] = 0
+                ready[i] = False
+                publish_fn(active)
+        for i in range(P):
+            if pending[i]:
+                countdown[i] -= 1
+                if countdown[i] == 0:
+                    pending[i], ready[i] = False, True
+        history.append((list(active), list(st["tokens"]), list(st["tails"])))
+        step_fn(t)
+    return history
+
+
+def test_algorithm1_closed_loop_device_equals_model():
+    from oracle import policy as opol
+    from paper_2606_29207_b200 import Policy
+    P, R, steps = 4, 32, 200
+    wl = Workload("alg1", 32, 8, R, P, [70, 31, 33, 100, 64])
+    kw = dict(beta_mem=1.0, beta_slo=1.0, gamma=0.8, t_a_max_s=1.0, bw_hbm=1e30, c_kv_cap=4096.0 * 400,
+              t_step_s=1.0, t_prewarm_s=3.0, n_kv_heads=8, head_dim=128, n_layers=1)
+    pol, oc = Policy(**kw), opol.PolicyConstants(**kw)
+    assert pol.initial_nodes([s - 1 for s in wl.contexts]) == 1          # 298 tokens fit one 400-token node
+
+    ses = Session(wl, steps=steps, slack_slots=16)
+    kf = ses.kf
+    kf.set_active_partitions([1, 0, 0, 0])
+    ses.prepare()
+
+    def gpu_step(t):
+        kf.token_boundary()
+        q, (kn, vn) = ses.q_for(0, t), ses.kv_new_for(0, t)
+        ses.layer_step(0, q, kn, vn)
+        kf.step_commit()
+        if t % 9 == 0 or t == steps - 1:
+            o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+            for r, S0 in enumerate(wl.contexts):
+                o_ref, lse_ref = oracle_request(wl, 0, r, t, S0 + t)
+                check_close(o[r], lse[r], o_ref, lse_ref, f"alg1 step{t} r{r}")
+
+    h_gpu = _controller_loop(steps, P, kf.partition_state, pol.step, kf.set_active_partitions, gpu_step)
+
+    model = RoutingModel(P, R, wl.batch, kf.Jmax, kf.cfg.slots_per_partition)
+    model.set_active([1, 0, 0, 0])
+    for r, n in enumerate(ses.len0):
+        model.open_request(r, n)
+
+    def model_step(t):
+        model.token_boundary()
+        model.step_commit()
+
+    h_model = _controller_loop(steps, P, model.partition_state,
+                               lambda tok, tails, pe, re: opol.monitor(oc, tok, tails, pe, re), model.set_active, model_step)
+    assert h_gpu == h_model                                   # same decisions, same occupancy, every step
+    _same(kf, model)
+    assert kf.status() == KF_OK
+    actives = [tuple(a) for a, _, _ in h_gpu]
+    assert len(set(actives)) >= 3                             # the policy scaled at least twice
+    final_tokens = h_gpu[-1][1]
+    assert sum(1 for x in final_tokens if x > 0) >= 3
+    # a node stops receiving ranges once published away; it may still grow until its tails' current ranges fill
+    assert max(final_tokens[:3]) <= 400 + wl.batch * R        # (the last node has no successor to hand over to)
+    ses.close()
