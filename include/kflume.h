@@ -22,6 +22,10 @@
  *     on the caller's stream, never synchronise, never allocate, launch fixed grids and read all variable
  *     state (lengths, routes, work plan) from device memory -- so a CUDA Graph captured around them stays
  *     valid across route updates (the single-GPU analogue of PAPER.md:165-179, requirement R1 at :127).
+ *   - One ctx = one stream order: the calls of a ctx share device-side scheduler words and completion counters, so
+ *     they must be issued so that they execute one after another (one stream, or streams ordered by events).  Use
+ *     separate ctxs (with separate workspaces) for concurrent batches.  Host-side entry points are not thread-safe
+ *     per ctx.
  *   - There is NO CPU fallback: without a CUDA device kf_create() returns KF_ECUDA.
  *
  * Notation: B = max_requests, H_q / H_kv = query / KV heads, G = H_q / H_kv, d = head_dim = 128,
