@@ -10,6 +10,11 @@
 
 namespace kf {
 
+// Release side of the partial hand-off: orders this thread's stores of a partial before the counter increment that
+// publishes it.  acq_rel at gpu scope is all the message-passing pattern needs; __threadfence() is the sequentially
+// consistent fence (MEMBAR.SC + L1 invalidate), several hundred ns more per hop of the merge tail.
+__device__ __forceinline__ void release_fence() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+
 __device__ __forceinline__ float warp_max(float v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
@@ -185,7 +190,7 @@ __device__ __forceinline__ Counters launch_prologue(const Dev &d, int w, int W, 
 // the last worker to finish rewinds the tickets and flips the epoch for the next launch
 __device__ __forceinline__ void launch_epilogue(const Dev &d, int W, int lane) {
     if (lane == 0) {
-        __threadfence();
+        release_fence();
         const int old = atomicAdd(d.sched + 1, 1);
         if (old == W - 1) {
             d.sched[0] = 0;
@@ -201,7 +206,7 @@ __device__ __forceinline__ void launch_epilogue(const Dev &d, int W, int lane) {
 __device__ __forceinline__ void piece_done(const AttendParams &p, const Counters &c, int u, const Unit &un, int g,
                                            int lane) {
     const Dev &d = p.d;
-    __threadfence();
+    release_fence();
     __syncwarp();
     if (lane == 0) {
         if (un.n_pieces > 1)
@@ -220,8 +225,7 @@ __device__ __forceinline__ void wait_counter(const int32_t *ctr, int target, int
             __nanosleep(64);
         }
     }
-    __syncwarp();
-    __threadfence();
+    __syncwarp();  // lane 0's acquire happens-before the other lanes' loads of the partials (L2 loads, __ldcg)
 }
 
 // Fused tail: once the chunk list is exhausted every worker turns into a merge worker.
@@ -262,7 +266,7 @@ __device__ __forceinline__ void merge_phase(const AttendParams &p, const Counter
                 wait_counter(&c.unit[u], un.n_pieces, lane);
                 merge_unit_head(p, un, g, i, true, lane);
                 if (d.scratch[un.req] > 1) {
-                    __threadfence();
+                    release_fence();
                     __syncwarp();
                     if (lane == 0) atomicAdd(&c.group[un.req * Hkv + g], 1);
                 }
