@@ -64,7 +64,7 @@ __device__ __forceinline__ PieceDest piece_dest(const AttendParams &p, const Uni
 // by other SMs, possibly in this same launch.  The lse values and the first batch of rows are requested before
 // anything is computed, so a merge of <= 16 partials costs one L2 round trip.  The accumulation order is j
 // ascending, whoever calls this, so every path (fused tail, stand-alone kernels) produces the same bits.
-constexpr int kMergeBatch = 16;
+constexpr int kMergeBatch = 32;
 
 // __noinline__: this code runs once or twice per worker at the very end of a launch, with a cold instruction
 // cache -- one shared copy of it costs far fewer instruction-fetch misses than an inlined copy per call site.
