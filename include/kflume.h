@@ -227,7 +227,9 @@ int kf_step_graph_destroy(kf_graph *graph);
  * kf_status: synchronises `stream`, returns the device error word (KF_OK or the FIRST latched KF_E*) and
  *   clears it.
  * kf_plan_info: downloads the work-plan header into out[8] [host]: {n_units, n_tiles, n_workers_active,
- *   n_pieces, n_range_entries, tile_tokens, max_workers, 0}.  Synchronises `stream`.
+ *   n_pieces, n_range_entries, tile_tokens, max_workers, n_levels}.  Synchronises `stream`.  Like kf_attend it first
+ *   rebuilds the plan if a kf_step_commit happened since the last kf_token_boundary (device error ESTATE if the new
+ *   tail position has no route yet): call it between kf_token_boundary and kf_step_commit.
  * kf_launch_count: number of CUDA kernels this ctx has launched so far (host-side counter). */
 int kf_route_snapshot(kf_ctx *ctx, int32_t *len, int32_t *n_ranges, int32_t *part, int32_t *slot,
                       int32_t *free_head, int32_t *rr_cursor, kf_stream stream);

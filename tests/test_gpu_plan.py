@@ -92,3 +92,43 @@ def test_attend_after_commit_without_boundary():
     ses.layer_step(0, q, k_new, v_new)
     assert kf.status() == KF_ESTATE
     ses.close()
+
+
+def test_many_requests_plan_scratch_spills_to_global():
+    # 1024 requests x 10 ranges = 10240 (request, range) entries and 4-5 scheduling levels: the plan kernel's
+    # per-(level, entry) arrays no longer fit its 192 KB of shared memory and fall back to the global scratch area
+    # (kf_state.cu: take()).  Routes against the integer model; sampled requests against the oracle; two steps so
+    # that the kept plan is exercised on this path as well.
+    import random
+    rnd = random.Random(5)
+    B, R = 1024, 64
+    ctx = [rnd.randrange(560, 640) for _ in range(B)]
+    wl = Workload("many_requests", 8, 2, R, 16, ctx)
+    ses = Session(wl, steps=2)
+    ses.prepare()
+    kf = ses.kf
+    model = RoutingModel(wl.n_partitions, R, B, kf.Jmax, kf.cfg.slots_per_partition)
+    for r, n in enumerate(ses.len0):
+        model.open_request(r, n)
+    for step in range(2):
+        kf.token_boundary()
+        model.token_boundary()
+        q = ses.q_for(0, step)
+        k_new, v_new = ses.kv_new_for(0, step)
+        ses.o.fill_(float("nan"))
+        ses.lse.fill_(float("nan"))
+        ses.layer_step(0, q, k_new, v_new)
+        info = kf.plan_info()             # (before the commit: afterwards the plan of the NEXT step would be built)
+        assert info["n_entries"] >= 9 * B and info["n_units"] == 2 * info["n_entries"]
+        kf.step_commit()
+        model.step_commit()
+        assert kf.status() == KF_OK
+        o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+        assert np.isfinite(o).all() and np.isfinite(lse).all()
+        for r in (0, 1, 511, 777, 1023):
+            o_ref, lse_ref = oracle_request(wl, 0, r, step, ctx[r] + step)
+            check_close(o[r], lse[r], o_ref, lse_ref, f"many_requests step{step} r{r}")
+    snap, ms = kf.route_snapshot(), model.snapshot()
+    for key in ("len", "n_ranges", "part", "slot", "free_head", "rr_cursor"):
+        assert snap[key] == ms[key], key
+    ses.close()
