@@ -373,3 +373,31 @@ def test_layer_step_host_matches_device_path():
     assert torch.equal(oh, o_dev) and torch.equal(lh, l_dev)
     assert kf.status() == KF_OK
     ses.close()
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_closed_request_rows_untouched_and_64_partitions(impl):
+    # P = 64 (the maximum), 5 requests of which #1 and #3 are closed before the step: their output rows must stay
+    # untouched, the others must match the oracle; the freed slots are reused by a request opened afterwards
+    wl = Workload("holes", 32, 8, 32, 64, [100, 70, 33, 64, 129])
+    ses = Session(wl, impl=impl, slack_slots=2)
+    ses.prepare()
+    kf = ses.kf
+    kf.close_request(1)
+    kf.close_request(3)
+    kf.token_boundary()
+    q = ses.q_for(0, 0)
+    k_new, v_new = ses.kv_new_for(0, 0)
+    ses.o.fill_(float("nan"))
+    ses.lse.fill_(float("nan"))
+    ses.layer_step(0, q, k_new, v_new)
+    assert kf.status() == KF_OK
+    o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+    for r in (0, 2, 4):
+        o_ref, lse_ref = oracle_request(wl, 0, r, 0, wl.contexts[r])
+        check_close(o[r], lse[r], o_ref, lse_ref, f"holes r{r}")
+    for r in (1, 3):
+        assert np.isnan(o[r]).all() and np.isnan(lse[r]).all()
+    snap = kf.route_snapshot()
+    assert snap["len"][1] == -1 and snap["n_ranges"][3] == 0
+    ses.close()
