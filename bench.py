@@ -196,6 +196,61 @@ def run_reference(args):
     return 0
 
 
+def run_route_install(args):
+    """--route-install: latency of a scale event (kf_set_active_partitions, the paper's route install: 7.2 us on its
+    CPU) and of kf_token_boundary with a kept / a rebuilt work plan.  Medians; one JSON line."""
+    import statistics
+    import torch
+    from kf_inputs import workloads
+    from paper_2606_29207_b200.workload import Session
+    wl = workloads.by_name(args.workload)
+    P = wl.n_partitions
+
+    def event_us(fn):
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        t0 = time.perf_counter()
+        fn()
+        t1 = time.perf_counter()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) * 1e3, (t1 - t0) * 1e6
+
+    out = {"mode": "route-install", "workload": wl.name, "n_partitions": P}
+    for key, refresh in (("kept_plan", 0), ("rebuilt_plan", 1)):
+        ses = Session(wl, n_layers_phys=1, steps=400, slack_slots=4, plan_refresh_steps=refresh)
+        ses.open_all()                                   # routes only: pool contents do not matter here
+        kf = ses.kf
+        kf.token_boundary()
+        if key == "kept_plan":
+            ev, host = [], []
+            for i in range(200):
+                mask = [1] * P
+                mask[i % P] = i % 2
+                if not any(mask):
+                    mask[0] = 1
+                e, h = event_us(lambda: kf.set_active_partitions(mask))
+                ev.append(e)
+                host.append(h)
+            kf.set_active_partitions([1] * P)
+            out["set_active_event_us"] = statistics.median(ev)
+            out["set_active_host_enqueue_us"] = statistics.median(host)
+        ev = []
+        for _ in range(60):
+            ev.append(event_us(kf.token_boundary)[0])
+            kf.step_commit()
+        out[f"token_boundary_{key}_event_us"] = statistics.median(ev)
+        assert kf.status() == 0
+        ses.close()
+    e = []
+    for _ in range(60):
+        e.append(event_us(lambda: None)[0])
+    out["empty_event_pair_us"] = statistics.median(e)
+    print(json.dumps(out))
+    return 0
+
+
 # ---------------------------------------------------------------------------------------------------------
 def main():
     ap = argparse.ArgumentParser()
@@ -209,6 +264,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 50)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--min-tiles", type=int, default=0)
+    ap.add_argument("--route-install", action="store_true", help="measure the latency of a scale event (route "
+                    "install) and of the token boundary instead of the decode benchmark")
     ap.add_argument("--no-l2-flush", action="store_true", help="do not flush L2 between timed steps when the KV of a "
                     "layer-step fits L2 (cfg1)")
     ap.add_argument("--no-graph", action="store_true", help="launch the calls of a step one by one instead of "
@@ -216,6 +273,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.route_install:
+        return run_route_install(args)
     args.warmup = max(args.warmup, 3)
 
     import torch
