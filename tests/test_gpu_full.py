@@ -223,3 +223,28 @@ def test_fig10_head_shapes_sampled(name, reqs, heads):
     # all requests see different q/K/V but the same context length: lse ~ ln S + scale^2 |q|^2 / 2 (loose sanity)
     assert np.all(np.abs(lse - (np.log(wl.contexts[0]) + 0.5)) < 1.0)
     ses.close()
+
+
+def test_cfg3_full_size_through_the_step_graph():
+    # bench.py's timed region launches every step as ONE replay of the static step graph with re-bound inputs:
+    # the same at full size here, sampled against the oracle at steps 0 and 2 (kept plan, grown tails)
+    wl = workloads.cfg3()
+    ses = Session(wl, steps=3)
+    ses.prepare()
+    kf = ses.kf
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        ins = [(ses.q_for(0, t),) + ses.kv_new_for(0, t) for t in range(3)]
+        g = kf.step_graph_create([0], [ins[0][0]], [ins[0][1]], [ins[0][2]], [ses.o], [ses.lse])
+        for t in range(3):
+            g.launch([ins[t][0]], [ins[t][1]], [ins[t][2]], [ses.o], [ses.lse])
+            side.synchronize()
+            if t in (0, 2):
+                o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+                assert np.isfinite(o).all() and np.isfinite(lse).all()
+                for r, heads in ((2, [0, 31]), (7, [5]), (15, [17])):
+                    _check_request(wl, (o, lse), 0, r, t, wl.contexts[r] + t, heads, what=f"cfg3 graph step{t}")
+        assert kf.status() == KF_OK
+        assert kf.route_snapshot()["len"] == [s - 1 + 3 for s in wl.contexts]
+        g.destroy()
+    ses.close()
