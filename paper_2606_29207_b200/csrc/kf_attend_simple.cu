@@ -135,7 +135,17 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) attend_simple_kernel(Attend
 }
 
 int launch_attend_simple(const AttendParams &p, int n_ctas, cudaStream_t s) {
-    attend_simple_kernel<<<n_ctas, kWarpsPerCta * 32, 0, s>>>(p);
+    cudaLaunchConfig_t cfg = {};  // cooperative: see launch_one() in kf_attend_tma.cu
+    cfg.gridDim = dim3(n_ctas);
+    cfg.blockDim = dim3(kWarpsPerCta * 32);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, attend_simple_kernel, p);
     return 1;
 }
 

@@ -384,7 +384,20 @@ static int setup_one() {
 template <int WARPS, int STAGES>
 static int launch_one(const AttendParams &p, int n_ctas, cudaStream_t s) {
     const int smem = WARPS * STAGES * kStageBytes + 1024;
-    attend_tma_kernel<WARPS, STAGES><<<n_ctas, WARPS * 32, smem, s>>>(p);
+    // Cooperative launch: the fused merge makes workers wait for partials of other workers of the SAME launch, so
+    // every CTA must be resident at once.  The grid never exceeds the SM count, but only a cooperative launch makes
+    // the hardware gang-schedule it when other work shares the GPU (it fails instead of deadlocking otherwise).
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(n_ctas);
+    cfg.blockDim = dim3(WARPS * 32);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, attend_tma_kernel<WARPS, STAGES>, p);
     return 1;
 }
 
