@@ -433,7 +433,8 @@ def main():
     r1.record()
     torch.cuda.synchronize(dev)
     eager_ms_per_step = None if flush else r0.elapsed_time(r1) / roof_steps   # (the flush writes sit in this region)
-    attend_ms = sum(a.elapsed_time(b) for a, b in attend_events) / len(attend_events)
+    attend_times = sorted(a.elapsed_time(b) for a, b in attend_events)
+    attend_ms = sum(attend_times) / len(attend_times)
     roof_bytes = sum(algorithmic_bytes(wl, [n + step + i for n in lens], n_layers)[0] for i in range(roof_steps))
     attend_bytes = roof_bytes / (roof_steps * n_layers)  # per kf_attend launch (append rows are ~1e-5 of it)
     step += roof_steps
@@ -543,7 +544,8 @@ def main():
         "roofline": {"bound": "hbm", "kernel": "attend_tma_kernel" if args.attend_impl != 1 else "attend_simple_kernel",
                      "achieved": achieved, "peak": peak, "unit": UNIT, "frac": achieved / peak,
                      "traffic": NCU_TRAFFIC_BYTES.get(wl.name), "algorithmic_bytes_per_launch": attend_bytes,
-                     "avg_launch_ms": attend_ms, "peak_source": peak_src,
+                     "avg_launch_ms": attend_ms, "median_launch_ms": attend_times[len(attend_times) // 2],
+                     "min_launch_ms": attend_times[0], "launches_timed": len(attend_times), "peak_source": peak_src,
                      "frac_of_nominal_8000": achieved / NOMINAL_PEAK_GBS,
                      "read_probe_gbs": probe_gbs, "frac_of_read_probe": achieved / probe_gbs if probe_gbs else None},
         "cpu_baseline": cpu,
