@@ -394,6 +394,7 @@ int kf_partial_attend(kf_ctx *ctx, int32_t layer, const void *q, const uint8_t *
     ap.o = nullptr;
     ap.lse = nullptr;
     ap.fused = 0;
+    ap.commit = 0;
     ap.part_mask = 0;
     for (int p = 0; p < ctx->cfg.n_partitions; ++p)
         if (!partition_mask || partition_mask[p]) ap.part_mask |= 1ull << p;
@@ -410,8 +411,8 @@ int kf_merge_partials(kf_ctx *ctx, const float *o_part, const float *lse_part, f
     return after_launch(ctx, launch_merge_ranges(ctx->dev, o_part, lse_part, o, lse, s));
 }
 
-int kf_attend(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, float *o_part, float *lse_part,
-              kf_stream stream) {
+int kf_attend_impl(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, float *o_part, float *lse_part,
+                   int commit, kf_stream stream) {
     if (!ctx || bad_layer(ctx, layer) || !q || !o || !lse || ((uintptr_t)q & 15) || ((uintptr_t)o & 15)) return KF_EINVAL;
     if ((o_part == nullptr) != (lse_part == nullptr) || ((uintptr_t)o_part & 15)) return KF_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
@@ -426,8 +427,16 @@ int kf_attend(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, f
     ap.o = o;
     ap.lse = lse;
     ap.fused = 1;
+    ap.commit = commit;
     ap.part_mask = ~0ull;
-    return run_attend(ctx, ap, s);
+    rc = run_attend(ctx, ap, s);
+    if (rc == KF_OK && commit) ctx->plan_dirty = true;  // lengths moved
+    return rc;
+}
+
+int kf_attend(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, float *o_part, float *lse_part,
+              kf_stream stream) {
+    return kf_attend_impl(ctx, layer, q, o, lse, o_part, lse_part, 0, stream);
 }
 
 int kf_step_commit(kf_ctx *ctx, kf_stream stream) {
@@ -446,8 +455,8 @@ static bool device_can_read(const void *host_ptr) {
     return a.type == cudaMemoryTypeHost && a.devicePointer == host_ptr;
 }
 
-int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host, const void *v_new_host,
-                       float *o_host, float *lse_host, kf_stream stream) {
+int kf_layer_step_host_impl(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host,
+                            const void *v_new_host, float *o_host, float *lse_host, int commit, kf_stream stream) {
     if (!ctx || bad_layer(ctx, layer) || !q_host || !k_new_host || !v_new_host || !o_host || !lse_host) return KF_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
     const Dev &d = ctx->dev;
@@ -459,7 +468,7 @@ int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const voi
         int rc = after_launch(ctx, launch_kv_append_stage(d, layer, (const __half *)k_new_host, (const __half *)v_new_host,
                                                           (const __half *)q_host, d.stage_q, s));
         if (rc != KF_OK) return rc;
-        return kf_attend(ctx, layer, d.stage_q, o_host, lse_host, nullptr, nullptr, stream);
+        return kf_attend_impl(ctx, layer, d.stage_q, o_host, lse_host, nullptr, nullptr, commit, stream);
     }
     const size_t qb = (size_t)d.B * d.Hq * kHeadDim * 2, kb = (size_t)d.B * d.Hkv * kHeadDim * 2;
     cudaError_t e = cudaMemcpyAsync(d.stage_q, q_host, qb, cudaMemcpyHostToDevice, s);
@@ -468,12 +477,17 @@ int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const voi
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     int rc = kf_kv_append(ctx, layer, d.stage_k, d.stage_v, stream);
     if (rc != KF_OK) return rc;
-    rc = kf_attend(ctx, layer, d.stage_q, d.stage_o, d.stage_lse, nullptr, nullptr, stream);
+    rc = kf_attend_impl(ctx, layer, d.stage_q, d.stage_o, d.stage_lse, nullptr, nullptr, commit, stream);
     if (rc != KF_OK) return rc;
     e = cudaMemcpyAsync(o_host, d.stage_o, (size_t)d.B * d.Hq * kHeadDim * 4, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(lse_host, d.stage_lse, (size_t)d.B * d.Hq * 4, cudaMemcpyDeviceToHost, s);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     return KF_OK;
+}
+
+int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host, const void *v_new_host,
+                       float *o_host, float *lse_host, kf_stream stream) {
+    return kf_layer_step_host_impl(ctx, layer, q_host, k_new_host, v_new_host, o_host, lse_host, 0, stream);
 }
 
 int kf_route_snapshot(kf_ctx *ctx, int32_t *len, int32_t *n_ranges, int32_t *part, int32_t *slot, int32_t *free_head,

@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32) attend_simple_kernel(Attend
         }
     }
     if (p.fused) merge_phase(p, ctr, W, lane);
-    launch_epilogue(d, W, lane);
+    launch_epilogue(d, W, lane, p.commit);
 }
 
 int launch_attend_simple(const AttendParams &p, int n_ctas, cudaStream_t s) {

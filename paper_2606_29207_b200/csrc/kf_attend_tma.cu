@@ -369,7 +369,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
         d.worker_times[4 * w + 2] = t_first;
         d.worker_times[4 * w + 3] = global_ns();
     }
-    launch_epilogue(d, W, lane);
+    launch_epilogue(d, W, lane, p.commit);
 }
 
 template <int WARPS, int STAGES>

@@ -115,6 +115,7 @@ struct AttendParams {
     float *lse;      // [B][Hq]
     uint64_t part_mask;
     int32_t fused;
+    int32_t commit;  // 1: the last worker of this launch performs the step commit (static step graph only)
 };
 
 __device__ __forceinline__ void set_error(const Dev &d, int code) { atomicCAS(d.error, 0, code); }

@@ -13,6 +13,17 @@ struct kf_ctx {
     char cuda_err[256];
 };
 
+// library-internal entry points of the static step graph (kf_graph.cu); not exported through include/kflume.h:
+// the same calls as their public namesakes plus a fusion that only makes sense inside one captured step
+#define KF_INTERNAL __attribute__((visibility("hidden")))
+extern "C" {
+KF_INTERNAL int kf_attend_impl(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, float *o_part, float *lse_part,
+                   int commit, kf_stream stream);                      // commit != 0: + kf_step_commit in the same launch
+KF_INTERNAL int kf_layer_step_host_impl(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host,
+                                        const void *v_new_host, float *o_host, float *lse_host, int commit,
+                                        kf_stream stream);
+}
+
 namespace kf {
 int cuda_fail(kf_ctx *ctx, cudaError_t e);  // records the error text in the ctx, returns KF_ECUDA
 }

@@ -90,16 +90,20 @@ int kf_step_graph_create(kf_ctx *ctx, int32_t n_layer_steps, const int32_t *laye
         delete g;
         return cuda_fail(ctx, e);
     }
+    // One fusion that only exists inside the captured step: the step commit is done by the last worker of the last
+    // attend launch (2n + 1 kernels per step instead of 2n + 2); the observable state after a launch is that of
+    // the public call sequence.  (Folding the first append into the single-CTA plan kernel was measured and
+    // dropped: one CTA needs 13 us to copy B = 64 rows that B CTAs copy in 4.)
     int rc = kf_token_boundary(ctx, stream);
     for (int i = 0; i < n_layer_steps && rc == KF_OK; ++i) {
+        const int commit = i == n_layer_steps - 1;
         if (g->host_io) {
-            rc = kf_layer_step_host(ctx, layers[i], q[i], k_new[i], v_new[i], o[i], lse[i], stream);
+            rc = kf_layer_step_host_impl(ctx, layers[i], q[i], k_new[i], v_new[i], o[i], lse[i], commit, stream);
         } else {
             rc = kf_kv_append(ctx, layers[i], k_new[i], v_new[i], stream);
-            if (rc == KF_OK) rc = kf_attend(ctx, layers[i], q[i], o[i], lse[i], nullptr, nullptr, stream);
+            if (rc == KF_OK) rc = kf_attend_impl(ctx, layers[i], q[i], o[i], lse[i], nullptr, nullptr, commit, stream);
         }
     }
-    if (rc == KF_OK) rc = kf_step_commit(ctx, stream);
     e = cudaStreamEndCapture(s, &g->graph);
     g->kernels_per_launch = (int)(ctx->launches - launches0);
     ctx->launches = launches0;  // nothing ran yet
@@ -109,9 +113,9 @@ int kf_step_graph_create(kf_ctx *ctx, int32_t n_layer_steps, const int32_t *laye
         if (e != cudaSuccess) rc = cuda_fail(ctx, e);
     }
     if (rc == KF_OK && !g->host_io) {
-        // kernel order of the capture: plan, n x (append, attend), commit
+        // kernel order of the capture: plan, n x (append, attend)
         std::vector<cudaGraphNode_t> chain;
-        if (kernel_chain(g->graph, chain) != 0 || (int)chain.size() != 2 * n_layer_steps + 2) {
+        if (kernel_chain(g->graph, chain) != 0 || (int)chain.size() != 2 * n_layer_steps + 1) {
             snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "unexpected step-graph topology");
             rc = KF_ECUDA;
         } else {
@@ -173,6 +177,7 @@ int kf_step_graph_launch(kf_graph *g, const void *const *q, const void *const *k
                 ap.o = o[i];
                 ap.lse = lse[i];
                 ap.fused = 1;
+                ap.commit = i == g->n - 1;
                 ap.part_mask = ~0ull;
                 void *args[1] = {&ap};
                 cudaKernelNodeParams p = g->attend_params[i];

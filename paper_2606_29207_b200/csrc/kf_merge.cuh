@@ -187,8 +187,11 @@ __device__ __forceinline__ Counters launch_prologue(const Dev &d, int w, int W, 
     return c;
 }
 
-// the last worker to finish rewinds the tickets and flips the epoch for the next launch
-__device__ __forceinline__ void launch_epilogue(const Dev &d, int W, int lane) {
+// the last worker to finish rewinds the tickets and flips the epoch for the next launch; with `commit` (the last
+// layer-step of a static step graph) it also performs the step commit a5 -- len_r += 1 -- which no worker of this
+// launch reads any more: each of them read len before its own release below
+__device__ __forceinline__ void launch_epilogue(const Dev &d, int W, int lane, int commit = 0) {
+    int last = 0;
     if (lane == 0) {
         release_fence();
         const int old = atomicAdd(d.sched + 1, 1);
@@ -198,6 +201,15 @@ __device__ __forceinline__ void launch_epilogue(const Dev &d, int W, int lane) {
             d.sched[2] = 0;
             d.sched[3] = 0;
             d.sched[4] = d.sched[4] + 1;
+            last = 1;
+        }
+    }
+    if (commit) {
+        last = __shfl_sync(0xffffffffu, last, 0);
+        if (last) {
+            asm volatile("fence.acq_rel.gpu;" ::: "memory");  // acquire side: every worker's reads of len are done
+            for (int r = lane; r < d.B; r += 32)
+                if (d.len[r] >= 0) d.len[r] += 1;
         }
     }
 }

@@ -265,10 +265,10 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
             }
         }
         __syncthreads();
-        if (s_keep) return;
     } else if (tid == 0) {
         *d.plan_age = 0;
     }
+    if (do_boundary && s_keep) return;
     int used = 0;
     auto take = [&](int n, int *fallback) -> int * {
         if (used + n <= kPlanSmemInts) {
