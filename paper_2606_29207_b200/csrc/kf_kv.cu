@@ -53,12 +53,15 @@ __global__ void __launch_bounds__(256) kv_append_kernel(Dev d, int layer, const 
 __global__ void __launch_bounds__(256) kv_append_stage_kernel(Dev d, int layer, const __half *k_new,
                                                               const __half *v_new, const __half *q_src,
                                                               __half *q_dst) {
+    // grid (B, kStageSplit): bus reads are latency-bound (~2 us each), so a request's q rows are spread over several
+    // CTAs; slice 0 also appends the K/V rows
     const int r = blockIdx.x;
     const int q_chunks = d.Hq * 16;  // 16-byte chunks of this request's q rows
-    for (int i = threadIdx.x; i < q_chunks; i += blockDim.x) {
+    for (int i = blockIdx.y * blockDim.x + threadIdx.x; i < q_chunks; i += gridDim.y * blockDim.x) {
         const size_t off = (size_t)r * q_chunks + i;
         reinterpret_cast<int4 *>(q_dst)[off] = __ldcv(reinterpret_cast<const int4 *>(q_src) + off);
     }
+    if (blockIdx.y != 0) return;
     const int len = d.len[r];
     if (len < 0) return;
     const int j = len / d.R, off = len - j * d.R;
@@ -93,7 +96,8 @@ int launch_kv_append(const Dev &d, int layer, const __half *k_new, const __half 
 
 int launch_kv_append_stage(const Dev &d, int layer, const __half *k_new, const __half *v_new, const __half *q_src,
                            __half *q_dst, cudaStream_t s) {
-    kv_append_stage_kernel<<<d.B, 256, 0, s>>>(d, layer, k_new, v_new, q_src, q_dst);
+    const int split = d.Hq * 16 > 256 ? (d.Hq * 16 + 255) / 256 : 1;  // one q chunk per thread
+    kv_append_stage_kernel<<<dim3(d.B, split), 256, 0, s>>>(d, layer, k_new, v_new, q_src, q_dst);
     return 1;
 }
 
