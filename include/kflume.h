@@ -138,6 +138,13 @@ int kf_close_request(kf_ctx *ctx, int32_t req, kf_stream stream);
  *   tokens[P] = committed tokens resident on each partition (x 2*H_kv*d*2 B*L = KV bytes),
  *   tails[P] = open requests whose tail range lives there.  Any pointer may be NULL.  Synchronises `stream`. */
 int kf_set_active_partitions(kf_ctx *ctx, const uint8_t *active, kf_stream stream);
+/* kf_set_active_requests -- which OPEN requests take part in the following decode steps (continuous batching: a
+ *   request may sit out steps without being closed; Algorithm 1 counts only "r active", l.7).  active: [device]
+ *   uint8[B], non-zero = active, or NULL = all (the initial state).  A paused request keeps its routes and KV;
+ *   kf_token_boundary opens no range for it, kf_kv_append ignores its row, the attend / merge calls produce no
+ *   output for it (its rows of o / lse / partials are left untouched), kf_step_commit leaves its len alone, and
+ *   kf_partition_state does not count it as a tail.  The buffer is read asynchronously on `stream`. */
+int kf_set_active_requests(kf_ctx *ctx, const uint8_t *active, kf_stream stream);
 int kf_partition_state(kf_ctx *ctx, int32_t *active, int64_t *tokens, int32_t *tails, kf_stream stream);
 
 /* kf_load_context: copies tokens [tok_begin, tok_begin + n_tokens) of request `req`, layer `layer`, into the

@@ -40,6 +40,7 @@ class RoutingModel:
         self.rr_cursor = 0                                  # ranges allocated so far
         self.rr_last = -1                                   # partition of the last allocation
         self.active = [True] * n_partitions                 # partitions that receive new ranges
+        self.req_active = [True] * max_requests             # requests that take part in decode steps ("r active")
         self.free_head = [0] * n_partitions                 # bump allocator
         self.free_list: List[List[int]] = [[] for _ in range(n_partitions)]  # LIFO of released slots
 
@@ -87,7 +88,7 @@ class RoutingModel:
         Returns the events [(req, range_index, partition, slot)]."""
         events = []
         for r in range(self.B):
-            if self.len[r] < 0:
+            if self.len[r] < 0 or not self.req_active[r]:
                 continue
             if self.len[r] % self.R == 0 and len(self.route[r]) == self.len[r] // self.R:
                 p, s = self._alloc(r)
@@ -107,7 +108,7 @@ class RoutingModel:
 
     def step_commit(self) -> None:
         for r in range(self.B):
-            if self.len[r] >= 0:
+            if self.len[r] >= 0 and self.req_active[r]:
                 self.len[r] += 1
 
     def close_request(self, req: int) -> None:
@@ -124,6 +125,10 @@ class RoutingModel:
             raise RoutingError("EINVAL")
         self.active = [bool(a) for a in active]
 
+    def set_active_requests(self, active=None) -> None:
+        """Requests that take part in the following decode steps; a paused request keeps its routes and tokens."""
+        self.req_active = [True] * self.B if active is None else [bool(a) for a in active]
+
     def partition_state(self) -> Dict[str, object]:
         """What the scaling policy monitors (Algorithm 1, l.6-9): committed tokens per partition, tails per partition."""
         tokens, tails = [0] * self.P, [0] * self.P
@@ -132,7 +137,7 @@ class RoutingModel:
                 continue
             for j, (p, _) in enumerate(self.route[r]):
                 tokens[p] += max(0, min(self.R, self.len[r] - j * self.R))
-                if j == len(self.route[r]) - 1:
+                if j == len(self.route[r]) - 1 and self.req_active[r]:   # "r active" (Algorithm 1, l.7)
                     tails[p] += 1
         return {"active": [1 if a else 0 for a in self.active], "tokens": tokens, "tails": tails}
 

@@ -19,7 +19,7 @@ EXPORTS = [
     "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_step_commit", "kf_layer_step_host",
     "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count", "kf_worker_times",
     "kf_step_graph_create", "kf_step_graph_launch", "kf_step_graph_destroy", "kf_probe_read",
-    "kf_set_active_partitions", "kf_partition_state",
+    "kf_set_active_partitions", "kf_partition_state", "kf_set_active_requests",
     "kf_policy_bytes_per_token", "kf_policy_threshold", "kf_policy_initial_nodes", "kf_policy_step",
 ]
 
@@ -93,6 +93,7 @@ def load_library():
     L.kf_step_graph_launch.argtypes = [vp, pp, pp, pp, pp, pp, vp]
     L.kf_step_graph_destroy.argtypes = [vp]
     L.kf_set_active_partitions.argtypes = [vp, ctypes.POINTER(ctypes.c_uint8), vp]
+    L.kf_set_active_requests.argtypes = [vp, vp, vp]
     L.kf_partition_state.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32), vp]
     pcp = ctypes.POINTER(kf_policy_config)
     u8p = ctypes.POINTER(ctypes.c_uint8)
@@ -271,6 +272,12 @@ class KFlume:
         assert len(active) == self.P
         arr = (ctypes.c_uint8 * self.P)(*[1 if x else 0 for x in active])
         self._check(self.lib.kf_set_active_partitions(self.h, arr, self._stream(stream)), "kf_set_active_partitions")
+
+    def set_active_requests(self, active=None, stream=None):
+        """active: CUDA uint8 tensor [B] (non-zero = takes part in decode steps) or None = all."""
+        if active is not None:
+            assert active.is_cuda and active.dtype == self.torch.uint8 and active.numel() == self.B
+        self._check(self.lib.kf_set_active_requests(self.h, _ptr(active), self._stream(stream)), "kf_set_active_requests")
 
     def partition_state(self, stream=None) -> dict:
         act, tok, tails = (ctypes.c_int32 * self.P)(), (ctypes.c_int64 * self.P)(), (ctypes.c_int32 * self.P)()

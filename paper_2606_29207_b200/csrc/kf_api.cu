@@ -32,7 +32,7 @@ size_t max_chunks_of(const kf_config *c) {
 inline size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t len, n_ranges, route_part, route_slot, rr_cursor, rr_last, active, part_tokens, part_tails, free_head, free_cnt, free_stack, error, plan, units, chunks, plan_age, sched,
+    size_t len, n_ranges, route_part, route_slot, rr_cursor, rr_last, req_active, active, part_tokens, part_tails, free_head, free_cnt, free_stack, error, plan, units, chunks, plan_age, sched,
         scratch, unit_counter, group_counter, piece_o, piece_lse, range_o, range_lse, stage_q, stage_k, stage_v,
         stage_o, stage_lse, tmaps, worker_times, total;
 };
@@ -83,6 +83,7 @@ Layout make_layout(const kf_config *c) {
     L.route_slot = take(E * 4);
     L.rr_cursor = take(4);
     L.rr_last = take(4);
+    L.req_active = take(B * 4);
     L.active = take(P * 4);
     L.part_tokens = take(P * 8);
     L.part_tails = take(P * 4);
@@ -291,6 +292,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.route_slot = (int32_t *)(ws + L.route_slot);
     d.rr_cursor = (int32_t *)(ws + L.rr_cursor);
     d.rr_last = (int32_t *)(ws + L.rr_last);
+    d.req_active = (int32_t *)(ws + L.req_active);
     d.active = (int32_t *)(ws + L.active);
     d.part_tokens = (long long *)(ws + L.part_tokens);
     d.part_tails = (int32_t *)(ws + L.part_tails);
@@ -320,6 +322,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.v_off = half_pool_bytes(cfg);
     for (int p = 0; p < cfg->n_partitions; ++p) d.pool[p] = (unsigned char *)pool_ptrs[p];
 
+    launch_set_req_active(ctx->dev, nullptr, 0);  // every request takes part in decode steps until told otherwise
     if (plan_setup() != 0) return cuda_fail(ctx, cudaGetLastError());
     if (ctx->impl == KF_IMPL_TMA) {
         int rc = encode_tmaps(ctx, pool_ptrs);
@@ -515,6 +518,12 @@ int kf_set_active_partitions(kf_ctx *ctx, const uint8_t *active, kf_stream strea
         if (active[p]) mask |= 1ull << p;
     if (mask == 0) return KF_EINVAL;
     return after_launch(ctx, launch_set_active(ctx->dev, mask, (cudaStream_t)stream));
+}
+
+int kf_set_active_requests(kf_ctx *ctx, const uint8_t *active_dev, kf_stream stream) {
+    if (!ctx) return KF_EINVAL;
+    ctx->plan_dirty = true;
+    return after_launch(ctx, launch_set_req_active(ctx->dev, active_dev, (cudaStream_t)stream));
 }
 
 int kf_partition_state(kf_ctx *ctx, int32_t *active, int64_t *tokens, int32_t *tails, kf_stream stream) {

@@ -73,6 +73,7 @@ struct Dev {
     int32_t *route_slot; // [B][Jmax]
     int32_t *rr_cursor;  // [1]   ranges allocated so far
     int32_t *rr_last;    // [1]   partition of the last allocation (-1: none yet)
+    int32_t *req_active; // [B]   1: the request takes part in decode steps (kf_set_active_requests); 0: paused
     int32_t *active;     // [P]   1: partition receives new ranges (the published active set)
     long long *part_tokens;  // [P] scratch of kf_partition_state
     int32_t *part_tails;     // [P]
@@ -147,6 +148,7 @@ int launch_plan(const Dev &d, int do_boundary, cudaStream_t s);  // (a1, optiona
 int plan_setup();        // cudaFuncSetAttribute for the plan kernel's dynamic shared memory; 0 or KF_ECUDA
 int launch_step_commit(const Dev &d, cudaStream_t s);
 int launch_set_active(const Dev &d, unsigned long long mask, cudaStream_t s);
+int launch_set_req_active(const Dev &d, const unsigned char *mask_dev, cudaStream_t s);
 int launch_partition_state(const Dev &d, long long *tokens, int *tails, cudaStream_t s);
 int launch_load_context(const Dev &d, int layer, int req, int tok_begin, int n_tokens, const __half *k,
                         const __half *v, cudaStream_t s);

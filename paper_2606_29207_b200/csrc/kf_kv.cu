@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(256) kv_append_kernel(Dev d, int layer, const 
                                                         const __half *__restrict__ v_new) {
     const int r = blockIdx.x;
     const int len = d.len[r];
-    if (len < 0) return;
+    if (len < 0 || !d.req_active[r]) return;
     const int j = len / d.R, off = len - j * d.R;
     if (j >= d.n_ranges[r]) {
         if (threadIdx.x == 0) set_error(d, KF_ESTATE);
@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(256) kv_append_stage_kernel(Dev d, int layer, 
     }
     if (blockIdx.y != 0) return;
     const int len = d.len[r];
-    if (len < 0) return;
+    if (len < 0 || !d.req_active[r]) return;
     const int j = len / d.R, off = len - j * d.R;
     if (j >= d.n_ranges[r]) {
         if (threadIdx.x == 0) set_error(d, KF_ESTATE);

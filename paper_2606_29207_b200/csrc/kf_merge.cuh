@@ -209,7 +209,7 @@ __device__ __forceinline__ void launch_epilogue(const Dev &d, int W, int lane, i
         if (last) {
             asm volatile("fence.acq_rel.gpu;" ::: "memory");  // acquire side: every worker's reads of len are done
             for (int r = lane; r < d.B; r += 32)
-                if (d.len[r] >= 0) d.len[r] += 1;
+                if (d.len[r] >= 0 && d.req_active[r]) d.len[r] += 1;
         }
     }
 }

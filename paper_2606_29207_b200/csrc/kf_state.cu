@@ -97,7 +97,7 @@ __device__ int token_boundary_warp(const Dev &d, int lane) {
         bool need = false;
         if (r < d.B) {
             const int len = d.len[r];
-            need = len >= 0 && (len % d.R) == 0 && d.n_ranges[r] == len / d.R;
+            need = len >= 0 && d.req_active[r] && (len % d.R) == 0 && d.n_ranges[r] == len / d.R;
         }
         unsigned m = __ballot_sync(0xffffffffu, need);
         opened += __popc(m);
@@ -119,6 +119,14 @@ __global__ void set_active_kernel(Dev d, unsigned long long mask) {
     if (p < d.P) d.active[p] = (int)((mask >> p) & 1ull);
 }
 
+// which open requests take part in the following decode steps (continuous batching: a request may pause);
+// mask == nullptr: all.  The plan depends on it: aged to stale.
+__global__ void set_req_active_kernel(Dev d, const unsigned char *mask) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r < d.B) d.req_active[r] = mask ? (mask[r] ? 1 : 0) : 1;
+    if (r == 0) *d.plan_age = kPlanStale;
+}
+
 // per-partition occupancy for the scaling policy (Algorithm 1, l.6-9): committed tokens resident on partition p
 // and the number of open requests whose tail range lives there.  One thread per request, atomics on [P] words.
 __global__ void partition_state_kernel(Dev d, long long *tokens, int *tails) {
@@ -131,13 +139,13 @@ __global__ void partition_state_kernel(Dev d, long long *tokens, int *tails) {
         const int p = d.route_part[(size_t)r * d.Jmax + j];
         const long long cnt = max(0, min(d.R, len - j * d.R));
         atomicAdd(reinterpret_cast<unsigned long long *>(tokens + p), (unsigned long long)cnt);
-        if (j == J - 1) atomicAdd(tails + p, 1);
+        if (j == J - 1 && d.req_active[r]) atomicAdd(tails + p, 1);  // "r active" (Alg. 1 l.7)
     }
 }
 
 __global__ void step_commit_kernel(Dev d) {
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
-    if (r < d.B && d.len[r] >= 0) d.len[r] += 1;
+    if (r < d.B && d.len[r] >= 0 && d.req_active[r]) d.len[r] += 1;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -289,7 +297,7 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
     // 1. per request: tokens attended this step S = len + 1, ranges J = ceil(S / R)
     for (int r = tid; r < B; r += nt) {
         const int len = d.len[r];
-        int64_t S = len >= 0 ? (int64_t)len + 1 : 0;
+        int64_t S = (len >= 0 && d.req_active[r]) ? (int64_t)len + 1 : 0;  // closed or paused: no work this step
         int J = (int)((S + d.R - 1) / d.R);
         const int nr = d.n_ranges[r];
         if (J > nr) {  // no route for the tail position: kf_token_boundary was not called
@@ -464,6 +472,10 @@ int plan_setup() {
 }
 int launch_set_active(const Dev &d, unsigned long long mask, cudaStream_t s) {
     set_active_kernel<<<1, kMaxPartitions, 0, s>>>(d, mask);
+    return 1;
+}
+int launch_set_req_active(const Dev &d, const unsigned char *mask_dev, cudaStream_t s) {
+    set_req_active_kernel<<<(d.B + 127) / 128, 128, 0, s>>>(d, mask_dev);
     return 1;
 }
 int launch_partition_state(const Dev &d, long long *tokens, int *tails, cudaStream_t s) {

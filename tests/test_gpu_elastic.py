@@ -176,3 +176,52 @@ def test_algorithm1_closed_loop_device_equals_model():
     # a node stops receiving ranges once published away; it may still grow until its tails' current ranges fill
     assert max(final_tokens[:3]) <= 400 + wl.batch * R        # (the last node has no successor to hand over to)
     ses.close()
+
+
+def test_paused_requests_sit_out_steps():
+    # requests pause and resume between decode steps (kf_set_active_requests); paused rows are untouched, their
+    # length and routes frozen; everything else matches the oracle and the model at every step
+    wl = Workload("pause", 32, 8, 32, 3, [70, 32, 33, 100, 64, 5])
+    steps = 14
+    ses = Session(wl, steps=steps, slack_slots=4)
+    ses.prepare()
+    kf = ses.kf
+    B = wl.batch
+    model = RoutingModel(3, 32, B, kf.Jmax, kf.cfg.slots_per_partition)
+    for r, n in enumerate(ses.len0):
+        model.open_request(r, n)
+    schedule = {0: [1, 0, 1, 1, 0, 1], 4: [1, 1, 0, 1, 0, 1], 8: [0, 1, 1, 0, 1, 1], 11: None}
+    act = [1] * B
+    lens = list(ses.len0)
+    pos_dev = torch.tensor(lens, dtype=torch.int32, device="cuda")
+    from kf_inputs import gen, gen_device
+    for t in range(steps):
+        if t in schedule:
+            mask = schedule[t]
+            act = [1] * B if mask is None else mask
+            kf.set_active_requests(None if mask is None else torch.tensor(mask, dtype=torch.uint8, device="cuda"))
+            model.set_active_requests(mask)
+        kf.token_boundary()
+        model.token_boundary()
+        q = ses.q_for(0, t)
+        # K/V_new of a request is the generator value at ITS OWN next position (paused requests do not advance)
+        pos_dev.copy_(torch.tensor(lens, dtype=torch.int32))
+        k_new = gen_device.fill_rows(gen.STREAM_K, 0, pos_dev, wl.n_kv_heads, seed=wl.seed)
+        v_new = gen_device.fill_rows(gen.STREAM_V, 0, pos_dev, wl.n_kv_heads, seed=wl.seed)
+        ses.o.fill_(float("nan"))
+        ses.lse.fill_(float("nan"))
+        ses.layer_step(0, q, k_new, v_new)
+        kf.step_commit()
+        model.step_commit()
+        assert kf.status() == KF_OK
+        o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+        for r in range(B):
+            if act[r]:
+                o_ref, lse_ref = oracle_request(wl, 0, r, t, lens[r] + 1)
+                check_close(o[r], lse[r], o_ref, lse_ref, f"pause step{t} r{r}")
+                lens[r] += 1
+            else:
+                assert np.isnan(o[r]).all() and np.isnan(lse[r]).all(), (t, r)
+        _same(kf, model)
+        assert kf.route_snapshot()["len"] == lens
+    ses.close()

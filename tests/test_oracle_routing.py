@@ -199,3 +199,26 @@ def test_scale_down_keeps_existing_ranges_and_starves_the_retired_node():
     assert st["tokens"][0] * 2 * 8 * 128 * 32 * 2 == st["tokens"][0] * 131072
     with pytest.raises(RoutingError):
         m.set_active([0, 0, 0])
+
+
+def test_paused_requests_keep_routes_and_length():
+    # continuous batching: a request that sits out steps ("r active", Algorithm 1 l.7) is frozen -- no range is
+    # opened for it even at a range edge, its length does not move, it is not counted as a tail -- and resumes intact
+    R = 4
+    m = RoutingModel(2, R, 3, 8, 8)
+    for r, n in enumerate([4, 3, 6]):             # request 0 sits exactly at a range edge
+        m.open_request(r, n)
+    m.set_active_requests([0, 1, 1])
+    routes0 = list(m.route[0])
+    for _ in range(5):
+        ev = m.token_boundary()
+        assert all(e[0] != 0 for e in ev)
+        m.step_commit()
+    assert m.len == [4, 8, 11] and m.route[0] == routes0
+    st = m.partition_state()
+    assert sum(st["tails"]) == 2 and sum(st["tokens"]) == 4 + 8 + 11
+    m.set_active_requests(None)                   # resume: now the edge opens range 1 for request 0
+    ev = m.token_boundary()
+    assert [e[:2] for e in ev if e[0] == 0] == [(0, 1)]
+    m.step_commit()
+    assert m.len[0] == 5 and sum(m.partition_state()["tails"]) == 3
