@@ -265,6 +265,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 50)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--min-tiles", type=int, default=0)
+    ap.add_argument("--kv-l2-policy", type=int, default=0, help="kf_config.kv_l2_policy: 0 default, 1 evict-first, 2 normal")
     ap.add_argument("--route-install", action="store_true", help="measure the latency of a scale event (route "
                     "install) and of the token boundary instead of the decode benchmark")
     ap.add_argument("--no-l2-flush", action="store_true", help="do not flush L2 between timed steps when the KV of a "
@@ -306,7 +307,7 @@ def main():
         per_layer = wl.slots_per_partition(total_steps) * wl.n_partitions * wl.range_tokens * wl.kv_bytes_per_token()
         L_phys = max(1, min(n_layers, int(0.85 * free // per_layer)))
     ses = Session(wl, impl=args.attend_impl, n_layers_phys=L_phys, steps=total_steps, min_tiles=args.min_tiles,
-                  device=str(dev))
+                  device=str(dev), kv_l2_policy=args.kv_l2_policy)
     kf = ses.kf
     ses.prepare()
     assert kf.status() == 0

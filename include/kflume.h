@@ -85,6 +85,8 @@ typedef struct kf_config {
     int32_t sched_decay_pct;        /* 1..99: share of a unit's remaining tiles that each scheduling level takes */
     int32_t plan_refresh_steps;     /* the work plan is rebuilt when a route changes or after this many token boundaries
                                      * (0 => 128; 1 => every step); in between, tail ranges grow inside the kept plan */
+    int32_t kv_l2_policy;           /* L2 policy of the K/V tile loads: 0 => default (1); 1 = evict-first (K/V is read once
+                                     * per launch; keeps q, partials and the plan resident: +1..5% measured); 2 = normal */
 } kf_config;
 
 typedef struct kf_ctx kf_ctx;

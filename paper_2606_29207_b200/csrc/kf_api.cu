@@ -59,6 +59,7 @@ bool valid_config(const kf_config *c) {
     if (c->sched_first_pct < 0 || c->sched_first_pct > 100) return false;
     if (c->sched_decay_pct < 0 || c->sched_decay_pct > 99) return false;
     if (c->plan_refresh_steps < 0) return false;
+    if (c->kv_l2_policy < 0 || c->kv_l2_policy > 2) return false;
     // rows of one K (or V) half-pool must fit the int32 TMA coordinate
     const double rows = (double)c->n_layers * c->slots_per_partition * c->n_kv_heads * c->range_tokens;
     if (rows >= 2147483647.0) return false;
@@ -280,7 +281,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.warps_per_cta = warps;
     d.stages = cfg->pipeline_stages ? cfg->pipeline_stages : kDefaultStages;
     d.max_chunks = (int32_t)max_chunks_of(cfg);
-    d.l2_hint = getenv("KF_L2_HINT") ? atoi(getenv("KF_L2_HINT")) : 0;  // experiment knob
+    d.l2_hint = cfg->kv_l2_policy == 2 ? 0 : 1;  // K/V is read once per launch: evict-first by default
     d.plan_refresh = cfg->plan_refresh_steps > 0 ? cfg->plan_refresh_steps : kDefaultPlanRefresh;
     d.sched_first = 0.01f * (cfg->sched_first_pct ? cfg->sched_first_pct : kDefaultFirstPct);
     d.sched_decay = 0.01f * (cfg->sched_decay_pct ? cfg->sched_decay_pct : kDefaultDecayPct);
