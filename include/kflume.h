@@ -75,7 +75,7 @@ typedef struct kf_config {
     int32_t slots_per_partition;    /* token-range slots in each partition pool                   */
     float softmax_scale;            /* 0 => 1/sqrt(head_dim); scores are scale * q.k              */
     int32_t attend_impl;            /* KF_IMPL_*                                                  */
-    int32_t min_tiles_per_worker;   /* smallest chunk of the work plan, in 16-token tiles; 0 => 8 when the step has at
+    int32_t min_tiles_per_worker;   /* smallest chunk of the work plan, in 16-token tiles; 0 => 12 when the step has at
                                      * least 16 tiles per worker, else 4 */
     /* tuning of the attend kernel and its work plan; 0 => default.  Results are bit-identical for a given
      * (min_tiles_per_worker, workers_per_sm, sched_*) because the plan's cuts depend only on these. */

@@ -330,9 +330,9 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
     const int Nt = block_exclusive_scan(tpre, E);
     if (tid == 0) {
         tpre[E] = Nt;
-        // smallest chunk: fewer, larger pieces pay off once every worker has real work (measured: 8 beats 4 by
+        // smallest chunk: fewer, larger pieces pay off once every worker has real work (measured: 8..12 beat 4 by
         // 1-7% from 64K context tokens up), while a latency-bound launch wants all the parallelism it can get
-        s_m = d.min_tiles > 0 ? d.min_tiles : (Nt >= 16 * d.max_workers ? 8 : 4);
+        s_m = d.min_tiles > 0 ? d.min_tiles : (Nt >= 16 * d.max_workers ? 12 : 4);
     }
     __syncthreads();
 
