@@ -33,9 +33,9 @@ NOMINAL_PEAK_GBS = 8000.0        # BASELINE.json's "~8 TB/s" denominator (contex
 FALLBACK_PEAK_GBS = 6650.0       # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 
 # dram__bytes_read.sum + dram__bytes_write.sum per kf_attend launch from the committed `ncu --set full` capture
-# (profiles/r01f_attend_full_<workload>.md); None where no capture exists for that workload.
-NCU_TRAFFIC_BYTES = {"cfg1": 16931456, "cfg2": 1099491056, "cfg3": 4798301336, "cfg4": 4336263200,
-                     "cfg5": 37223307860}
+# (profiles/r01g_attend_full_<workload>.md); None where no capture exists for that workload.
+NCU_TRAFFIC_BYTES = {"cfg1": 16939392, "cfg2": 1085991552, "cfg3": 4782093992, "cfg4": 4307839832,
+                     "cfg5": 37122728208}
 
 
 def load_peak():
