@@ -463,9 +463,9 @@ def main():
     value = sharding.throughput_gbs(total_bytes_all, ms)
     ms_per_step = ms / args.steps
 
-    # ---- end to end: HOST buffers, copies inside the timed region.  One replay per step of a host-io step graph
-    #      (pinned, pre-registered buffers: PAPER.md:177): every layer-step copies q / k_new / v_new host->device and
-    #      o / lse device->host; the caller rewrites the pinned inputs and reads the result every step ---------------
+    # ---- end to end: HOST buffers, transfers inside the timed region.  One replay per step of a host-io step graph
+    #      (pinned buffers): every layer-step reads q / k_new / v_new from host memory over the bus and
+    #      writes o / lse to host memory; the caller reads the result on the host every step ---------------------------
     B, Hq, Hkv = wl.batch, wl.n_q_heads, wl.n_kv_heads
     host_in = []
     for i in range(e2e_steps):
@@ -491,11 +491,9 @@ def main():
                 qx, kx, vx = host_in[i][layer % L_phys]
                 kf.layer_step_host(layer % L_phys, qx, kx, vx, o_h[layer], l_h[layer])
             kf.step_commit()
-        else:
-            for layer in range(n_layers):           # the producer writes this step's inputs into the bound buffers
-                qx, kx, vx = host_in[i][layer % L_phys]
-                qh[layer].copy_(qx), kh[layer].copy_(kx), vh[layer].copy_(vx)
-            hgraph.launch()
+        else:                                       # this step's own pinned input buffers are re-bound
+            hgraph.launch([host_in[i][lp][0] for lp in layer_ids], [host_in[i][lp][1] for lp in layer_ids],
+                          [host_in[i][lp][2] for lp in layer_ids], o_h, l_h)
         torch.cuda.current_stream(dev).synchronize()      # the caller reads the step's result on the host
         checksum += float(l_h[n_layers - 1][0, 0])
     e1.record()

@@ -214,11 +214,14 @@ int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const voi
  * kf_step_graph_create: captures on `stream` (must not be the legacy default stream; nothing executes) and
  *   instantiates.  layers: [host] int32[n], physical layer of each layer-step.  q, k_new, v_new, o, lse: [host]
  *   arrays of n pointers, shapes as in kf_kv_append / kf_attend.  host_io == 0: they are [device] pointers and may
- *   be re-bound at every launch.  host_io != 0: they are PINNED [host] buffers (the end-to-end path: each
- *   layer-step copies q / k_new / v_new to device staging and o / lse back); they are bound for the graph's
- *   lifetime -- the caller rewrites their contents between launches (pre-registered buffers).
+ *   be re-bound at every launch.  host_io != 0: they are PINNED [host] buffers (the end-to-end path of
+ *   kf_layer_step_host: zero-copy reads of q / k_new / v_new, o / lse written straight to the host).  Pinned,
+ *   16-byte aligned buffers may be re-bound at every launch as well; buffers that had to go through copy nodes
+ *   (not device-accessible) are bound for the graph's lifetime -- the caller rewrites their contents between
+ *   launches (pre-registered buffers).
  * kf_step_graph_launch: one decode step.  q .. lse: all NULL = keep the bound pointers; else all five arrays
- *   [host, n pointers each] re-bind the device pointers (host-side node update; no re-instantiation).
+ *   [host, n pointers each] re-bind the pointers (host-side node update; no re-instantiation; KF_EINVAL for a
+ *   host-io graph with copy nodes or for host pointers the GPU cannot dereference).
  *   Asynchronous on `stream`.  Errors as the calls it contains (device errors via kf_status).
  * kf_step_graph_destroy: frees the graph; the ctx must still be alive. */
 typedef struct kf_graph kf_graph;

@@ -341,7 +341,8 @@ class StepGraph:
         return [(ctypes.c_void_p * self.n)(*[t.data_ptr() for t in lst]) for lst in (q, k_new, v_new, o, lse)]
 
     def launch(self, q=None, k_new=None, v_new=None, o=None, lse=None, stream=None):
-        """One decode step.  Pass all five lists to re-bind the device pointers, or none to keep them."""
+        """One decode step.  Pass all five lists to re-bind the pointers (device tensors, or pinned host tensors for a
+        host-io graph), or none to keep them."""
         if q is None:
             args = [None] * 5
         else:

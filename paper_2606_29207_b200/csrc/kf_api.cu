@@ -17,6 +17,15 @@ int cuda_fail(kf_ctx *ctx, cudaError_t e) {
     if (ctx) snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
     return KF_ECUDA;
 }
+// true if the GPU can dereference this host pointer as it is (pinned memory under unified addressing)
+bool device_can_read(const void *host_ptr) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, host_ptr) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeHost && a.devicePointer == host_ptr;
+}
 }  // namespace kf
 
 namespace {
@@ -449,15 +458,6 @@ int kf_step_commit(kf_ctx *ctx, kf_stream stream) {
     return after_launch(ctx, launch_step_commit(ctx->dev, (cudaStream_t)stream));
 }
 
-// true if the GPU can dereference this host pointer as it is (pinned memory under unified addressing)
-static bool device_can_read(const void *host_ptr) {
-    cudaPointerAttributes a;
-    if (cudaPointerGetAttributes(&a, host_ptr) != cudaSuccess) {
-        cudaGetLastError();
-        return false;
-    }
-    return a.type == cudaMemoryTypeHost && a.devicePointer == host_ptr;
-}
 
 int kf_layer_step_host_impl(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host,
                             const void *v_new_host, float *o_host, float *lse_host, int commit, kf_stream stream) {

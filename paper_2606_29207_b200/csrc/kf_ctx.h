@@ -26,4 +26,5 @@ KF_INTERNAL int kf_layer_step_host_impl(kf_ctx *ctx, int32_t layer, const void *
 
 namespace kf {
 int cuda_fail(kf_ctx *ctx, cudaError_t e);  // records the error text in the ctx, returns KF_ECUDA
+bool device_can_read(const void *host_ptr);  // pinned host memory the GPU can dereference as it is
 }

@@ -21,7 +21,8 @@ struct kf_graph {
     cudaGraph_t graph;
     cudaGraphExec_t exec;
     int n;                                  // layer-steps per launch
-    int host_io;                            // 1: q/k/v/o/lse are pinned host buffers bound at create time
+    int host_io;                            // 1: q/k/v/o/lse are pinned host buffers
+    bool zero_copy;                         // host_io graph made of kernels only (no copy nodes): re-bindable
     int kernels_per_launch;
     std::vector<int32_t> layers;
     std::vector<cudaGraphNode_t> append_nodes, attend_nodes;   // [n] (device-pointer graphs only)
@@ -77,6 +78,7 @@ int kf_step_graph_create(kf_ctx *ctx, int32_t n_layer_steps, const int32_t *laye
     g->exec = nullptr;
     g->n = n_layer_steps;
     g->host_io = host_io ? 1 : 0;
+    g->zero_copy = false;
     g->layers.assign(layers, layers + n_layer_steps);
     g->q.assign(q, q + n_layer_steps);
     g->k.assign(k_new, k_new + n_layer_steps);
@@ -112,8 +114,13 @@ int kf_step_graph_create(kf_ctx *ctx, int32_t n_layer_steps, const int32_t *laye
         e = cudaGraphInstantiate(&g->exec, g->graph, 0);
         if (e != cudaSuccess) rc = cuda_fail(ctx, e);
     }
-    if (rc == KF_OK && !g->host_io) {
-        // kernel order of the capture: plan, n x (append, attend)
+    size_t n_nodes = 0;
+    if (rc == KF_OK && cudaGraphGetNodes(g->graph, nullptr, &n_nodes) != cudaSuccess) n_nodes = 0;
+    // a host-io graph whose layer-steps all took the zero-copy path consists of kernels only: same shape as a
+    // device graph (the staging kernel in place of the append kernel), so it can be re-bound the same way
+    g->zero_copy = g->host_io && n_nodes == (size_t)(2 * n_layer_steps + 1);
+    if (rc == KF_OK && (!g->host_io || g->zero_copy)) {
+        // kernel order of the capture: plan, n x (append or stage, attend)
         std::vector<cudaGraphNode_t> chain;
         if (kernel_chain(g->graph, chain) != 0 || (int)chain.size() != 2 * n_layer_steps + 1) {
             snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "unexpected step-graph topology");
@@ -147,13 +154,33 @@ int kf_step_graph_launch(kf_graph *g, const void *const *q, const void *const *k
     if (!g || !stream) return KF_EINVAL;
     kf_ctx *ctx = g->ctx;
     const bool rebind = q || k_new || v_new || o || lse;
-    if (rebind && (g->host_io || !q || !k_new || !v_new || !o || !lse)) return KF_EINVAL;
+    if (rebind && ((g->host_io && !g->zero_copy) || !q || !k_new || !v_new || !o || !lse)) return KF_EINVAL;
     if (rebind) {
         for (int i = 0; i < g->n; ++i) {
             if (!q[i] || !k_new[i] || !v_new[i] || !o[i] || !lse[i] || ((uintptr_t)q[i] & 15) || ((uintptr_t)k_new[i] & 15) ||
                 ((uintptr_t)v_new[i] & 15) || ((uintptr_t)o[i] & 15))
                 return KF_EINVAL;
-            if (k_new[i] != g->k[i] || v_new[i] != g->v[i]) {
+            if (g->host_io) {
+                // kv_append_stage_kernel(Dev d, int layer, k_new, v_new, q_src, q_dst); the attend node reads stage_q
+                const bool in_changed = q[i] != g->q[i] || k_new[i] != g->k[i] || v_new[i] != g->v[i];
+                const bool out_changed = o[i] != g->o[i] || lse[i] != g->lse[i];
+                if ((in_changed && !(device_can_read(q[i]) && device_can_read(k_new[i]) && device_can_read(v_new[i]))) ||
+                    (out_changed && !(device_can_read(o[i]) && device_can_read(lse[i]))))
+                    return KF_EINVAL;
+                if (in_changed) {
+                    int layer = g->layers[i];
+                    const void *kk = k_new[i], *vv = v_new[i], *qq = q[i];
+                    void *qd = ctx->dev.stage_q;
+                    void *args[6] = {&ctx->dev, &layer, &kk, &vv, &qq, &qd};
+                    cudaKernelNodeParams p = g->append_params[i];
+                    p.kernelParams = args;
+                    p.extra = nullptr;
+                    const cudaError_t e = cudaGraphExecKernelNodeSetParams(g->exec, g->append_nodes[i], &p);
+                    if (e != cudaSuccess) return cuda_fail(ctx, e);
+                    g->k[i] = k_new[i];
+                    g->v[i] = v_new[i];
+                }
+            } else if (k_new[i] != g->k[i] || v_new[i] != g->v[i]) {
                 // kv_append_kernel(Dev d, int layer, const __half *k_new, const __half *v_new)
                 int layer = g->layers[i];
                 const void *kk = k_new[i], *vv = v_new[i];
@@ -166,12 +193,12 @@ int kf_step_graph_launch(kf_graph *g, const void *const *q, const void *const *k
                 g->k[i] = k_new[i];
                 g->v[i] = v_new[i];
             }
-            if (q[i] != g->q[i] || o[i] != g->o[i] || lse[i] != g->lse[i]) {
+            if ((!g->host_io && q[i] != g->q[i]) || o[i] != g->o[i] || lse[i] != g->lse[i]) {
                 // attend_*_kernel(AttendParams p): same struct as kf_attend builds, new q / o / lse
                 AttendParams ap;
                 ap.d = ctx->dev;
                 ap.layer = g->layers[i];
-                ap.q = (const __half *)q[i];
+                ap.q = g->host_io ? ctx->dev.stage_q : (const __half *)q[i];
                 ap.o_part = ctx->dev.range_o;
                 ap.lse_part = ctx->dev.range_lse;
                 ap.o = o[i];
@@ -185,10 +212,10 @@ int kf_step_graph_launch(kf_graph *g, const void *const *q, const void *const *k
                 p.extra = nullptr;
                 const cudaError_t e = cudaGraphExecKernelNodeSetParams(g->exec, g->attend_nodes[i], &p);
                 if (e != cudaSuccess) return cuda_fail(ctx, e);
-                g->q[i] = q[i];
                 g->o[i] = o[i];
                 g->lse[i] = lse[i];
             }
+            g->q[i] = q[i];
         }
     }
     const cudaError_t e = cudaGraphLaunch(g->exec, (cudaStream_t)stream);

@@ -128,16 +128,23 @@ def test_step_graph_host_io_matches_device_path():
     side = torch.cuda.Stream()
     with torch.cuda.stream(side):
         g = kf.step_graph_create([0], [qh], [kh], [vh], [oh], [lh], host_io=True)
-        with pytest.raises(KFlumeError) as ei:       # host-io graphs are bound for life
-            g.launch([qh], [kh], [vh], [oh], [lh])
+        pageable = torch.zeros((B, Hq, 128), dtype=torch.float16)
+        with pytest.raises(KFlumeError) as ei:       # host pointers must be pinned: the kernels read them directly
+            g.launch([pageable], [kh], [vh], [oh], [lh])
         assert ei.value.code == KF_EINVAL
+        oh2, lh2 = torch.zeros_like(oh).pin_memory(), torch.zeros_like(lh).pin_memory()
         for t in range(steps):
             q, (kn, vn) = ses.q_for(0, t), ses.kv_new_for(0, t)
             side.synchronize()
-            qh.copy_(q.cpu()), kh.copy_(kn.cpu()), vh.copy_(vn.cpu())
-            g.launch()
+            if t % 2 == 0:           # rewrite the bound buffers ...
+                qh.copy_(q.cpu()), kh.copy_(kn.cpu()), vh.copy_(vn.cpu())
+                g.launch([qh], [kh], [vh], [oh], [lh])
+                out = (oh, lh)
+            else:                    # ... or re-bind to this step's own pinned buffers
+                g.launch([q.cpu().pin_memory()], [kn.cpu().pin_memory()], [vn.cpu().pin_memory()], [oh2], [lh2])
+                out = (oh2, lh2)
             side.synchronize()
-            _check_step(ses, wl, 0, t, oh.numpy(), lh.numpy(), "graph_host")
+            _check_step(ses, wl, 0, t, out[0].numpy(), out[1].numpy(), "graph_host")
         assert kf.status() == KF_OK
         g.destroy()
     ses.close()
