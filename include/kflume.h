@@ -87,6 +87,8 @@ typedef struct kf_config {
                                      * (0 => 128; 1 => every step); in between, tail ranges grow inside the kept plan */
     int32_t kv_l2_policy;           /* L2 policy of the K/V tile loads: 0 => default (1); 1 = evict-first (K/V is read once
                                      * per launch; keeps q, partials and the plan resident: +1..5% measured); 2 = normal */
+    int32_t diagnostics;            /* non-zero: the attend kernel records per-worker timestamps (kf_worker_times);
+                                     * 0 (default): it reads no timer and writes nothing beyond the method's outputs */
 } kf_config;
 
 typedef struct kf_ctx kf_ctx;
@@ -135,7 +137,12 @@ int kf_close_request(kf_ctx *ctx, int32_t req, kf_stream stream);
  *   order (kf_token_boundary, kf_open_request); existing routes never change, partitions that leave the set keep
  *   serving the ranges they hold.  Allocation order: the first active partition after the one used last, cyclically
  *   (with all P active: the k-th range ever allocated goes to partition k mod P).  All partitions start active.
- *   This call IS the critical-path "route install" (paper: 7.2 us on the CPU): one tiny kernel.
+ *   This call is the critical-path "route install" (paper: 7.2 us on the CPU): one tiny kernel.
+ *   DEVIATION from Algorithm 1 l.16-17 / PAPER.md:240 ("redirect active tails on i to prewarm[i]" at the next token
+ *   boundary): with fixed-size ranges (reading 20) a tail keeps appending to the node that holds its
+ *   current range until that range is full -- up to R tokens per tail -- and only then moves to a node of the new
+ *   active set.  A node that left the set can therefore still grow by (its tails) * R tokens: C_thresh may be
+ *   overshot by n_i * R * bytes_per_token, and kf_policy_step keeps reporting want_publish for it meanwhile.
  * kf_partition_state -- occupancy that the policy monitors (Algorithm 1, l.6-9): [host] active[P] (0/1),
  *   tokens[P] = committed tokens resident on each partition (x 2*H_kv*d*2 B*L = KV bytes),
  *   tails[P] = open requests whose tail range lives there.  Any pointer may be NULL.  Synchronises `stream`. */
@@ -157,10 +164,14 @@ int kf_load_context(kf_ctx *ctx, int32_t layer, int32_t req, int32_t tok_begin, 
 
 /* ---- the decode step -----------------------------------------------------------------------------
  * (a1) kf_token_boundary -- route update at the token boundary (Fig. 5 at :173).
- *   For every open request, ascending, whose tail range is full (len % R == 0 and no range len/R yet):
- *   allocate (partition, slot) as above and APPEND the route entry; earlier entries never change.  Then
- *   rebuilds the device-side work plan for a step over len+1 tokens.  Call once per decode step, before
- *   the per-layer calls.  Device errors: ENOSPC. */
+ *   For every open, active request, ascending, whose tail position len has no route (its tail range is full:
+ *   len % R == 0 -- or an earlier boundary found no slot for it): allocate (partition, slot) as above and APPEND the
+ *   route entry; earlier entries never change.  Then rebuilds the device-side work plan for a step over len+1
+ *   tokens (or keeps it, plan_refresh_steps).  Call once per decode step, before the per-layer calls.
+ *   Device errors: ENOSPC (no active partition has a free slot, or Jmax reached).  Such a request WAITS: kf_kv_append
+ *   drops its row (ESTATE), the attend calls produce its output over the len committed tokens only, kf_step_commit
+ *   does not advance it, and every later kf_token_boundary re-tries -- so it resumes at the same position once
+ *   kf_close_request frees a slot or kf_set_active_partitions adds a node (reading 24). */
 int kf_token_boundary(kf_ctx *ctx, kf_stream stream);
 
 /* (a2) kf_kv_append -- the tail node appends (K_new, V_new).
@@ -192,7 +203,8 @@ int kf_merge_partials(kf_ctx *ctx, const float *o_part, const float *lse_part, f
 int kf_attend(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, float *o_part, float *lse_part,
               kf_stream stream);
 
-/* (a5) kf_step_commit -- len_r += 1 for every open request (the step boundary). */
+/* (a5) kf_step_commit -- len_r += 1 for every open, active request whose tail position had a route in this step
+ *   (the step boundary; a request waiting for a slot stays where it is, see kf_token_boundary). */
 int kf_step_commit(kf_ctx *ctx, kf_stream stream);
 
 /* One layer-step with HOST buffers (end-to-end path): q / k_new / v_new [host, fp16, shapes as above] in,
@@ -232,26 +244,17 @@ int kf_step_graph_launch(kf_graph *graph, const void *const *q, const void *cons
                          float *const *o, float *const *lse, kf_stream stream);
 int kf_step_graph_destroy(kf_graph *graph);
 
-/* ---- inspection (tests, tools) -------------------------------------------------------------------
+/* ---- inspection (tests) ---------------------------------------------------------------------------
  * kf_route_snapshot: downloads the routing state into [host] arrays (any may be NULL):
  *   len[B] (-1 = closed), n_ranges[B], part[B][Jmax], slot[B][Jmax] (-1 where unused), free_head[P],
  *   rr_cursor[1].  Synchronises `stream`.
  * kf_status: synchronises `stream`, returns the device error word (KF_OK or the FIRST latched KF_E*) and
  *   clears it.
- * kf_plan_info: downloads the work-plan header into out[8] [host]: {n_units, n_tiles, n_workers_active,
- *   n_pieces, n_range_entries, tile_tokens, max_workers, n_levels}.  Synchronises `stream`.  Like kf_attend it first
- *   rebuilds the plan if a kf_step_commit happened since the last kf_token_boundary (device error ESTATE if the new
- *   tail position has no route yet): call it between kf_token_boundary and kf_step_commit.
  * kf_launch_count: number of CUDA kernels this ctx has launched so far (host-side counter). */
 int kf_route_snapshot(kf_ctx *ctx, int32_t *len, int32_t *n_ranges, int32_t *part, int32_t *slot,
                       int32_t *free_head, int32_t *rr_cursor, kf_stream stream);
 int kf_status(kf_ctx *ctx, kf_stream stream);
-int kf_plan_info(kf_ctx *ctx, int32_t *out, kf_stream stream);
 int64_t kf_launch_count(const kf_ctx *ctx);
-/* kf_worker_times (diagnostics): per-worker timestamps of the LAST attend launch, out[max_workers][4] [host] =
- *   {SM id | (time spent streaming chunks, ns) << 8, t_start, t_first_tile_ready (0: took no chunk), t_end} in
- *   globaltimer nanoseconds; *n_workers = max_workers.  Synchronises `stream`. */
-int kf_worker_times(kf_ctx *ctx, int64_t *out, int32_t *n_workers, kf_stream stream);
 
 /* ---- Algorithm 1: the A-node scaling policy, host-side controller ----------------------------
  * Pure host arithmetic (double), no GPU work.  Feed it kf_partition_state(); act on it with
@@ -264,6 +267,8 @@ int kf_worker_times(kf_ctx *ctx, int64_t *out, int32_t *n_workers, kf_stream str
  *        tau_fill = (C_thresh - b_i) / g_i                                   (Eq. 2; +inf for nodes without tails)
  *        want_prewarm = tau_fill * T_step < T_prewarm and no prewarm pending or ready for i
  *        want_publish = b_i >= gamma * C_thresh and the prewarm for i is ready
+ *      (want_publish stays asserted for a node that has already left the active set while its tails drain their
+ *      current ranges: see the deviation note at kf_set_active_partitions)
  *      tokens, tails: [host] [P] as kf_partition_state returns them; prewarm_pending / prewarm_ready: [host] uint8[P]
  *      kept by the caller (a prewarm is the background bring-up of a fresh node); out: [host] [P]. */
 typedef struct kf_policy_config {
@@ -284,11 +289,22 @@ int64_t kf_policy_initial_nodes(const kf_policy_config *cfg, const int64_t *s, i
 int kf_policy_step(const kf_policy_config *cfg, int32_t n_partitions, const int64_t *tokens, const int32_t *tails,
                    const uint8_t *prewarm_pending, const uint8_t *prewarm_ready, kf_policy_decision *out);
 
-/* kf_probe_read (measurement aid): streams all P KV pools of the ctx once, in one launch, with plain 128-bit loads on
- * a persistent grid and discards the data -- the read-only HBM bandwidth this box delivers to a trivial kernel, the
- * third roofline denominator next to the nominal 8 TB/s and the measured copy bandwidth.
- * sink: [device] 4 bytes, scratch.  *bytes_read [host, may be NULL] = P * kf_pool_bytes().  Asynchronous on `stream`;
- * time it with events.  Not counted in kf_launch_count. */
+/* ---- diagnostics (not part of the method; nothing here runs on the hot path) -------------------------------------
+ * kf_plan_info: downloads the work-plan header into out[8] [host]: {n_units, n_tiles, n_workers_active,
+ *   n_pieces, n_range_entries, tile_tokens, max_workers, n_levels}.  Synchronises `stream`.  Like kf_attend it first
+ *   rebuilds the plan if a kf_step_commit happened since the last kf_token_boundary (device error ESTATE if the new
+ *   tail position has no route yet): call it between kf_token_boundary and kf_step_commit.
+ * kf_worker_times: per-worker timestamps of the LAST attend launch, out[max_workers][4] [host] =
+ *   {SM id | (time spent streaming chunks, ns) << 8, t_start, t_first_tile_ready (0: took no chunk), t_end} in
+ *   globaltimer nanoseconds; *n_workers = max_workers.  Synchronises `stream`.  KF_ESTATE unless the ctx was created
+ *   with kf_config.diagnostics != 0 (only then does the attend kernel read the timer and write these words).
+ * kf_probe_read (measurement aid): streams all P KV pools of the ctx once, in one launch, with plain 128-bit loads on
+ *   a persistent grid and discards the data -- the read-only HBM bandwidth this box delivers to a trivial kernel, the
+ *   third roofline denominator next to the nominal 8 TB/s and the measured copy bandwidth.
+ *   sink: [device] 4 bytes, scratch.  *bytes_read [host, may be NULL] = P * kf_pool_bytes().  Asynchronous on `stream`;
+ *   time it with events.  Not counted in kf_launch_count. */
+int kf_plan_info(kf_ctx *ctx, int32_t *out, kf_stream stream);
+int kf_worker_times(kf_ctx *ctx, int64_t *out, int32_t *n_workers, kf_stream stream);
 int kf_probe_read(kf_ctx *ctx, void *sink, size_t *bytes_read, kf_stream stream);
 
 #ifdef __cplusplus

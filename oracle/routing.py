@@ -14,7 +14,12 @@ attending).  Where the paper is silent the readings of DESIGN.md apply:
              the new A node, while existing KV ranges remain in place", :240) the next range goes to the
              first active partition after the one used last, cyclically -- which is k % P when all are active;
              slot = per-partition LIFO free list if non-empty, else bump allocator free_head[p]++
-  reading 10: exhaustion (slot >= slots_per_partition, or range index >= max_ranges) -> error ENOSPC
+  reading 10: exhaustion (no free slot, or range index >= max_ranges) -> error ENOSPC
+  reading 24: a FULL partition is passed over by the round-robin (ENOSPC only when no active partition has a free
+             slot); a request whose boundary failed has no route for its tail position: it appends nothing, is NOT
+             advanced by the step commit, and every later boundary re-tries the allocation at the same position --
+             the paper's "existing KV ranges remain in place ... future appends use the new A node" (:240) then
+             holds again as soon as a slot is freed or a node is activated
 
 Pure Python, no numpy: written to be checked against the text by eye.
 """
@@ -49,19 +54,14 @@ class RoutingModel:
         if len(self.route[req]) >= self.Jmax:
             raise RoutingError("ENOSPC: max_ranges_per_request")
         p = None
-        for i in range(1, self.P + 1):                      # first active partition after the last one used
+        for i in range(1, self.P + 1):       # first active partition WITH A FREE SLOT after the last one used
             c = (self.rr_last + i) % self.P
-            if self.active[c]:
+            if self.active[c] and (self.free_list[c] or self.free_head[c] < self.slots):
                 p = c
                 break
         if p is None:
-            raise RoutingError("ENOSPC: no active partition")
-        if self.free_list[p]:
-            slot = self.free_list[p][-1]
-        else:
-            slot = self.free_head[p]
-            if slot >= self.slots:
-                raise RoutingError("ENOSPC: partition full")
+            raise RoutingError("ENOSPC: no active partition with a free slot")
+        slot = self.free_list[p][-1] if self.free_list[p] else self.free_head[p]
         # commit
         self.rr_cursor += 1
         self.rr_last = p
@@ -84,15 +84,25 @@ class RoutingModel:
             self._alloc(req)
 
     def token_boundary(self) -> List[Tuple[int, int, int, int]]:
-        """Open a new range for every open request whose tail range is full (reading 8).
-        Returns the events [(req, range_index, partition, slot)]."""
-        events = []
+        """Open a new range for every open request whose tail position has no route: its tail range is full
+        (reading 8: len % R == 0), or an earlier boundary found no slot for it (reading 24).
+        Returns the events [(req, range_index, partition, slot)].  Every such request is tried, in ascending order;
+        if any of them found no slot, RoutingError(ENOSPC) is raised AFTER the loop (the device latches an error word
+        and carries on) and ``last_events`` holds the events of the requests that did get a range."""
+        events, failed = [], None
         for r in range(self.B):
             if self.len[r] < 0 or not self.req_active[r]:
                 continue
-            if self.len[r] % self.R == 0 and len(self.route[r]) == self.len[r] // self.R:
-                p, s = self._alloc(r)
+            if len(self.route[r]) * self.R <= self.len[r]:
+                try:
+                    p, s = self._alloc(r)
+                except RoutingError as e:
+                    failed = failed or e
+                    continue
                 events.append((r, len(self.route[r]) - 1, p, s))
+        self.last_events = events
+        if failed is not None:
+            raise failed
         return events
 
     def append_position(self, req: int) -> Tuple[int, int, int]:
@@ -107,8 +117,10 @@ class RoutingModel:
         return p, s, n - j * self.R
 
     def step_commit(self) -> None:
+        """len += 1 for every open, active request whose tail position had a route in this step (reading 24: a
+        request that is waiting for a slot appended nothing and stays where it is)."""
         for r in range(self.B):
-            if self.len[r] >= 0 and self.req_active[r]:
+            if self.len[r] >= 0 and self.req_active[r] and len(self.route[r]) * self.R > self.len[r]:
                 self.len[r] += 1
 
     def close_request(self, req: int) -> None:

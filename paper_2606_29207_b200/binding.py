@@ -34,6 +34,7 @@ class kf_config(ctypes.Structure):
         ("workers_per_sm", ctypes.c_int32), ("pipeline_stages", ctypes.c_int32),
         ("sched_first_pct", ctypes.c_int32), ("sched_decay_pct", ctypes.c_int32),
         ("plan_refresh_steps", ctypes.c_int32), ("kv_l2_policy", ctypes.c_int32),
+        ("diagnostics", ctypes.c_int32),
     ]
 
 
@@ -113,7 +114,7 @@ def load_library():
 def make_config(n_q_heads, n_kv_heads, range_tokens, n_partitions, max_requests, max_ranges_per_request,
                 slots_per_partition, n_layers=1, softmax_scale=0.0, attend_impl=KF_IMPL_AUTO,
                 min_tiles_per_worker=0, head_dim=128, workers_per_sm=0, pipeline_stages=0, sched_first_pct=0,
-                sched_decay_pct=0, plan_refresh_steps=0, kv_l2_policy=0) -> kf_config:
+                sched_decay_pct=0, plan_refresh_steps=0, kv_l2_policy=0, diagnostics=0) -> kf_config:
     c = kf_config()
     c.n_q_heads, c.n_kv_heads, c.head_dim, c.n_layers = n_q_heads, n_kv_heads, head_dim, n_layers
     c.range_tokens, c.n_partitions, c.max_requests = range_tokens, n_partitions, max_requests
@@ -123,6 +124,7 @@ def make_config(n_q_heads, n_kv_heads, range_tokens, n_partitions, max_requests,
     c.sched_first_pct, c.sched_decay_pct = sched_first_pct, sched_decay_pct
     c.plan_refresh_steps = plan_refresh_steps
     c.kv_l2_policy = kv_l2_policy
+    c.diagnostics = diagnostics
     return c
 
 

@@ -69,6 +69,7 @@ bool valid_config(const kf_config *c) {
     if (c->sched_decay_pct < 0 || c->sched_decay_pct > 99) return false;
     if (c->plan_refresh_steps < 0) return false;
     if (c->kv_l2_policy < 0 || c->kv_l2_policy > 2) return false;
+    if (c->diagnostics < 0) return false;
     // rows of one K (or V) half-pool must fit the int32 TMA coordinate
     const double rows = (double)c->n_layers * c->slots_per_partition * c->n_kv_heads * c->range_tokens;
     if (rows >= 2147483647.0) return false;
@@ -194,6 +195,18 @@ int run_attend(kf_ctx *ctx, const AttendParams &ap, cudaStream_t s) {
     return after_launch(ctx, launch_attend_tma(ap, ctx->n_ctas, s));
 }
 
+// device_can_read() with a small per-ctx cache: the pinned buffers of an end-to-end loop are the same few pointers
+// every layer-step, and cudaPointerGetAttributes costs ~1 us each.  (A cached pointer is trusted for the lifetime of
+// the ctx: un-pinning a buffer that is still in use is the caller's error either way.)
+bool host_ptr_ok(kf_ctx *ctx, const void *p) {
+    for (int i = 0; i < kf_ctx::kPinnedCache; ++i)
+        if (ctx->pinned[i] == p) return true;
+    if (!device_can_read(p)) return false;
+    ctx->pinned[ctx->pinned_next] = p;
+    ctx->pinned_next = (ctx->pinned_next + 1) % kf_ctx::kPinnedCache;
+    return true;
+}
+
 bool bad_layer(const kf_ctx *ctx, int layer) { return layer < 0 || layer >= ctx->cfg.n_layers; }
 
 }  // namespace
@@ -291,6 +304,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.stages = cfg->pipeline_stages ? cfg->pipeline_stages : kDefaultStages;
     d.max_chunks = (int32_t)max_chunks_of(cfg);
     d.l2_hint = cfg->kv_l2_policy == 2 ? 0 : 1;  // K/V is read once per launch: evict-first by default
+    d.diag = cfg->diagnostics ? 1 : 0;
     d.plan_refresh = cfg->plan_refresh_steps > 0 ? cfg->plan_refresh_steps : kDefaultPlanRefresh;
     d.sched_first = 0.01f * (cfg->sched_first_pct ? cfg->sched_first_pct : kDefaultFirstPct);
     d.sched_decay = 0.01f * (cfg->sched_decay_pct ? cfg->sched_decay_pct : kDefaultDecayPct);
@@ -465,8 +479,8 @@ int kf_layer_step_host_impl(kf_ctx *ctx, int32_t layer, const void *q_host, cons
     cudaStream_t s = (cudaStream_t)stream;
     const Dev &d = ctx->dev;
     const bool aligned = !(((uintptr_t)q_host | (uintptr_t)k_new_host | (uintptr_t)v_new_host | (uintptr_t)o_host) & 15);
-    if (aligned && device_can_read(q_host) && device_can_read(k_new_host) && device_can_read(v_new_host) &&
-        device_can_read(o_host) && device_can_read(lse_host)) {
+    if (aligned && host_ptr_ok(ctx, q_host) && host_ptr_ok(ctx, k_new_host) && host_ptr_ok(ctx, v_new_host) &&
+        host_ptr_ok(ctx, o_host) && host_ptr_ok(ctx, lse_host)) {
         // zero-copy: the append kernel reads k_new / v_new over the bus and stages q; the attend kernel's merge
         // tail writes o / lse straight into the host buffers.  No copy engine work at all.
         int rc = after_launch(ctx, launch_kv_append_stage(d, layer, (const __half *)k_new_host, (const __half *)v_new_host,
@@ -575,6 +589,7 @@ int64_t kf_launch_count(const kf_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
 int kf_worker_times(kf_ctx *ctx, int64_t *out, int32_t *n_workers, kf_stream stream) {
     if (!ctx || !out || !n_workers) return KF_EINVAL;
+    if (!ctx->dev.diag) return KF_ESTATE;  // the kernel records nothing unless kf_config.diagnostics asked for it
     cudaStream_t s = (cudaStream_t)stream;
     *n_workers = ctx->dev.max_workers;
     cudaError_t e = cudaMemcpyAsync(out, ctx->dev.worker_times, (size_t)ctx->dev.max_workers * 4 * 8,

@@ -26,6 +26,11 @@ constexpr int kSubTile = kTileTokens * 128;     // 16 rows x 128 B (64 halfs): o
 constexpr int kStageBytes = 4 * kSubTile;       // K lo | K hi | V lo | V hi = 8 KB
 constexpr int kTicketAhead = 3;                 // tiles before the end of a chunk at which the next ticket is taken
 constexpr int kRing = 8;                        // chunk descriptors in flight between the load and compute cursors
+// P is rounded to fp16 for the P.V MMA.  With p = exp2(s - m) in (0, 1] every weight below 2^-25 would flush to zero
+// there while the fp32 row sum l keeps it: on a long, peaked context (1M tokens, each 2^-25 below the maximum) that
+// is up to 3% of the mass missing from o but present in l.  So P (and l with it) is carried scaled by 2^kPShift:
+// p' = exp2(s - m + 14) in (0, 16384], flush threshold 2^-39 relative to the maximum; o'/l' = o/l, lse = m + log2(l') - 14.
+constexpr float kPShift = 14.f;
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -126,7 +131,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
     const int W = gridDim.x * WARPS;
     const int w = warp * gridDim.x + blockIdx.x;  // warp-major: the first chunks of a small launch spread over all SMs
     const int n_chunks = __ldg(&d.plan->n_pieces);
-    const long long t_start = global_ns();
+    const long long t_start = d.diag ? global_ns() : 0;
     long long t_first = 0, t_stream = 0;
     const Counters ctr = launch_prologue(d, w, W, lane);
     int m_first = -1;  // lane 0: pre-taken first merge ticket
@@ -259,7 +264,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
             const int stage = consumed % STAGES;
             const uint32_t sb = wbase + stage * kStageBytes;
             mbar_wait(bar0 + 8 * stage, (consumed / STAGES) & 1);
-            if (consumed == 0) t_first = global_ns();
+            if (d.diag && consumed == 0) t_first = global_ns();
 
             const int valid = min(kTileTokens, c_cnt - ct * kTileTokens);
             const bool ragged = valid < kTileTokens;
@@ -303,8 +308,9 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
             mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
             const float m_new = fmaxf(m_run, mx);
             const float alpha = fast_exp2(m_run - m_new);
-            const float p00 = fast_exp2(s[0][0] - m_new), p01 = fast_exp2(s[0][1] - m_new);
-            const float p10 = fast_exp2(s[1][0] - m_new), p11 = fast_exp2(s[1][1] - m_new);
+            const float m_off = m_new - kPShift;
+            const float p00 = fast_exp2(s[0][0] - m_off), p01 = fast_exp2(s[0][1] - m_off);
+            const float p10 = fast_exp2(s[1][0] - m_off), p11 = fast_exp2(s[1][1] - m_off);
             l_run = l_run * alpha + ((p00 + p01) + (p10 + p11));
             m_run = m_new;
             if (__any_sync(0xffffffffu, alpha != 1.f)) {
@@ -326,8 +332,10 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
                 mma16816(o[nd + 1], pa0, pa2, b2, b3);
             }
 
+            // the zero-stores above went through the generic proxy: every lane that wrote orders them before the
+            // async-proxy (TMA) refill of this stage, then the barrier, then the elected lane issues
+            if (ragged) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncwarp();  // every lane is done reading this stage
-            if (ragged && lane == 0) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             try_issue();   // refills this very stage: issued == consumed + STAGES whenever it issues
 
             ++consumed;
@@ -345,7 +353,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
 #pragma unroll
                     for (int n = 0; n < 16; ++n)
                         *reinterpret_cast<float2 *>(dst + 8 * n) = make_float2(o[n][0] * inv, o[n][1] * inv);
-                    const float lse = (m_run + log2f(lt)) * 0.6931471805599453f;
+                    const float lse = (m_run + log2f(lt) - kPShift) * 0.6931471805599453f;
                     if ((lane & 3) == 0) pd.lse[qrow] = lse;
                     if (pd.o2) {
                         float *dst2 = pd.o2 + (size_t)qrow * kHeadDim + qcol;
@@ -358,11 +366,11 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
                 if (p.fused) piece_done(p, ctr, cu, cun, g, lane);
             }
         }
-        t_stream = global_ns();
+        if (d.diag) t_stream = global_ns();
     }
     if (p.fused) merge_phase(p, ctr, W, lane, m_first);
 
-    if (lane == 0) {
+    if (d.diag && lane == 0) {
         // diagnostics: {SM | stream-end offset << 8, start, first tile ready (0 = no chunk), end}
         d.worker_times[4 * w] = sm_id() | ((w < n_chunks ? t_stream - t_start : 0) << 8);
         d.worker_times[4 * w + 1] = t_start;

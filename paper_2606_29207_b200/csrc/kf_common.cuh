@@ -62,6 +62,7 @@ struct Dev {
     int32_t max_workers, min_tiles;
     int32_t warps_per_cta, stages;      // launch shape of the attend kernels
     int32_t l2_hint;                    // 1: K/V tiles are loaded with an L2 evict-first policy
+    int32_t diag;                       // 1: the attend kernel records per-worker timestamps (worker_times)
     int32_t max_chunks;                 // capacity of chunks[] and of the piece buffers
     int32_t plan_refresh;               // a plan is rebuilt after this many token boundaries (or when routes change)
     float sched_first, sched_decay;     // GSS factor rho (chunk <= rho * remaining / workers); share of a unit's remaining tiles per level
@@ -133,6 +134,14 @@ __device__ __forceinline__ int live_tiles(const Unit &un, int cnt_live, int tile
     const int planned = (un.cnt + kTileTokens - 1) / kTileTokens;
     return (un.tail && tile_begin + n_tiles == planned) ? (cnt_live + kTileTokens - 1) / kTileTokens - tile_begin
                                                         : n_tiles;
+}
+
+// (a5) does request r advance at the step commit?  Open, taking part in the step, and its tail position had a route:
+// a request whose boundary could not get a slot (ENOSPC) appended nothing, so it must not move on -- the next
+// kf_token_boundary re-tries the allocation at the same position (reading 24).
+__device__ __forceinline__ bool commits(const Dev &d, int r) {
+    const int len = d.len[r];
+    return len >= 0 && d.req_active[r] && (long long)d.n_ranges[r] * d.R > len;
 }
 
 // byte offset (within a partition pool) of K row (layer, slot, g, t)

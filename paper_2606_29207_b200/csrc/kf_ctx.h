@@ -11,6 +11,9 @@ struct kf_ctx {
     bool plan_dirty;  // lengths moved (step commit) or routes were edited since the plan kernel last ran
     int64_t launches;
     char cuda_err[256];
+    static constexpr int kPinnedCache = 16;
+    const void *pinned[kPinnedCache];  // host pointers already verified as device-readable (kf_layer_step_host)
+    int pinned_next;
 };
 
 // library-internal entry points of the static step graph (kf_graph.cu); not exported through include/kflume.h:

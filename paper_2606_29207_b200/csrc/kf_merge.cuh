@@ -192,6 +192,7 @@ __device__ __forceinline__ Counters launch_prologue(const Dev &d, int w, int W, 
 // launch reads any more: each of them read len before its own release below
 __device__ __forceinline__ void launch_epilogue(const Dev &d, int W, int lane, int commit = 0) {
     int last = 0;
+    __syncwarp();  // the other lanes' stores (merge outputs) and loads (len) are ordered before lane 0's release
     if (lane == 0) {
         release_fence();
         const int old = atomicAdd(d.sched + 1, 1);
@@ -209,7 +210,7 @@ __device__ __forceinline__ void launch_epilogue(const Dev &d, int W, int lane, i
         if (last) {
             asm volatile("fence.acq_rel.gpu;" ::: "memory");  // acquire side: every worker's reads of len are done
             for (int r = lane; r < d.B; r += 32)
-                if (d.len[r] >= 0 && d.req_active[r]) d.len[r] += 1;
+                if (commits(d, r)) d.len[r] += 1;
         }
     }
 }
@@ -218,9 +219,11 @@ __device__ __forceinline__ void launch_epilogue(const Dev &d, int W, int lane, i
 __device__ __forceinline__ void piece_done(const AttendParams &p, const Counters &c, int u, const Unit &un, int g,
                                            int lane) {
     const Dev &d = p.d;
-    release_fence();
+    // release: barrier first, THEN lane 0 fences and publishes -- the fence is cumulative over the stores of the
+    // other lanes that the barrier ordered before it (a fence in every lane before the barrier would not cover them)
     __syncwarp();
     if (lane == 0) {
+        release_fence();
         if (un.n_pieces > 1)
             atomicAdd(&c.unit[u], 1);
         else if (d.scratch[un.req] > 1)
@@ -278,9 +281,11 @@ __device__ __forceinline__ void merge_phase(const AttendParams &p, const Counter
                 wait_counter(&c.unit[u], un.n_pieces, lane);
                 merge_unit_head(p, un, g, i, true, lane);
                 if (d.scratch[un.req] > 1) {
-                    release_fence();
                     __syncwarp();
-                    if (lane == 0) atomicAdd(&c.group[un.req * Hkv + g], 1);
+                    if (lane == 0) {
+                        release_fence();
+                        atomicAdd(&c.group[un.req * Hkv + g], 1);
+                    }
                 }
             } else {
                 const int tb = t - nA;

@@ -16,13 +16,15 @@ __device__ bool alloc_range(const Dev &d, int req) {
         return false;
     }
     // round-robin over the ACTIVE partitions: the first active one after the partition used last, cyclically
-    // (with every partition active this is "the k-th range ever allocated goes to partition k mod P")
+    // (with every partition active this is "the k-th range ever allocated goes to partition k mod P").  A full
+    // partition is passed over (reading 24): ENOSPC is latched only when NO active partition has a free
+    // slot -- e.g. after a scale-down left fewer nodes than the pools were sized for.
     const int k = *d.rr_cursor;
     const int last = *d.rr_last;
     int p = -1;
     for (int i = 1; i <= d.P; ++i) {
         const int c = (last + i) % d.P;
-        if (d.active[c]) {
+        if (d.active[c] && (d.free_cnt[c] > 0 || d.free_head[c] < d.slots)) {
             p = c;
             break;
         }
@@ -32,16 +34,7 @@ __device__ bool alloc_range(const Dev &d, int req) {
         return false;
     }
     const int nfree = d.free_cnt[p];
-    int slot;
-    if (nfree > 0) {
-        slot = d.free_stack[(size_t)p * d.slots + nfree - 1];
-    } else {
-        slot = d.free_head[p];
-        if (slot >= d.slots) {
-            set_error(d, KF_ENOSPC);
-            return false;
-        }
-    }
+    const int slot = nfree > 0 ? d.free_stack[(size_t)p * d.slots + nfree - 1] : d.free_head[p];
     *d.rr_cursor = k + 1;
     *d.rr_last = p;
     if (nfree > 0)
@@ -97,7 +90,9 @@ __device__ int token_boundary_warp(const Dev &d, int lane) {
         bool need = false;
         if (r < d.B) {
             const int len = d.len[r];
-            need = len >= 0 && d.req_active[r] && (len % d.R) == 0 && d.n_ranges[r] == len / d.R;
+            // the tail position has no route yet: the tail range is full (len % R == 0) -- or an earlier boundary
+            // could not get a slot for it (ENOSPC) and the request has been waiting since (reading 24)
+            need = len >= 0 && d.req_active[r] && (long long)d.n_ranges[r] * d.R <= len;
         }
         unsigned m = __ballot_sync(0xffffffffu, need);
         opened += __popc(m);
@@ -145,7 +140,7 @@ __global__ void partition_state_kernel(Dev d, long long *tokens, int *tails) {
 
 __global__ void step_commit_kernel(Dev d) {
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
-    if (r < d.B && d.len[r] >= 0 && d.req_active[r]) d.len[r] += 1;
+    if (r < d.B && commits(d, r)) d.len[r] += 1;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -135,6 +135,60 @@ def test_enospc():
         m2.token_boundary()
 
 
+def test_full_partition_is_passed_over():
+    # reading 24, worked by hand: P = 2, 2 slots each, R = 4.  Only node 0 is active while request 0 loads 8 tokens:
+    # both of its ranges land on node 0 -> (0,0),(0,1): node 0 is full.  Node 1 joins.  Request 1 (4 tokens): the
+    # first active node after node 0 is node 1 -> (1,0).  Request 2 (4 tokens): the round-robin would return to node 0,
+    # which has no free slot, so it is passed over -> (1,1).  Now everything is full: ENOSPC.
+    m = RoutingModel(2, 4, 4, 4, 2)
+    m.set_active([1, 0])
+    m.open_request(0, 8)
+    assert m.route[0] == [(0, 0), (0, 1)]
+    m.set_active([1, 1])
+    m.open_request(1, 4)
+    assert m.route[1] == [(1, 0)]
+    m.open_request(2, 4)
+    assert m.route[2] == [(1, 1)]
+    assert m.free_head == [2, 2] and m.rr_cursor == 4
+    with pytest.raises(RoutingError):
+        m.open_request(3, 1)
+
+
+def test_request_waits_for_a_slot_and_resumes():
+    # reading 24, worked by hand: P = 1, 3 slots, R = 4.  r0 holds 4 tokens in slot 0, r1 holds 8 in slots 1, 2.
+    # Boundary: both tail ranges are full and no slot is left -> ENOSPC, nobody gets a range; the commit leaves both
+    # where they are (nothing was appended).  r1 is closed: slots 1 then 2 go on the LIFO list.  Next boundary: r0 takes
+    # slot 2 (top of the list), appends at offset 0 of it, commits to 5.  r2 opens with 1 token -> slot 1.
+    m = RoutingModel(1, 4, 3, 4, 3)
+    m.open_request(0, 4)
+    m.open_request(1, 8)
+    assert m.route == [[(0, 0)], [(0, 1), (0, 2)], []]
+    for _ in range(2):                       # waiting does not move anything, however often it is re-tried
+        with pytest.raises(RoutingError):
+            m.token_boundary()
+        assert m.last_events == []
+        with pytest.raises(RoutingError):
+            m.append_position(0)
+        m.step_commit()
+        assert m.len == [4, 8, -1] and m.rr_cursor == 3
+    m.close_request(1)
+    assert m.token_boundary() == [(0, 1, 0, 2)]
+    assert m.append_position(0) == (0, 2, 0)
+    m.step_commit()
+    assert m.len == [5, -1, -1]
+    m.open_request(2, 1)
+    assert m.route[2] == [(0, 1)]
+    # a boundary where one request finds a slot and a later one does not: the first still gets its range
+    m2 = RoutingModel(1, 2, 2, 4, 3)
+    m2.open_request(0, 2)
+    m2.open_request(1, 2)                    # slots 0, 1 used, one left
+    with pytest.raises(RoutingError):
+        m2.token_boundary()
+    assert m2.last_events == [(0, 1, 0, 2)] and m2.route[1] == [(0, 1)]
+    m2.step_commit()
+    assert m2.len == [3, 2]
+
+
 def test_kv_byte_formula():
     # PAPER.md:234 C_total = sum_i 2*s_i*H_kv*d_h*L*2B; PAPER.md:35 sanity: Llama-3.1-8B, batch 64 x 4K
     # tokens = 32 GiB (128 KiB/token over 32 layers)
