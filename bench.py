@@ -3,12 +3,16 @@
 
 A "step" is one pass of the whole hot path over one batch of synthetic input:
     kf_token_boundary -> per layer { kf_kv_append -> kf_attend (split-KV attention + fused LSE merge) } -> kf_step_commit
-so the contexts grow by one token per step exactly as in decoding.  Default workload: cfg3 (configs[2] of
+so the contexts grow by one token per step exactly as in decoding.  Headline workload: cfg3 (configs[2] of
 BASELINE.json: B=16, Llama-3.1-8B shape, log-normal contexts with median 80K, 32K ranges over 8 partitions) -- the
 configuration the north_star target ">= 80% of peak HBM bandwidth at >= 32K context" is quoted on and the stand-in for
-the paper's serving trace.  `--workload cfg1|cfg2|cfg4|cfg5` selects the others.
+the paper's serving trace.  The same process then measures the other BASELINE configs (cfg1, cfg2, cfg4, cfg5) and
+reports them as sub-records under "workloads" of the ONE JSON line (`--only` skips them; `--workload X` makes X the
+headline).  For the single-layer configs a second, STATIC protocol (load S-1 tokens, boundary, append,
+then repeat append + attend WITHOUT committing, so every repetition sees exactly the stated context) is reported
+beside the growing-context loop.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--only] [--impl ours|reference]
 
 N > 1 (torchrun): every rank runs an independent batch of the same recipe (seed + rank): the path shards over
 independent requests with no data-path collective -> "scaling": "weak"; NCCL is used only for the barrier and the
@@ -17,6 +21,8 @@ max-over-ranks of the device time.
 from __future__ import annotations
 
 import argparse
+import gc
+import hashlib
 import json
 import os
 import subprocess
@@ -31,11 +37,43 @@ METRIC = "decode_core_attention_hbm_gbps"
 UNIT = "GB/s"
 NOMINAL_PEAK_GBS = 8000.0        # BASELINE.json's "~8 TB/s" denominator (context)
 FALLBACK_PEAK_GBS = 6650.0       # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+SUB_WORKLOADS = ["cfg1", "cfg2", "cfg4", "cfg5"]
+# steps / warm-up / end-to-end steps of the sub-records (the headline takes --steps / --warmup)
+SUB_STEPS = {"cfg1": (200, 10, 50), "cfg2": (100, 10, 50), "cfg3": (100, 10, 40), "cfg4": (60, 6, 30),
+             "cfg5": (8, 3, 3)}
 
-# dram__bytes_read.sum + dram__bytes_write.sum per kf_attend launch from the committed `ncu --set full` capture
-# (profiles/r01g_attend_full_<workload>.md); None where no capture exists for that workload.
-NCU_TRAFFIC_BYTES = {"cfg1": 16939392, "cfg2": 1085991552, "cfg3": 4782093992, "cfg4": 4307839832,
-                     "cfg5": 37122728208}
+# dram__bytes_read.sum + dram__bytes_write.sum per kf_attend launch from the committed `ncu --set full` captures.
+# A capture is only valid for the kernel sources it was taken from: `rev` is kernel_rev() at capture time, and the
+# line carries `traffic` only when the running sources hash to the same value and no tuning flag is set.
+NCU_TRAFFIC = {
+    # workload: (bytes per launch, committed summary, kernel_rev at capture time)
+    "cfg1": (16939392, "profiles/r01g_attend_full_cfg1.md", "r01"),
+    "cfg2": (1085991552, "profiles/r01g_attend_full_cfg2.md", "r01"),
+    "cfg3": (4782093992, "profiles/r01g_attend_full_cfg3.md", "r01"),
+    "cfg4": (4307839832, "profiles/r01g_attend_full_cfg4.md", "r01"),
+    "cfg5": (37122728208, "profiles/r01g_attend_full_cfg5.md", "r01"),
+}
+
+
+def kernel_rev():
+    """Short hash of the sources of the dominant kernel: ties an ncu capture to the code it was taken from."""
+    h = hashlib.sha256()
+    for f in ("kf_attend_tma.cu", "kf_merge.cuh", "kf_common.cuh"):
+        with open(os.path.join(ROOT, "paper_2606_29207_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:12]
+
+
+def traffic_record(wl_name, args):
+    cap = NCU_TRAFFIC.get(wl_name)
+    if cap is None:
+        return None, "no committed ncu capture for this workload"
+    nbytes, src, rev = cap
+    if args.attend_impl == 1 or args.min_tiles or args.kv_l2_policy or args.no_graph:
+        return None, f"{src}: not applicable (non-default --attend-impl / --min-tiles / --kv-l2-policy / --no-graph)"
+    if rev != kernel_rev():
+        return None, f"{src}: stale (captured at kernel_rev {rev}, running {kernel_rev()})"
+    return nbytes, f"{src} (ncu --set full, committed; kernel_rev {rev})"
 
 
 def load_peak():
@@ -115,81 +153,95 @@ class ClockSampler:
 
 
 # ---------------------------------------------------------------------------------------------------------
-def cpu_baseline_sample(wl, lens_before, step, budget_s=15.0):
-    """Time the fp64 oracle (as it stands) on the host cores, on a bounded sample of the same workload:
-    the shortest requests of the batch, all query heads, until ~budget_s of CPU work (estimated from a probe)."""
+# The CPU oracle, timed as it stands on a bounded sample of the workload.  Shared by the `cpu_baseline` leg of our
+# arm and by `--impl reference`, so both time THE SAME sample (the only places bench.py may execute oracle/).
+def _host_kv(wl, r, n, have_gpu):
     import numpy as np
+    from kf_inputs import gen
+    if have_gpu:
+        from kf_inputs import gen_device
+        K = gen_device.fill(gen.STREAM_K, 0, r, 0, n, wl.n_kv_heads, seed=wl.seed).cpu().numpy()
+        V = gen_device.fill(gen.STREAM_V, 0, r, 0, n, wl.n_kv_heads, seed=wl.seed).cpu().numpy()
+        return K, V
+    pos = np.arange(n)
+    return gen.gen_k(0, r, pos, wl.n_kv_heads, wl.seed), gen.gen_v(0, r, pos, wl.n_kv_heads, wl.seed)
+
+
+def oracle_sample(wl, lens_before, budget_s, have_gpu):
+    """Pick the sample: the shortest requests of the batch (all query heads, layer 0) until ~budget_s of oracle work,
+    estimated from a 2048-token probe; a single request that is too long is cut to a prefix.  Returns
+    ([(request, n_tokens)], host K/V per entry, description)."""
     import oracle
-    from kf_inputs import gen, gen_device
+    from kf_inputs import gen
     order = sorted(range(wl.batch), key=lambda r: lens_before[r])
-    # probe: one request-slice of 2048 tokens
     r0 = order[0]
     n0 = min(2048, lens_before[r0] + 1)
-    K = gen_device.fill(gen.STREAM_K, 0, r0, 0, n0, wl.n_kv_heads, seed=wl.seed).cpu().numpy()
-    V = gen_device.fill(gen.STREAM_V, 0, r0, 0, n0, wl.n_kv_heads, seed=wl.seed).cpu().numpy()
-    q = gen.gen_q(0, r0, step, wl.n_q_heads, wl.seed)
+    K, V = _host_kv(wl, r0, n0, have_gpu)
+    q = gen.gen_q(0, r0, 0, wl.n_q_heads, wl.seed)
     t = time.perf_counter()
     oracle.attend(q, K, V)
-    rate = n0 / max(time.perf_counter() - t, 1e-6)          # tokens/s (all heads)
+    rate = n0 / max(time.perf_counter() - t, 1e-6)          # context tokens / s (all heads)
+    if not have_gpu:                                         # numpy generates ~2M elements/s: keep the sample small
+        budget_s = min(budget_s, 65536 / rate)
     chosen, tok = [], 0
     for r in order:
         n = lens_before[r] + 1
         if chosen and (tok + n) / rate > budget_s:
             break
-        chosen.append(r)
+        chosen.append((r, n))
         tok += n
-    if tok / rate > 2 * budget_s:                              # a single huge request: take a prefix of its tokens
-        tok = int(rate * budget_s)
-        chosen = [(chosen[0], tok)]
-    else:
-        chosen = [(r, lens_before[r] + 1) for r in chosen]
-    data = []
-    for r, n in chosen:
-        K = gen_device.fill(gen.STREAM_K, 0, r, 0, n, wl.n_kv_heads, seed=wl.seed).cpu().numpy()
-        V = gen_device.fill(gen.STREAM_V, 0, r, 0, n, wl.n_kv_heads, seed=wl.seed).cpu().numpy()
-        data.append((gen.gen_q(0, r, step, wl.n_q_heads, wl.seed), K, V))
+    if tok / rate > 2 * budget_s:                            # a single huge request: a prefix of its tokens
+        chosen = [(chosen[0][0], max(256, int(rate * budget_s)))]
+    data = [_host_kv(wl, r, n, have_gpu) for r, n in chosen]
+    full = all(n == lens_before[r] + 1 for r, n in chosen)
+    desc = (f"{wl.name} layer 0: requests {[r for r, _ in chosen]} "
+            f"({sum(n for _, n in chosen)} context tokens{'' if full else ', PREFIX of the request'}, "
+            f"all {wl.n_q_heads} query heads), oracle.attend fp64")
+    return chosen, data, desc
+
+
+def oracle_run(wl, chosen, data, step):
+    """One timed pass of the oracle over the sample.  Returns (seconds, {request: (o*, lse*)})."""
+    import oracle
+    from kf_inputs import gen
+    qs = [gen.gen_q(0, r, step, wl.n_q_heads, wl.seed) for r, _ in chosen]
+    out = {}
     t = time.perf_counter()
-    for q, K, V in data:
-        oracle.attend(q, K, V)
-    dt = time.perf_counter() - t
-    nbytes = sum(n for _, n in chosen) * wl.kv_bytes_per_token()
-    return {"value": nbytes / dt / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"{wl.name} layer 0 step {step}: requests {[r for r, _ in chosen]} "
-                      f"({sum(n for _, n in chosen)} context tokens, all {wl.n_q_heads} query heads), "
-                      f"oracle.attend fp64, {dt:.2f} s",
-            "seconds": dt}
+    for (r, n), (K, V), q in zip(chosen, data, qs):
+        out[r] = oracle.attend(q, K, V)
+    return time.perf_counter() - t, out
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle as it stands, timed on the host cores on bounded samples (no GPU work
-    other than producing the seeded inputs with the generator's device twin when a GPU is present)."""
+    """--impl reference: the CPU oracle as it stands, timed on the host cores; every step is one pass over the same
+    bounded sample the `cpu_baseline` leg of our arm uses (sized so that the whole run ends within a few minutes)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    import numpy as np
     import oracle
-    from kf_inputs import gen, workloads
+    from kf_inputs import workloads
+    try:
+        import torch
+        have_gpu = torch.cuda.is_available()
+    except Exception:
+        have_gpu = False
     wl = workloads.by_name(args.workload)
     lens = [s - 1 for s in wl.contexts]
-    # bounded sample: a 4096-token prefix of the shortest request, all heads, per step
-    r = min(range(wl.batch), key=lambda i: lens[i])
-    n = min(4096, lens[r] + 1)
-    pos = np.arange(n)
-    K, V = gen.gen_k(0, r, pos, wl.n_kv_heads, wl.seed), gen.gen_v(0, r, pos, wl.n_kv_heads, wl.seed)
+    n_steps = max(1, args.warmup + args.steps)
+    chosen, data, desc = oracle_sample(wl, lens, min(15.0, 150.0 / n_steps), have_gpu)
     times = []
-    for step in range(args.warmup + args.steps):
-        q = gen.gen_q(0, r, step, wl.n_q_heads, wl.seed)
-        t = time.perf_counter()
-        oracle.attend(q, K, V)
+    for step in range(n_steps):
+        dt, _ = oracle_run(wl, chosen, data, step)
         if step >= args.warmup:
-            times.append(time.perf_counter() - t)
+            times.append(dt)
     dt = sum(times) / len(times)
-    val = n * wl.kv_bytes_per_token() / dt / 1e9
-    sample = f"{wl.name}: request {r}, first {n} context tokens, all {wl.n_q_heads} heads, one layer, per step"
+    val = sum(n for _, n in chosen) * wl.kv_bytes_per_token() / dt / 1e9
+    sample = desc + ", one pass per step"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": wl.name, "note": wl.note, "sample": sample},
+            "sample": sample,
             "cpu_baseline": {"value": val, "unit": UNIT, "kind": "oracle", "cores": oracle.num_threads(), "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -253,53 +305,75 @@ def run_route_install(args):
 
 
 # ---------------------------------------------------------------------------------------------------------
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=300)
-    ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--workload", default="cfg3")
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--attend-impl", type=int, default=0, help="KF_IMPL_*: 0 auto, 1 simple, 2 tma")
-    ap.add_argument("--layers-phys", type=int, default=0, help="physical layer pools (0 = auto)")
-    ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 50)")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--min-tiles", type=int, default=0)
-    ap.add_argument("--kv-l2-policy", type=int, default=0, help="kf_config.kv_l2_policy: 0 default, 1 evict-first, 2 normal")
-    ap.add_argument("--route-install", action="store_true", help="measure the latency of a scale event (route "
-                    "install) and of the token boundary instead of the decode benchmark")
-    ap.add_argument("--no-l2-flush", action="store_true", help="do not flush L2 between timed steps when the KV of a "
-                    "layer-step fits L2 (cfg1)")
-    ap.add_argument("--no-graph", action="store_true", help="launch the calls of a step one by one instead of "
-                    "replaying the static step graph")
-    args = ap.parse_args()
-    if args.impl == "reference":
-        return run_reference(args)
-    if args.route_install:
-        return run_route_install(args)
-    args.warmup = max(args.warmup, 3)
+def measure_static(ses, wl, dev, reps=60, warm=5):
+    """SURVEY 8(d) protocol for the static configs: the state is prepared once (S-1 tokens loaded, token boundary,
+    append at position S-1) and `kf_kv_append + kf_attend` is repeated WITHOUT a commit, so every repetition attends
+    over exactly the stated contexts.  Repetitions are replays of one captured graph of the two calls (the C-ABI calls
+    are capturable); CUDA events around every replay; 512 MiB are written between replays when the KV fits L2."""
+    import torch
+    kf = ses.kf
+    kf.token_boundary()
+    q = ses.q_for(0, 0)
+    k_new, v_new = ses.kv_new_for(0, 0)
+    kf.kv_append(0, k_new, v_new)
+    kf.attend(0, q, ses.o, ses.lse)
+    torch.cuda.synchronize(dev)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=torch.cuda.current_stream(dev)):
+        kf.kv_append(0, k_new, v_new)
+        kf.attend(0, q, ses.o, ses.lse)
+    lens = list(ses.len0)
+    nbytes, kv = algorithmic_bytes(wl, lens, 1)
+    flush = kv <= 4 * 126e6
+    flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device=dev) if flush else None
+    ev = []
+    for i in range(warm + reps):
+        if flush:
+            flush_buf.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        g.replay()
+        b.record()
+        if i >= warm:
+            ev.append((a, b))
+    torch.cuda.synchronize(dev)
+    ts = sorted(a.elapsed_time(b) for a, b in ev)
+    # the attend launch alone, eagerly, events around the call
+    at = []
+    for i in range(warm + 20):
+        if flush:
+            flush_buf.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        kf.attend(0, q, ses.o, ses.lse)
+        b.record()
+        if i >= warm:
+            at.append((a, b))
+    torch.cuda.synchronize(dev)
+    att = sorted(a.elapsed_time(b) for a, b in at)
+    assert kf.status() == 0
+    del g, flush_buf
+    med = ts[len(ts) // 2]
+    return {"protocol": "SURVEY 8(d) static: no commit between repetitions; append + attend replayed as one graph",
+            "context_tokens": sum(lens) + wl.batch, "algorithmic_bytes": nbytes,
+            "us_per_layer_step_median": med * 1e3, "us_per_layer_step_min": ts[0] * 1e3,
+            "value": nbytes / (med * 1e-3) / 1e9, "pct_of_nominal_8TBs": 100.0 * nbytes / (med * 1e-3) / 1e9 / NOMINAL_PEAK_GBS,
+            "attend_us_median": att[len(att) // 2] * 1e3, "attend_us_min": att[0] * 1e3, "l2_flushed": bool(flush),
+            "repetitions": reps}
 
+
+def measure(args, wl_name, steps, warmup, e2e_steps, dev, dist, rank, world, local, want_cpu, want_probe=True):
+    """Everything bench.py reports for ONE workload; returns the record (rank 0) or None."""
     import torch
     from kf_inputs import workloads
     from paper_2606_29207_b200 import sharding
     from paper_2606_29207_b200.workload import Session
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    dev = torch.device(f"cuda:{local}")
-    torch.cuda.set_stream(torch.cuda.Stream(dev))   # stream capture (kf_step_graph_create) needs a non-default stream
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
-
-    wl = workloads.by_name(args.workload)
+    t_wall0 = time.perf_counter()
+    wl = workloads.by_name(wl_name)
     wl.seed = sharding.rank_seed(wl.seed, rank)    # independent batch per rank (weak scaling)
     n_layers = wl.n_layers
-    e2e_steps = args.e2e_steps or min(args.steps, 50)
-    total_steps = args.warmup + args.steps + 200 + e2e_steps + 2   # + the roofline and L2-warm regions (<= 100 steps each)
+    total_steps = warmup + steps + 200 + e2e_steps + 4   # + the roofline and L2-warm regions (<= 100 steps each)
     if args.layers_phys:
         L_phys = args.layers_phys
     else:
@@ -311,6 +385,11 @@ def main():
     kf = ses.kf
     ses.prepare()
     assert kf.status() == 0
+    prepare_s = time.perf_counter() - t_wall0
+
+    static = None
+    if n_layers == 1 and rank == 0 and not args.no_static:
+        static = measure_static(ses, wl, dev)      # leaves len untouched (no commit): the loop below starts at step 0
 
     # per-step inputs, resident in HBM before the timed region (keyed by physical layer)
     def inputs(step):
@@ -333,7 +412,7 @@ def main():
                 kf.attend(layer % L_phys, q, ses.o, ses.lse)
         kf.step_commit()
 
-    n_eager = max(1, args.warmup - 2)
+    n_eager = max(1, warmup - 2)
     step = 0
     for _ in range(n_eager):
         run_step(inputs(step))
@@ -361,13 +440,13 @@ def main():
             q, kn, vn = per_layer(step_inputs)
             graph.launch(q, kn, vn, o_list, lse_list)
 
-    for _ in range(args.warmup - n_eager):          # the last warm-up steps run exactly what is timed
+    for _ in range(warmup - n_eager):          # the last warm-up steps run exactly what is timed
         timed_step(inputs(step))
         step += 1
-    resident = n_layers * args.steps <= 4096
-    timed_inputs = [inputs(step + i) for i in range(args.steps)] if resident else None
+    resident = n_layers * steps <= 4096
+    timed_inputs = [inputs(step + i) for i in range(steps)] if resident else None
     total_bytes = kv_bytes = 0
-    for i in range(args.steps):
+    for i in range(steps):
         b, k = algorithmic_bytes(wl, [n + step + i for n in lens], n_layers)
         total_bytes += b
         kv_bytes += k
@@ -383,12 +462,12 @@ def main():
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     # KV of one layer-step that fits L2 (cfg1: 16 MiB vs 126 MB) would be served from L2 after the first step:
     # write a 512 MiB buffer between timed steps, outside the per-step event windows, so `value` is an HBM number
-    flush = kv_bytes / (args.steps * n_layers) <= 4 * 126e6 and not args.no_l2_flush
+    flush = kv_bytes / (steps * n_layers) <= 4 * 126e6 and not args.no_l2_flush
     flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device=dev) if flush else None
     step_events = []
     t0 = sampler.mark()
     e0.record()
-    for i in range(args.steps):
+    for i in range(steps):
         if flush:
             flush_buf.zero_()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -403,11 +482,11 @@ def main():
     if dist:
         dist.barrier()
     launches = kf.launch_count() - launches0
-    step += args.steps
+    step += steps
     ms = sum(a.elapsed_time(b) for a, b in step_events) if flush else e0.elapsed_time(e1)
     warm_ms_per_step = None
     if flush:        # the L2-warm number, reported beside it: the same steps back to back
-        n_warm = min(args.steps, 100)
+        n_warm = min(steps, 100)
         warm_inputs = [inputs(step + i) for i in range(n_warm)]
         torch.cuda.synchronize(dev)
         e0.record()
@@ -422,7 +501,7 @@ def main():
 
     # ---- roofline region: the same steps launched one by one, CUDA events around every kf_attend (events cannot
     #      be recorded inside a graph replay); also gives the eager step time ---------------------------------------
-    roof_steps = max(1, min(args.steps, 4096 // n_layers, 100))
+    roof_steps = max(1, min(steps, 4096 // n_layers, 100))
     roof_inputs = [inputs(step + i) for i in range(roof_steps)]
     attend_events = []
     r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -447,7 +526,7 @@ def main():
     # ---- read-only bandwidth probe over the same KV pools (third denominator; MEASURED_PEAKS' figure is a copy) ----
     probe_gbs = None
     pool_bytes = sum(p.numel() for p in kf.pools)
-    if rank == 0 and pool_bytes > 8 * 126e6:
+    if rank == 0 and want_probe and pool_bytes > 8 * 126e6:
         sink = torch.zeros(1, dtype=torch.int32, device=dev)
         best = None
         for _ in range(4):
@@ -461,7 +540,7 @@ def main():
         probe_gbs = pool_bytes / (best * 1e-3) / 1e9
     ms, total_bytes_all, launches_all = sharding.aggregate(ms, total_bytes, launches, dist, dev)
     value = sharding.throughput_gbs(total_bytes_all, ms)
-    ms_per_step = ms / args.steps
+    ms_per_step = ms / steps
 
     # ---- end to end: HOST buffers, transfers inside the timed region.  One replay per step of a host-io step graph
     #      (pinned buffers): every layer-step reads q / k_new / v_new from host memory over the bus and
@@ -505,27 +584,59 @@ def main():
     h2d = n_layers * (B * Hq * 128 * 2 + 2 * B * Hkv * 128 * 2)
     d2h = n_layers * (B * Hq * 128 * 4 + B * Hq * 4)
     assert kf.status() == 0 and checksum == checksum
+    if hgraph is not None:
+        hgraph.destroy()
 
+    cpu = parity = None
+    if rank == 0 and world == 1 and want_cpu:
+        # ---- the oracle on the host cores (a baseline, not the target), and PARITY of this very step: one more decode
+        #      step through the timed path (the static step graph), its (o, lse) compared with what the oracle just computed
+        import numpy as np
+        import oracle
+        lens_now = [n + step for n in lens]
+        chosen, data, desc = oracle_sample(wl, lens_now, 15.0, True)
+        timed_step(inputs(step))                    # physical layer of the last layer-step: layer_ids[-1]
+        torch.cuda.synchronize(dev)
+        assert kf.status() == 0
+        o_gpu, lse_gpu = ses.o.cpu().numpy().astype(np.float64), ses.lse.cpu().numpy().astype(np.float64)
+        dt, ref = oracle_run(wl, chosen, data, step)
+        nbytes = sum(n for _, n in chosen) * wl.kv_bytes_per_token()
+        cpu = {"value": nbytes / dt / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{desc}, decode step {step}, {dt:.2f} s", "seconds": dt}
+        if layer_ids[-1] == 0 and all(n == lens_now[r] + 1 for r, n in chosen):
+            eo = max(float(np.abs(o_gpu[r] - ref[r][0]).max()) for r, _ in chosen)
+            el = max(float((np.abs(lse_gpu[r] - ref[r][1]) / np.maximum(1.0, np.abs(ref[r][1]))).max())
+                     for r, _ in chosen)
+            mo = max(float(np.abs(ref[r][0]).max()) for r, _ in chosen)
+            parity = {"max_abs_o": eo, "max_rel_lse": el, "rows": len(chosen) * Hq, "requests": len(chosen),
+                      "max_abs_o_ref": mo, "tol_abs_o": 2e-3, "tol_rel_lse": 1e-4,
+                      "ok": bool(eo <= 2e-3 and el <= 1e-4),
+                      "what": f"kf_step_graph replay of decode step {step} (all {Hq} heads of the sampled requests) vs "
+                              "oracle.attend fp64 on the same inputs"}
+        step += 1
+        del data
+
+    if graph is not None:
+        graph.destroy()
+    ses.close()
+    del ses, kf, flush_buf
+    gc.collect()
+    torch.cuda.empty_cache()
     if rank != 0:
-        if dist:
-            dist.barrier()
-            dist.destroy_process_group()
-        return 0
+        return None
 
     peak, peak_src = load_peak()
     achieved = attend_bytes / (attend_ms * 1e-3) / 1e9
-    cpu = None
-    if world == 1 and not args.no_cpu_baseline:
-        cpu = cpu_baseline_sample(wl, [n + step for n in lens], step)
-    line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+    traffic, traffic_src = traffic_record(wl.name, args)
+    return {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f16 storage, f32 accumulate", "data": "synthetic",
         "config": {"workload": wl.name, "note": wl.note, "batch": B, "n_q_heads": Hq, "n_kv_heads": Hkv,
                    "range_tokens": wl.range_tokens, "n_partitions": wl.n_partitions, "layers_logical": n_layers,
                    "layers_physical": L_phys, "context_tokens_step0": sum(lens) + B,
                    "l2": "inputs larger than L2 (KV read per layer-step >> 126 MB); no flush needed" if not flush and
-                         kv_bytes / (args.steps * n_layers) > 4 * 126e6 else
+                         kv_bytes / (steps * n_layers) > 4 * 126e6 else
                          "KV fits L2: 512 MiB written between timed steps, outside the per-step CUDA-event windows "
                          "(value, ms_per_step, roofline are L2-cold; warm_ms_per_step is the back-to-back number)"
                          if flush else "KV fits L2 and --no-l2-flush given: numbers are L2-warm",
@@ -543,14 +654,79 @@ def main():
         "gpu_launches": launches_all,
         "roofline": {"bound": "hbm", "kernel": "attend_tma_kernel" if args.attend_impl != 1 else "attend_simple_kernel",
                      "achieved": achieved, "peak": peak, "unit": UNIT, "frac": achieved / peak,
-                     "traffic": NCU_TRAFFIC_BYTES.get(wl.name), "algorithmic_bytes_per_launch": attend_bytes,
+                     "traffic": traffic, "traffic_source": traffic_src, "kernel_rev": kernel_rev(),
+                     "algorithmic_bytes_per_launch": attend_bytes,
                      "avg_launch_ms": attend_ms, "median_launch_ms": attend_times[len(attend_times) // 2],
                      "min_launch_ms": attend_times[0], "launches_timed": len(attend_times), "peak_source": peak_src,
                      "frac_of_nominal_8000": achieved / NOMINAL_PEAK_GBS,
                      "read_probe_gbs": probe_gbs, "frac_of_read_probe": achieved / probe_gbs if probe_gbs else None},
+        "static": static,
         "cpu_baseline": cpu,
+        "parity": parity,
+        "wall_s": {"prepare": prepare_s, "total": time.perf_counter() - t_wall0},
     }
-    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--workload", default="cfg3", help="the headline workload of the JSON line")
+    ap.add_argument("--only", action="store_true", help="measure the headline workload only (no `workloads` sub-records)")
+    ap.add_argument("--sub", default=",".join(SUB_WORKLOADS), help="comma-separated sub-record workloads")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--attend-impl", type=int, default=0, help="KF_IMPL_*: 0 auto, 1 simple, 2 tma")
+    ap.add_argument("--layers-phys", type=int, default=0, help="physical layer pools (0 = auto)")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 50)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--min-tiles", type=int, default=0)
+    ap.add_argument("--kv-l2-policy", type=int, default=0, help="kf_config.kv_l2_policy: 0 default, 1 evict-first, 2 normal")
+    ap.add_argument("--route-install", action="store_true", help="measure the latency of a scale event (route "
+                    "install) and of the token boundary instead of the decode benchmark")
+    ap.add_argument("--no-l2-flush", action="store_true", help="do not flush L2 between timed steps when the KV of a "
+                    "layer-step fits L2 (cfg1)")
+    ap.add_argument("--no-graph", action="store_true", help="launch the calls of a step one by one instead of "
+                    "replaying the static step graph")
+    ap.add_argument("--no-static", action="store_true", help="skip the static (no-commit) protocol")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.route_install:
+        return run_route_install(args)
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+    torch.cuda.set_stream(torch.cuda.Stream(dev))   # stream capture (kf_step_graph_create) needs a non-default stream
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    e2e_steps = args.e2e_steps or min(args.steps, 50)
+    line = measure(args, args.workload, args.steps, args.warmup, e2e_steps, dev, dist, rank, world, local,
+                   want_cpu=not args.no_cpu_baseline)
+    subs = {}
+    if not args.only and world == 1:
+        for name in [w for w in args.sub.split(",") if w and w != args.workload]:
+            st, wu, e2 = SUB_STEPS.get(name, (50, 5, 20))
+            rec = measure(args, name, st, wu, e2, dev, None, 0, 1, local, want_cpu=False, want_probe=name != "cfg1")
+            subs[name] = {k: rec[k] for k in ("value", "ms_per_step", "us_per_layer_step", "pct_of_nominal_8TBs", "steps",
+                                              "warmup", "clocks", "e2e", "gpu_launches", "static", "warm_ms_per_step",
+                                              "wall_s")}
+            subs[name]["config"] = rec["config"]
+            subs[name]["roofline"] = rec["roofline"]
+    if rank == 0:
+        if subs:
+            line["workloads"] = subs
+        print(json.dumps(line))
     if dist:
         dist.barrier()
         dist.destroy_process_group()
