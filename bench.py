@@ -294,6 +294,11 @@ def run_route_install(args):
             ev.append(event_us(kf.token_boundary)[0])
             kf.step_commit()
         out[f"token_boundary_{key}_event_us"] = statistics.median(ev)
+        if key == "kept_plan":
+            # graph progress signalling: gate release on the signalling stream -> ReadValue32-style wait
+            # inside a running graph -> WriteValue32-style readiness flag -> seen by the spinning host thread
+            med, mn = kf.signal_roundtrip(2000, torch.cuda.Stream(), torch.cuda.Stream())
+            out["signal_roundtrip_us_median"], out["signal_roundtrip_us_min"] = med, mn
         assert kf.status() == 0
         ses.close()
     e = []

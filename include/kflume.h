@@ -244,6 +244,33 @@ int kf_step_graph_launch(kf_graph *graph, const void *const *q, const void *cons
                          float *const *o, float *const *lse, kf_stream stream);
 int kf_step_graph_destroy(kf_graph *graph);
 
+/* ---- graph progress signalling ---------------------------------------------------------
+ * The paper's static graph "contains only local compute and signal writes": where an outbound buffer becomes ready a
+ * WriteValue32-style write sets a flag in host-visible memory, "allowing the CPU to observe graph progress without
+ * ending replay" (:167); the other way round a ReadValue32-style wait inside the graph holds a stage back until the CPU
+ * has written a completion flag to GPU memory -- on "a dedicated signaling stream rather than the graph's execution
+ * stream: the execution stream is already blocked on that wait, so enqueuing the flag write on the same stream would
+ * place it behind the wait and deadlock" (:175).  The single-GPU analogue: a host thread (the paper's CPU routing
+ * loop) can hand the inputs of layer-step i to a RUNNING step graph and pick its outputs up, layer-step by
+ * layer-step, with no re-capture -- e.g. while it edits the routing table for the next step.
+ *
+ * kf_step_graph_flags: adds the signal nodes to a step graph that has not been launched yet (it is re-captured on
+ *   `stream`; nothing executes).  ready_host: [host] PINNED uint32[n] or NULL: after layer-step i of launch L the graph
+ *   writes seq(L, i) = (L - 1) * n + i + 1 to ready_host[i]; every write of that layer-step (o[i] / lse[i], also when
+ *   they are host buffers) is visible to a host thread that has read the value.  gates != 0: before layer-step i of
+ *   launch L (before its kf_kv_append reads k_new[i] / v_new[i] / q[i]) the graph waits until gate word i -- device
+ *   memory inside the workspace -- is >= seq(L, i) (cyclic 32-bit comparison).  Both values are re-written into the
+ *   graph's mem-op nodes at every launch (host-side update, no re-instantiation).  KF_ESTATE after the first launch;
+ *   KF_EINVAL if ready_host is not pinned memory the GPU can address.
+ * kf_step_graph_seq: the sequence number layer-step i will carry in the NEXT launch (0 on bad arguments).
+ * kf_step_graph_release: writes `seq` to gate word i with a stream memory operation on `signal_stream`.  Everything the
+ *   host stored into the layer-step's pinned input buffers before this call is visible to the kernels behind the
+ *   gate.  KF_ESTATE if `signal_stream` is the stream of the graph's last launch (the deadlock of PAPER.md:175 is
+ *   refused instead of entered) or the graph has no gates.  A gate may be released before the launch that waits on it. */
+int kf_step_graph_flags(kf_graph *graph, uint32_t *ready_host, int32_t gates, kf_stream stream);
+uint32_t kf_step_graph_seq(const kf_graph *graph, int32_t layer_step);
+int kf_step_graph_release(kf_graph *graph, int32_t layer_step, uint32_t seq, kf_stream signal_stream);
+
 /* ---- inspection (tests) ---------------------------------------------------------------------------
  * kf_route_snapshot: downloads the routing state into [host] arrays (any may be NULL):
  *   len[B] (-1 = closed), n_ranges[B], part[B][Jmax], slot[B][Jmax] (-1 where unused), free_head[P],
@@ -302,8 +329,14 @@ int kf_policy_step(const kf_policy_config *cfg, int32_t n_partitions, const int6
  *   a persistent grid and discards the data -- the read-only HBM bandwidth this box delivers to a trivial kernel, the
  *   third roofline denominator next to the nominal 8 TB/s and the measured copy bandwidth.
  *   sink: [device] 4 bytes, scratch.  *bytes_read [host, may be NULL] = P * kf_pool_bytes().  Asynchronous on `stream`;
- *   time it with events.  Not counted in kf_launch_count. */
+ *   time it with events.  Not counted in kf_launch_count.
+ * kf_signal_roundtrip: latency of the signalling path above, `iters` times: a two-node graph [wait gate >= seq] ->
+ *   [write seq to a pinned host word] is launched on exec_stream, the host releases the gate on signal_stream and
+ *   spins on the host word.  *median_us / *min_us [host] = host enqueue + GPU reaction + write visible to the host: an
+ *   upper bound on "GPU store -> host sees it".  Synchronises both streams. */
 int kf_plan_info(kf_ctx *ctx, int32_t *out, kf_stream stream);
+int kf_signal_roundtrip(kf_ctx *ctx, int32_t iters, kf_stream exec_stream, kf_stream signal_stream, double *median_us,
+                        double *min_us);
 int kf_worker_times(kf_ctx *ctx, int64_t *out, int32_t *n_workers, kf_stream stream);
 int kf_probe_read(kf_ctx *ctx, void *sink, size_t *bytes_read, kf_stream stream);
 

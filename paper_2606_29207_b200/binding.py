@@ -19,6 +19,7 @@ EXPORTS = [
     "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_step_commit", "kf_layer_step_host",
     "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count", "kf_worker_times",
     "kf_step_graph_create", "kf_step_graph_launch", "kf_step_graph_destroy", "kf_probe_read",
+    "kf_step_graph_flags", "kf_step_graph_seq", "kf_step_graph_release", "kf_signal_roundtrip",
     "kf_set_active_partitions", "kf_partition_state", "kf_set_active_requests",
     "kf_policy_bytes_per_token", "kf_policy_threshold", "kf_policy_initial_nodes", "kf_policy_step",
 ]
@@ -93,6 +94,10 @@ def load_library():
     L.kf_step_graph_create.argtypes = [vp, i32, ctypes.POINTER(i32), i32, pp, pp, pp, pp, pp, vp, ctypes.POINTER(vp)]
     L.kf_step_graph_launch.argtypes = [vp, pp, pp, pp, pp, pp, vp]
     L.kf_step_graph_destroy.argtypes = [vp]
+    L.kf_step_graph_flags.argtypes = [vp, vp, i32, vp]
+    L.kf_step_graph_seq.argtypes, L.kf_step_graph_seq.restype = [vp, i32], ctypes.c_uint32
+    L.kf_step_graph_release.argtypes = [vp, i32, ctypes.c_uint32, vp]
+    L.kf_signal_roundtrip.argtypes = [vp, i32, vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     L.kf_set_active_partitions.argtypes = [vp, ctypes.POINTER(ctypes.c_uint8), vp]
     L.kf_set_active_requests.argtypes = [vp, vp, vp]
     L.kf_partition_state.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32), vp]
@@ -271,6 +276,14 @@ class KFlume:
         self._check(self.lib.kf_probe_read(self.h, _ptr(sink), ctypes.byref(n), self._stream(stream)), "kf_probe_read")
         return int(n.value)
 
+    def signal_roundtrip(self, iters: int, exec_stream, signal_stream):
+        """kf_signal_roundtrip: (median_us, min_us) of gate release -> readiness flag seen by the host."""
+        med, mn = ctypes.c_double(0), ctypes.c_double(0)
+        self._check(self.lib.kf_signal_roundtrip(self.h, iters, ctypes.c_void_p(exec_stream.cuda_stream),
+                                                 ctypes.c_void_p(signal_stream.cuda_stream), ctypes.byref(med),
+                                                 ctypes.byref(mn)), "kf_signal_roundtrip")
+        return med.value, mn.value
+
     def set_active_partitions(self, active: Sequence[int], stream=None):
         assert len(active) == self.P
         arr = (ctypes.c_uint8 * self.P)(*[1 if x else 0 for x in active])
@@ -351,6 +364,26 @@ class StepGraph:
             self._keep = (list(q), list(k_new), list(v_new), list(o), list(lse))
             args = self._arrays(*self._keep)
         self.kf._check(self.kf.lib.kf_step_graph_launch(self.h, *args, self.kf._stream(stream)), "kf_step_graph_launch")
+
+    def flags(self, ready_host=None, gates: bool = False, stream=None):
+        """kf_step_graph_flags: ready_host = pinned int32/uint32 CPU tensor [n] (or None); gates = wait before each
+        layer-step until released.  Call before the first launch."""
+        if ready_host is not None:
+            assert not ready_host.is_cuda and ready_host.is_pinned() and ready_host.numel() == self.n
+            assert ready_host.element_size() == 4 and ready_host.is_contiguous()
+        self._ready = ready_host
+        self.kf._check(self.kf.lib.kf_step_graph_flags(self.h, _ptr(ready_host), 1 if gates else 0,
+                                                       self.kf._stream(stream)), "kf_step_graph_flags")
+
+    def seq(self, layer_step: int) -> int:
+        """Sequence number layer-step i carries in the NEXT launch."""
+        return int(self.kf.lib.kf_step_graph_seq(self.h, layer_step))
+
+    def release(self, layer_step: int, seq: int, signal_stream):
+        """kf_step_graph_release on the DEDICATED signalling stream."""
+        self.kf._check(self.kf.lib.kf_step_graph_release(self.h, layer_step, seq,
+                                                         ctypes.c_void_p(signal_stream.cuda_stream)),
+                       "kf_step_graph_release")
 
     def destroy(self):
         if getattr(self, "h", None) and self.kf.h:

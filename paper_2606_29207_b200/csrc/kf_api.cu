@@ -43,7 +43,7 @@ inline size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a
 struct Layout {
     size_t len, n_ranges, route_part, route_slot, rr_cursor, rr_last, req_active, active, part_tokens, part_tails, free_head, free_cnt, free_stack, error, plan, units, chunks, plan_age, sched,
         scratch, unit_counter, group_counter, piece_o, piece_lse, range_o, range_lse, stage_q, stage_k, stage_v,
-        stage_o, stage_lse, tmaps, worker_times, total;
+        stage_o, stage_lse, tmaps, gates, worker_times, total;
 };
 
 bool valid_config(const kf_config *c) {
@@ -120,6 +120,7 @@ Layout make_layout(const kf_config *c) {
     L.stage_o = take(B * Hq * kHeadDim * 4);
     L.stage_lse = take(B * Hq * 4);
     L.tmaps = take(P * 2 * 128);
+    L.gates = take((size_t)kMaxGraphLayerSteps * 4);
     L.worker_times = take((size_t)kMaxWorkers * 4 * 8);
     L.total = off;
     return L;
@@ -342,6 +343,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.stage_o = (float *)(ws + L.stage_o);
     d.stage_lse = (float *)(ws + L.stage_lse);
     d.tmaps = ws + L.tmaps;
+    d.gates = (uint32_t *)(ws + L.gates);
     d.worker_times = (long long *)(ws + L.worker_times);
     d.v_off = half_pool_bytes(cfg);
     for (int p = 0; p < cfg->n_partitions; ++p) d.pool[p] = (unsigned char *)pool_ptrs[p];

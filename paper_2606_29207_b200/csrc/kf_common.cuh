@@ -19,6 +19,7 @@ constexpr int kMaxLevels = 16;        // levels of the guided self-scheduling ch
 constexpr int kChunkSlack = 16 * kMaxWorkers;  // chunk capacity = units + kChunkSlack
 constexpr int kMaxGroup = 8;          // G = H_q / H_kv
 constexpr int kMaxPartitions = 64;
+constexpr int kMaxGraphLayerSteps = 4096;  // layer-steps per step graph = gate words in the workspace
 constexpr int kPlanStale = 1 << 30;    // plan_age value that forces a rebuild at the next token boundary
 
 // One unit of attention work: (request, token range, kv head).  Built by the plan kernel.
@@ -104,6 +105,7 @@ struct Dev {
     unsigned char *pool[kMaxPartitions];
     size_t v_off;        // byte offset of the V half of a pool
     const void *tmaps;   // [P][2] CUtensorMap (K, V) in device memory, 128-byte stride
+    uint32_t *gates;     // [kMaxGraphLayerSteps] gate words of the signalled step graph (kf_step_graph_flags)
     long long *worker_times;  // [kMaxWorkers][4]: {smid, t_start, t_first_tile, t_end} (globaltimer ns), diagnostics
 };
 
