@@ -13,6 +13,10 @@ Recipe (all uint64 arithmetic wraps):
     normal16(x)       = fp16_rn( fp32(sum of the 8 bytes of x - 1020) * c ),  c = fp32 bits 0x3B9CC4BF
     idx(layer, req, pos, head, dim) = dim | head<<7 | pos<<14 | req<<38 | layer<<54
     streams: q=1 (pos field = decode step), K=2, V=3, cfg-3 lengths=0x33, cfg-5 lengths=0x55
+    W-side stages: hidden state x=4 (pos field = decode step), weights Wq=0x10, Wkv=0x11, Wo=0x12,
+    Wgate=0x13, Wup=0x14, Wdown=0x15: element [n][k] of a weight matrix [out_features][in_features] is
+    normal16(hash(key, idx(layer, 0, pos=n, head=k>>7, dim=k&127))) * 2^-s with 2^-s ~ 1/sqrt(in_features)
+    (an exact power-of-two scaling in fp16), so y = x W^T has unit variance for unit-variance x.
 """
 from __future__ import annotations
 
@@ -21,6 +25,8 @@ import numpy as np
 SEED = 260629207
 STREAM_Q, STREAM_K, STREAM_V = 1, 2, 3
 STREAM_LEN_CFG3, STREAM_LEN_CFG5 = 0x33, 0x55
+STREAM_X = 4
+STREAM_WQ, STREAM_WKV, STREAM_WO, STREAM_WGATE, STREAM_WUP, STREAM_WDOWN = 0x10, 0x11, 0x12, 0x13, 0x14, 0x15
 
 _M1 = np.uint64(0xBF58476D1CE4E5B9)
 _M2 = np.uint64(0x94D049BB133111EB)
@@ -94,3 +100,22 @@ def gen_k(layer: int, req: int, pos, n_kv_heads: int, seed: int = SEED) -> np.nd
 
 def gen_v(layer: int, req: int, pos, n_kv_heads: int, seed: int = SEED) -> np.ndarray:
     return tensor(STREAM_V, layer, req, pos, n_kv_heads, seed)
+
+
+def weight_shift(in_features: int) -> int:
+    """s with 2^-s the power of two nearest to 1/sqrt(in_features) from below in log2 (4096 -> 6, 14336 -> 7)."""
+    return int(round(0.5 * np.log2(in_features)))
+
+
+def gen_weight(stream: int, layer: int, n_out: int, n_in: int, seed: int = SEED) -> np.ndarray:
+    """Synthetic fp16 weight matrix [n_out][n_in] (n_in a multiple of 128) of one W-side stream."""
+    assert n_in % 128 == 0
+    t = tensor(stream, layer, 0, np.arange(n_out), n_in // 128, seed)            # [n_in/128][n_out][128]
+    w = np.ascontiguousarray(t.transpose(1, 0, 2)).reshape(n_out, n_in)
+    return (w.astype(np.float32) * np.float32(2.0 ** -weight_shift(n_in))).astype(np.float16)   # exact
+
+
+def gen_x(layer: int, batch: int, step: int, hidden: int, seed: int = SEED) -> np.ndarray:
+    """Hidden state x[batch][hidden] fp16 entering layer `layer` at decode step `step` (row r = request r)."""
+    return np.stack([tensor(STREAM_X, layer, r, [step], hidden // 128, seed)[:, 0, :].reshape(hidden)
+                     for r in range(batch)])

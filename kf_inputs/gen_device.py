@@ -71,3 +71,22 @@ def fill_rows(stream_id: int, layer: int, pos, heads: int, out=None, seed: int =
     if rc:
         raise RuntimeError(f"kfgen_fill_rows: cudaError {rc}")
     return out
+
+
+def fill_weight(stream_id: int, layer: int, n_out: int, n_in: int, out=None, seed: int = gen.SEED):
+    """Device twin of gen.gen_weight: fp16 CUDA tensor [n_out][n_in]."""
+    import torch
+    assert n_in % 128 == 0
+    t = fill(stream_id, layer, 0, 0, n_out, n_in // 128, seed=seed)               # [n_in/128][n_out][128]
+    w = t.permute(1, 0, 2).reshape(n_out, n_in) * (2.0 ** -gen.weight_shift(n_in))   # power of two: exact in fp16
+    if out is None:
+        return w.contiguous()
+    out.copy_(w)
+    return out
+
+
+def fill_x(layer: int, batch: int, step: int, hidden: int, seed: int = gen.SEED):
+    """Device twin of gen.gen_x: fp16 CUDA tensor [batch][hidden]."""
+    import torch
+    pos = torch.full((batch,), step, dtype=torch.int32, device="cuda")
+    return fill_rows(gen.STREAM_X, layer, pos, hidden // 128, seed=seed).reshape(batch, hidden)

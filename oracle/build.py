@@ -1,21 +1,21 @@
-"""Compile oracle/attention.c into oracle/libkforacle.so (gcc, OpenMP).  Test infrastructure only."""
+"""Compile oracle/attention.c and oracle/wside.c into oracle/libkforacle.so (gcc, OpenMP).  Test infrastructure only."""
 from __future__ import annotations
 
 import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "attention.c")
+SRCS = [os.path.join(HERE, "attention.c"), os.path.join(HERE, "wside.c")]
 LIB = os.path.join(HERE, "libkforacle.so")
 
 
 def build(force: bool = False) -> str:
     if (not force and os.path.exists(LIB)
-            and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
+            and all(os.path.getmtime(LIB) >= os.path.getmtime(s) for s in SRCS)):
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
     cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
-           "-o", tmp, SRC, "-lm"]
+           "-o", tmp] + SRCS + ["-lm"]
     subprocess.run(cmd, check=True)
     os.replace(tmp, LIB)
     return LIB
