@@ -87,6 +87,8 @@ typedef struct kf_config {
                                      * (0 => 128; 1 => every step); in between, tail ranges grow inside the kept plan */
     int32_t kv_l2_policy;           /* L2 policy of the K/V tile loads: 0 => default (1); 1 = evict-first (K/V is read once
                                      * per launch; keeps q, partials and the plan resident: +1..5% measured); 2 = normal */
+    int32_t attend_sms;             /* SM budget of the attend kernels: CTAs (one per SM) of their persistent grid; 0 => all
+                                     * SMs.  A narrower grid leaves SMs to kernels of other streams (kf_pipeline_step) */
     int32_t diagnostics;            /* non-zero: the attend kernel records per-worker timestamps (kf_worker_times);
                                      * 0 (default): it reads no timer and writes nothing beyond the method's outputs */
 } kf_config;
@@ -315,6 +317,67 @@ double kf_policy_threshold(const kf_policy_config *cfg);
 int64_t kf_policy_initial_nodes(const kf_policy_config *cfg, const int64_t *s, int32_t n_requests);
 int kf_policy_step(const kf_policy_config *cfg, int32_t n_partitions, const int64_t *tokens, const int32_t *tails,
                    const uint8_t *prewarm_pending, const uint8_t *prewarm_ready, kf_policy_decision *out);
+
+/* ---- W-node stages and the inter-layer kernel pipeline ----------------------------------
+ * The stages of a decode layer that run on the paper's weight-bearing W nodes, around core attention:
+ *   T_p  projection (step 1):  q = x Wq^T, then (k_new, v_new) = x Wkv^T -- "Q first": two
+ *        launches, so that everything which depends only on q can be released before the K/V projection is done;
+ *   T_f  post-attention (step 5): y = o Wo^T;  h = silu(y Wg^T) * (y Wu^T) (SwiGLU, the FFN of the
+ *        Llama models the paper serves);  x' = h Wd^T.
+ * Every contraction is the hand-written tcgen05 GEMM of kf_wgemm.cu (weights streamed once by TMA, accumulators in
+ * TMEM).  Tensors stored between kernels are fp16, accumulation is fp32.  No residuals, norms or rotary embedding:
+ * the weights are synthetic and this part exists to measure the pipeline of PAPER.md:266-280 (reading 26).
+ *
+ * Weights: ONE [device] buffer, 1024-byte aligned, kf_wside_weight_bytes() long; matrix `which` of layer l starts at
+ *   kf_wside_weight_offset() and is stored [out_features][in_features] fp16, rows contiguous:
+ *   KF_W_Q [H_q*d][hidden], KF_W_KV [2*H_kv*d][hidden] (K rows, then V rows), KF_W_O [hidden][H_q*d],
+ *   KF_W_GATE [ffn][hidden], KF_W_UP [ffn][hidden] (directly behind the gate), KF_W_DOWN [hidden][ffn].
+ * Workspace: [device], 256-byte aligned, kf_wside_workspace_bytes(); holds the fp16 copy of o, y, h and the split-K
+ *   partial sums.  The caller owns both buffers; the library owns the host-side handle.  The calls of one kf_wside must
+ *   execute one after another (they share the workspace): one stream, or streams ordered by events.
+ * Shapes: x, x_next [batch][hidden] fp16; q [batch][H_q][128], k_new / v_new [batch][H_kv][128] fp16 (the layouts
+ *   kf_kv_append / kf_attend take); o [batch][H_q][128] fp32 (what kf_attend writes).  1 <= batch <= max_batch <= 128.
+ *   hidden and ffn are multiples of 128, head_dim is 128.  All calls are asynchronous on `stream`, never synchronise,
+ *   never allocate, and can be captured into a CUDA graph. */
+#define KF_W_Q 0
+#define KF_W_KV 1
+#define KF_W_O 2
+#define KF_W_GATE 3
+#define KF_W_UP 4
+#define KF_W_DOWN 5
+typedef struct kf_wside_config {
+    int32_t hidden, n_q_heads, n_kv_heads, head_dim /* 128 */, ffn, n_layers, max_batch /* <= 128 */;
+} kf_wside_config;
+typedef struct kf_wside kf_wside;
+size_t kf_wside_weight_bytes(const kf_wside_config *cfg);
+size_t kf_wside_weight_offset(const kf_wside_config *cfg, int32_t layer, int32_t which);
+size_t kf_wside_workspace_bytes(const kf_wside_config *cfg);
+int kf_wside_create(kf_wside **out, const kf_wside_config *cfg, void *weights, void *workspace, size_t workspace_bytes);
+int kf_wside_destroy(kf_wside *w);
+const char *kf_wside_last_error(const kf_wside *w);
+int64_t kf_wside_launch_count(const kf_wside *w);
+int kf_w_project_q(kf_wside *w, int32_t layer, const void *x, int32_t batch, void *q, kf_stream stream);
+int kf_w_project_kv(kf_wside *w, int32_t layer, const void *x, int32_t batch, void *k_new, void *v_new, kf_stream stream);
+int kf_w_post_attention(kf_wside *w, int32_t layer, const float *o, int32_t batch, void *x_next, kf_stream stream);
+
+/* kf_pipeline_step -- ONE decode step of n_micro microbatches through n_layers layers, W-side stages included
+ *   (Fig. 7).  Microbatch m is the batch of ctxs[m] (its own requests, routing table and KV pools;
+ *   max_requests <= the kf_wside's max_batch, same head shape).  layers: [host] int32[n_layers] W-side layer of each
+ *   layer of the step (its KV layer is layers[l] % the ctx's physical layers).  x: [host] n_micro [device] pointers
+ *   [B_m][hidden] fp16: the hidden state entering layer 0, overwritten in place by every layer (x' of the last layer on
+ *   return).  q, k_new, v_new, o, lse: [host] arrays of n_micro [device] scratch buffers (shapes as in kf_attend).
+ *   Per microbatch and layer: kf_w_project_q, kf_w_project_kv, kf_kv_append, kf_attend, kf_w_post_attention; one
+ *   kf_token_boundary per microbatch at the start, the step commit with the last layer's attend.
+ *   pipelined == 0: everything on w_stream, microbatch after microbatch -- the serial schedule, T_p + T_A + T_f per
+ *   microbatch and layer.  pipelined != 0: projections and post-attention on w_stream, append + attention on a_stream
+ *   (must differ), ordered by events exactly as Fig. 7: while the A side attends one microbatch the W side finishes the
+ *   previous one and projects the next; a filled pipeline completes a microbatch every max(T_p + T_f, T_A) and
+ *   G_pipe = (T_p + T_A + T_f) / max(T_p + T_f, T_A).  On ONE GPU both sides share the SMs and the HBM,
+ *   so kf_config.attend_sms is the knob that leaves SMs to the GEMMs.  Results are identical in both modes.
+ *   Asynchronous; when w_stream has drained the step is complete. */
+int kf_pipeline_step(kf_wside *w, kf_ctx *const *ctxs, int32_t n_micro, int32_t n_layers, const int32_t *layers,
+                     void *const *x, void *const *q, void *const *k_new, void *const *v_new, float *const *o,
+                     float *const *lse, int32_t pipelined, kf_stream w_stream, kf_stream a_stream);
 
 /* ---- diagnostics (not part of the method; nothing here runs on the hot path) -------------------------------------
  * kf_plan_info: downloads the work-plan header into out[8] [host]: {n_units, n_tiles, n_workers_active,

@@ -22,7 +22,11 @@ EXPORTS = [
     "kf_step_graph_flags", "kf_step_graph_seq", "kf_step_graph_release", "kf_signal_roundtrip",
     "kf_set_active_partitions", "kf_partition_state", "kf_set_active_requests",
     "kf_policy_bytes_per_token", "kf_policy_threshold", "kf_policy_initial_nodes", "kf_policy_step",
+    "kf_wside_weight_bytes", "kf_wside_weight_offset", "kf_wside_workspace_bytes", "kf_wside_create", "kf_wside_destroy",
+    "kf_wside_last_error", "kf_wside_launch_count", "kf_w_project_q", "kf_w_project_kv", "kf_w_post_attention",
+    "kf_pipeline_step",
 ]
+KF_W_Q, KF_W_KV, KF_W_O, KF_W_GATE, KF_W_UP, KF_W_DOWN = range(6)
 
 
 class kf_config(ctypes.Structure):
@@ -35,8 +39,14 @@ class kf_config(ctypes.Structure):
         ("workers_per_sm", ctypes.c_int32), ("pipeline_stages", ctypes.c_int32),
         ("sched_first_pct", ctypes.c_int32), ("sched_decay_pct", ctypes.c_int32),
         ("plan_refresh_steps", ctypes.c_int32), ("kv_l2_policy", ctypes.c_int32),
-        ("diagnostics", ctypes.c_int32),
+        ("attend_sms", ctypes.c_int32), ("diagnostics", ctypes.c_int32),
     ]
+
+
+class kf_wside_config(ctypes.Structure):
+    _fields_ = [("hidden", ctypes.c_int32), ("n_q_heads", ctypes.c_int32), ("n_kv_heads", ctypes.c_int32),
+                ("head_dim", ctypes.c_int32), ("ffn", ctypes.c_int32), ("n_layers", ctypes.c_int32),
+                ("max_batch", ctypes.c_int32)]
 
 
 class kf_policy_config(ctypes.Structure):
@@ -109,6 +119,18 @@ def load_library():
     L.kf_policy_step.argtypes = [pcp, i32, ctypes.POINTER(i64), ctypes.POINTER(i32), u8p, u8p,
                                  ctypes.POINTER(kf_policy_decision)]
     L.kf_probe_read.argtypes = [vp, vp, ctypes.POINTER(sz), vp]
+    wcp = ctypes.POINTER(kf_wside_config)
+    L.kf_wside_weight_bytes.argtypes, L.kf_wside_weight_bytes.restype = [wcp], sz
+    L.kf_wside_weight_offset.argtypes, L.kf_wside_weight_offset.restype = [wcp, i32, i32], sz
+    L.kf_wside_workspace_bytes.argtypes, L.kf_wside_workspace_bytes.restype = [wcp], sz
+    L.kf_wside_create.argtypes = [ctypes.POINTER(vp), wcp, vp, vp, sz]
+    L.kf_wside_destroy.argtypes = [vp]
+    L.kf_wside_last_error.argtypes, L.kf_wside_last_error.restype = [vp], ctypes.c_char_p
+    L.kf_wside_launch_count.argtypes, L.kf_wside_launch_count.restype = [vp], i64
+    L.kf_w_project_q.argtypes = [vp, i32, vp, i32, vp, vp]
+    L.kf_w_project_kv.argtypes = [vp, i32, vp, i32, vp, vp, vp]
+    L.kf_w_post_attention.argtypes = [vp, i32, vp, i32, vp, vp]
+    L.kf_pipeline_step.argtypes = [vp, pp, i32, i32, ctypes.POINTER(i32), pp, pp, pp, pp, pp, pp, i32, vp, vp]
     for name in EXPORTS:
         if getattr(L, name).restype is None:
             getattr(L, name).restype = ctypes.c_int
@@ -119,7 +141,7 @@ def load_library():
 def make_config(n_q_heads, n_kv_heads, range_tokens, n_partitions, max_requests, max_ranges_per_request,
                 slots_per_partition, n_layers=1, softmax_scale=0.0, attend_impl=KF_IMPL_AUTO,
                 min_tiles_per_worker=0, head_dim=128, workers_per_sm=0, pipeline_stages=0, sched_first_pct=0,
-                sched_decay_pct=0, plan_refresh_steps=0, kv_l2_policy=0, diagnostics=0) -> kf_config:
+                sched_decay_pct=0, plan_refresh_steps=0, kv_l2_policy=0, diagnostics=0, attend_sms=0) -> kf_config:
     c = kf_config()
     c.n_q_heads, c.n_kv_heads, c.head_dim, c.n_layers = n_q_heads, n_kv_heads, head_dim, n_layers
     c.range_tokens, c.n_partitions, c.max_requests = range_tokens, n_partitions, max_requests
@@ -130,6 +152,7 @@ def make_config(n_q_heads, n_kv_heads, range_tokens, n_partitions, max_requests,
     c.plan_refresh_steps = plan_refresh_steps
     c.kv_l2_policy = kv_l2_policy
     c.diagnostics = diagnostics
+    c.attend_sms = attend_sms
     return c
 
 
@@ -424,3 +447,107 @@ class Policy:
         if rc != KF_OK:
             raise KFlumeError(rc, "kf_policy_step: invalid argument")
         return [(d.tau_fill, bool(d.want_prewarm), bool(d.want_publish)) for d in out]
+
+
+class WSide:
+    """The W-node stages (kf_wside_*, kf_w_*): QKV projection, W_O and the SwiGLU FFN as tcgen05 GEMMs, plus the
+    M-microbatch inter-layer pipeline (kf_pipeline_step).  Owns the weight and workspace buffers (torch)."""
+
+    def __init__(self, hidden: int, n_q_heads: int, n_kv_heads: int, ffn: int, n_layers: int = 1, max_batch: int = 128,
+                 device: str = "cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise KFlumeError(KF_ECUDA, "no CUDA device: libkflume has no CPU fallback")
+        self.lib, self.torch = load_library(), torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        c = kf_wside_config(hidden, n_q_heads, n_kv_heads, 128, ffn, n_layers, max_batch)
+        self.cfg = c
+        wb, sb = self.lib.kf_wside_weight_bytes(ctypes.byref(c)), self.lib.kf_wside_workspace_bytes(ctypes.byref(c))
+        if wb == 0 or sb == 0:
+            raise KFlumeError(KF_EINVAL, "invalid kf_wside_config")
+        self._w_store = torch.empty(wb + 1024, dtype=torch.uint8, device=self.device)
+        off = (-self._w_store.data_ptr()) % 1024
+        self.weights = self._w_store[off:off + wb]
+        self._s_store = torch.empty(sb + 256, dtype=torch.uint8, device=self.device)
+        off = (-self._s_store.data_ptr()) % 256
+        self.workspace = self._s_store[off:off + sb]
+        h = ctypes.c_void_p()
+        rc = self.lib.kf_wside_create(ctypes.byref(h), ctypes.byref(c), _ptr(self.weights), _ptr(self.workspace), sb)
+        self.h = h
+        if rc != KF_OK:
+            msg = self.lib.kf_wside_last_error(h).decode() if h else ""
+            if h:
+                self.lib.kf_wside_destroy(h)
+                self.h = None
+            raise KFlumeError(rc, f"kf_wside_create: {self.lib.kf_strerror(rc).decode()} {msg}")
+        self.hidden, self.Hq, self.Hkv, self.ffn, self.L = hidden, n_q_heads, n_kv_heads, ffn, n_layers
+
+    def shape(self, which: int):
+        qd, kvd = self.Hq * 128, self.Hkv * 128
+        return {KF_W_Q: (qd, self.hidden), KF_W_KV: (2 * kvd, self.hidden), KF_W_O: (self.hidden, qd),
+                KF_W_GATE: (self.ffn, self.hidden), KF_W_UP: (self.ffn, self.hidden),
+                KF_W_DOWN: (self.hidden, self.ffn)}[which]
+
+    def weight(self, layer: int, which: int):
+        """fp16 view [out_features][in_features] of one weight matrix inside the weight buffer (write into it)."""
+        off = self.lib.kf_wside_weight_offset(ctypes.byref(self.cfg), layer, which)
+        n, k = self.shape(which)
+        return self.weights[off:off + n * k * 2].view(self.torch.float16).view(n, k)
+
+    def _stream(self, stream=None):
+        s = self.torch.cuda.current_stream(self.device) if stream is None else stream
+        return ctypes.c_void_p(s.cuda_stream)
+
+    def _check(self, rc, what):
+        if rc != KF_OK:
+            extra = self.lib.kf_wside_last_error(self.h).decode() if rc == KF_ECUDA else ""
+            raise KFlumeError(rc, f"{what}: {self.lib.kf_strerror(rc).decode()} {extra}")
+
+    def project_q(self, layer, x, q, stream=None):
+        B = x.shape[0]
+        assert x.is_cuda and x.dtype == self.torch.float16 and x.is_contiguous() and x.shape == (B, self.hidden)
+        assert q.is_cuda and q.dtype == self.torch.float16 and q.is_contiguous() and q.numel() == B * self.Hq * 128
+        self._check(self.lib.kf_w_project_q(self.h, layer, _ptr(x), B, _ptr(q), self._stream(stream)), "kf_w_project_q")
+
+    def project_kv(self, layer, x, k_new, v_new, stream=None):
+        B = x.shape[0]
+        assert x.is_cuda and x.dtype == self.torch.float16 and x.is_contiguous() and x.shape == (B, self.hidden)
+        for t in (k_new, v_new):
+            assert t.is_cuda and t.dtype == self.torch.float16 and t.is_contiguous() and t.numel() == B * self.Hkv * 128
+        self._check(self.lib.kf_w_project_kv(self.h, layer, _ptr(x), B, _ptr(k_new), _ptr(v_new), self._stream(stream)),
+                    "kf_w_project_kv")
+
+    def post_attention(self, layer, o, x_next, stream=None):
+        B = o.shape[0]
+        assert o.is_cuda and o.dtype == self.torch.float32 and o.is_contiguous() and o.numel() == B * self.Hq * 128
+        assert x_next.is_cuda and x_next.dtype == self.torch.float16 and x_next.is_contiguous()
+        assert x_next.shape == (B, self.hidden)
+        self._check(self.lib.kf_w_post_attention(self.h, layer, _ptr(o), B, _ptr(x_next), self._stream(stream)),
+                    "kf_w_post_attention")
+
+    def pipeline_step(self, kfs, layers, x, q, k_new, v_new, o, lse, pipelined, w_stream, a_stream):
+        """kf_pipeline_step: kfs = list of KFlume (one per microbatch); x .. lse = lists of CUDA tensors."""
+        M = len(kfs)
+        arr = lambda lst: (ctypes.c_void_p * M)(*[t.data_ptr() for t in lst])   # noqa: E731
+        ctxs = (ctypes.c_void_p * M)(*[k.h.value for k in kfs])
+        la = (ctypes.c_int32 * len(layers))(*layers)
+        self._check(self.lib.kf_pipeline_step(self.h, ctxs, M, len(layers), la, arr(x), arr(q), arr(k_new), arr(v_new),
+                                              arr(o), arr(lse), 1 if pipelined else 0,
+                                              ctypes.c_void_p(w_stream.cuda_stream), ctypes.c_void_p(a_stream.cuda_stream)),
+                    "kf_pipeline_step")
+
+    def launch_count(self) -> int:
+        return int(self.lib.kf_wside_launch_count(self.h))
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.torch.cuda.synchronize(self.device)
+            self.lib.kf_wside_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -69,7 +69,7 @@ bool valid_config(const kf_config *c) {
     if (c->sched_decay_pct < 0 || c->sched_decay_pct > 99) return false;
     if (c->plan_refresh_steps < 0) return false;
     if (c->kv_l2_policy < 0 || c->kv_l2_policy > 2) return false;
-    if (c->diagnostics < 0) return false;
+    if (c->diagnostics < 0 || c->attend_sms < 0) return false;
     // rows of one K (or V) half-pool must fit the int32 TMA coordinate
     const double rows = (double)c->n_layers * c->slots_per_partition * c->n_kv_heads * c->range_tokens;
     if (rows >= 2147483647.0) return false;
@@ -266,7 +266,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     ctx->impl = cfg->attend_impl == KF_IMPL_AUTO ? KF_IMPL_TMA : cfg->attend_impl;
     // the CUDA-core kernel always runs 8 warps per CTA; the TMA kernel's shape is tunable
     const int warps = ctx->impl == KF_IMPL_SIMPLE ? kWarpsPerCta : (cfg->workers_per_sm ? cfg->workers_per_sm : kDefaultWarps);
-    ctx->n_ctas = ctx->sm_count;
+    ctx->n_ctas = cfg->attend_sms > 0 && cfg->attend_sms < ctx->sm_count ? cfg->attend_sms : ctx->sm_count;
     if (ctx->n_ctas * warps > kMaxWorkers) ctx->n_ctas = kMaxWorkers / warps;
     ctx->plan_dirty = true;
 

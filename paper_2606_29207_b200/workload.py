@@ -11,7 +11,8 @@ from typing import List, Optional
 from kf_inputs import gen, gen_device
 from kf_inputs.workloads import Workload
 
-from .binding import KF_IMPL_AUTO, KFlume, make_config
+from .binding import (KF_IMPL_AUTO, KF_W_DOWN, KF_W_GATE, KF_W_KV, KF_W_O, KF_W_Q, KF_W_UP, KFlume, WSide,
+                      make_config)
 
 
 class Session:
@@ -90,3 +91,20 @@ class Session:
 
     def close(self):
         self.kf.close()
+
+
+W_STREAMS = {KF_W_Q: gen.STREAM_WQ, KF_W_KV: gen.STREAM_WKV, KF_W_O: gen.STREAM_WO, KF_W_GATE: gen.STREAM_WGATE,
+             KF_W_UP: gen.STREAM_WUP, KF_W_DOWN: gen.STREAM_WDOWN}
+
+
+def make_wside(hidden: int, n_q_heads: int, n_kv_heads: int, ffn: int, n_layers: int = 1, max_batch: int = 128,
+               device: str = "cuda:0", seed: int = gen.SEED) -> WSide:
+    """A WSide whose weight buffer holds the seeded synthetic weights of kf_inputs (random-init stand-ins for the
+    Llama-3.1 weights of PAPER.md:288): matrix `which` of layer l = gen.gen_weight(W_STREAMS[which], l, ...)."""
+    w = WSide(hidden, n_q_heads, n_kv_heads, ffn, n_layers, max_batch, device)
+    for layer in range(n_layers):
+        for which, stream in W_STREAMS.items():
+            n, k = w.shape(which)
+            gen_device.fill_weight(stream, layer, n, k, out=w.weight(layer, which), seed=seed)
+    w.torch.cuda.synchronize(w.device)
+    return w
