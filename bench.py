@@ -309,6 +309,186 @@ def run_route_install(args):
     return 0
 
 
+
+def run_pipeline(args):
+    """--pipeline: W-side stages + M = 2 inter-layer kernel pipelining on ONE B200 (PAPER.md:252-280,
+    Fig. 11): for each workload (two microbatches of B_mu requests at context S, Llama-3.1-8B shape, synthetic weights)
+    measure T_p (Q + K/V projection), T_f (W_O + SwiGLU FFN), T_A (append + attend, as a function of the attend
+    kernel's SM budget), the serial and the pipelined step, and compare the measured ratio with the paper's model
+    G_pipe = (T_p + T_A + T_f) / max(T_p + T_f, T_A).  One JSON line."""
+    import statistics
+    import torch
+    from kf_inputs import gen_device, workloads
+    from kf_inputs.workloads import Workload
+    from paper_2606_29207_b200.workload import Session, make_wside
+
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    hidden, Hq, Hkv, ffn = 4096, 32, 8, 14336
+    n_layers = args.pipe_layers
+    Lw = 2                                           # physical weight layers (436 MB each >> L2), aliased
+    w = make_wside(hidden, Hq, Hkv, ffn, n_layers=Lw, max_batch=128)
+    weight_bytes_layer = sum(2 * a * b for a, b in (w.shape(i) for i in range(6)))
+    peak, peak_src = load_peak()
+    ws, as_ = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+
+    def graph_us(fn, reps=12, inner=8):
+        """Median device time of one fn(i), measured on replays of a CUDA graph that holds `inner` calls (the C-ABI
+        calls are capturable; a replay takes the host launch cost out of the measurement)."""
+        fn(0)
+        ws.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=ws):
+            for i in range(inner):
+                fn(i)
+        ts = []
+        for i in range(3 + reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(ws)
+            g.replay()
+            b.record(ws)
+            if i >= 3:
+                ts.append((a, b))
+        torch.cuda.synchronize(dev)
+        del g
+        return statistics.median(x.elapsed_time(y) for x, y in ts) * 1e3 / inner
+
+    cases = [tuple(int(v) for v in c.split("x")) for c in args.pipe_cases.split(",")]
+    sms_list = [int(v) for v in args.pipe_sms.split(",")]
+    rows = []
+    for (Bm, S) in cases:
+        R, P = 8192, 4
+        rec = {"B_mu": Bm, "seq": S, "microbatches": 2, "layers_per_step": n_layers}
+        best = None
+        for sms in sms_list:
+            wls = [Workload(f"mb{m}_b{Bm}_s{S}", Hq, Hkv, R, P, [S] * Bm, seed=260629207 + m) for m in range(2)]
+            total_steps = 40
+            sess = [Session(wl, n_layers_phys=1, steps=total_steps, attend_sms=0 if sms >= 148 else sms) for wl in wls]
+            for s_ in sess:
+                s_.prepare()
+            with torch.cuda.stream(ws):
+                bufs = []
+                for wl in wls:
+                    bufs.append({"x": gen_device.fill_x(0, Bm, 0, hidden, seed=wl.seed),
+                                 "q": torch.zeros((Bm, Hq, 128), dtype=torch.float16, device=dev),
+                                 "k": torch.zeros((Bm, Hkv, 128), dtype=torch.float16, device=dev),
+                                 "v": torch.zeros((Bm, Hkv, 128), dtype=torch.float16, device=dev),
+                                 "o": torch.zeros((Bm, Hq, 128), dtype=torch.float32, device=dev),
+                                 "lse": torch.zeros((Bm, Hq), dtype=torch.float32, device=dev)})
+                x0 = [b["x"].clone() for b in bufs]
+                layers = [l % Lw for l in range(n_layers)]
+                b0 = bufs[0]
+                if sms == sms_list[0]:
+                    # stage times, each alone on the GPU
+                    rec["T_p_us"] = graph_us(lambda i: (w.project_q(i % Lw, b0["x"], b0["q"], ws),
+                                                        w.project_kv(i % Lw, b0["x"], b0["k"], b0["v"], ws)))
+                    xs_ = torch.empty_like(b0["x"])
+                    rec["T_f_us"] = graph_us(lambda i: w.post_attention(i % Lw, b0["o"], xs_, ws))
+                kf0 = sess[0].kf
+                kf0.token_boundary(ws)
+                t_a = graph_us(lambda i: (kf0.kv_append(0, b0["k"], b0["v"], ws),
+                                          kf0.attend(0, b0["q"], b0["o"], b0["lse"], stream=ws)))
+                ws.synchronize()
+
+                def step_us(mode):
+                    """One decode step (n_layers layers x 2 microbatches) as ONE CUDA graph, replayed."""
+                    w.set_sms(148 - sms if mode and sms < 148 else 0)      # the GEMMs get the SMs the attend grid leaves
+                    def run():
+                        w.pipeline_step([s_.kf for s_ in sess], layers, [b_["x"] for b_ in bufs], [b_["q"] for b_ in bufs],
+                                        [b_["k"] for b_ in bufs], [b_["v"] for b_ in bufs], [b_["o"] for b_ in bufs],
+                                        [b_["lse"] for b_ in bufs], mode, ws, as_)
+                    run()
+                    ws.synchronize()
+                    g = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(g, stream=ws):
+                        run()
+                    ts = []
+                    for i in range(8):
+                        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        a.record(ws)
+                        g.replay()
+                        b.record(ws)
+                        if i >= 2:
+                            ts.append((a, b))
+                    torch.cuda.synchronize(dev)
+                    del g
+                    w.set_sms(0)
+                    return statistics.median(x.elapsed_time(y) for x, y in ts) * 1e3
+                ser = step_us(0)
+                pip = step_us(1)
+                for s_ in sess:
+                    assert s_.kf.status() == 0
+            for s_ in sess:
+                s_.close()
+            del sess, bufs
+            gc.collect()
+            torch.cuda.empty_cache()
+            per = {"attend_sms": sms, "T_A_us": t_a, "serial_us_per_layer_mb": ser / (2 * n_layers),
+                   "pipelined_us_per_layer_mb": pip / (2 * n_layers), "measured_ratio": ser / pip}
+            rec.setdefault("by_sms", []).append(per)
+            if best is None or per["pipelined_us_per_layer_mb"] < best["pipelined_us_per_layer_mb"]:
+                best = per
+        t_a148 = rec["by_sms"][0]["T_A_us"]
+        tp, tf = rec["T_p_us"], rec["T_f_us"]
+        kv_bytes = Bm * S * 4096
+        rec["T_A_us"] = t_a148
+        rec["model_G_pipe"] = (tp + t_a148 + tf) / max(tp + tf, t_a148)
+        rec["serial_us_per_layer_mb"] = rec["by_sms"][0]["serial_us_per_layer_mb"]
+        rec["serial_vs_sum_of_stages"] = rec["serial_us_per_layer_mb"] / (tp + t_a148 + tf)
+        rec["best"] = best
+        rec["measured_ratio_best"] = rec["serial_us_per_layer_mb"] / best["pipelined_us_per_layer_mb"]
+        # what ONE GPU allows: both stages are bound by the same HBM, so a filled pipeline cannot beat bytes / bandwidth
+        rec["bytes_per_layer_mb"] = weight_bytes_layer + kv_bytes
+        rec["one_gpu_hbm_floor_us"] = (weight_bytes_layer + kv_bytes) / (peak * 1e9) * 1e6
+        rec["W_side_GBs"] = weight_bytes_layer / ((tp + tf) * 1e-6) / 1e9
+        rec["pipelined_GBs"] = (weight_bytes_layer + kv_bytes) / (best["pipelined_us_per_layer_mb"] * 1e-6) / 1e9
+        rows.append(rec)
+    w.close()
+    print(json.dumps({"mode": "pipeline", "model": "Llama-3.1-8B shape (hidden 4096, 32/8 heads, ffn 14336), synthetic weights",
+                      "weight_bytes_per_layer": weight_bytes_layer, "peak_gbs": peak, "peak_source": peak_src,
+                      "cases": rows}))
+    return 0
+
+
+def run_sm_sweep(args):
+    """--sm-sweep: kf_attend GB/s against the SM budget of its persistent grid (kf_config.attend_sms)."""
+    import statistics
+    import torch
+    from kf_inputs import workloads
+    from paper_2606_29207_b200.workload import Session
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    wl = workloads.by_name(args.workload)
+    out = {"mode": "sm-sweep", "workload": wl.name, "points": []}
+    for sms in [int(v) for v in args.pipe_sms.split(",")]:
+        ses = Session(wl, n_layers_phys=1, steps=4, attend_sms=0 if sms >= 148 else sms)
+        ses.prepare()
+        kf = ses.kf
+        kf.token_boundary()
+        q = ses.q_for(0, 0)
+        k_new, v_new = ses.kv_new_for(0, 0)
+        kf.kv_append(0, k_new, v_new)
+        ts = []
+        for i in range(25):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            kf.attend(0, q, ses.o, ses.lse)
+            b.record()
+            if i >= 5:
+                ts.append((a, b))
+        torch.cuda.synchronize()
+        t = statistics.median(x.elapsed_time(y) for x, y in ts)
+        nbytes = algorithmic_bytes(wl, list(ses.len0), 1)[0]
+        out["points"].append({"attend_sms": sms, "attend_us": t * 1e3, "gbs": nbytes / (t * 1e-3) / 1e9})
+        assert kf.status() == 0
+        ses.close()
+        del ses
+        gc.collect()
+        torch.cuda.empty_cache()
+    print(json.dumps(out))
+    return 0
+
+
 # ---------------------------------------------------------------------------------------------------------
 def measure_static(ses, wl, dev, reps=60, warm=5):
     """SURVEY 8(d) protocol for the static configs: the state is prepared once (S-1 tokens loaded, token boundary,
@@ -695,11 +875,22 @@ def main():
     ap.add_argument("--no-graph", action="store_true", help="launch the calls of a step one by one instead of "
                     "replaying the static step graph")
     ap.add_argument("--no-static", action="store_true", help="skip the static (no-commit) protocol")
+    ap.add_argument("--pipeline", action="store_true", help="measure the W-side stages and the M = 2 inter-layer pipeline "
+                    "(PAPER.md:252-280) instead of the decode benchmark")
+    ap.add_argument("--pipe-cases", default="16x2048,16x8192,16x16384,32x4096,64x2048,64x8192,128x2048,128x4096,128x16384",
+                    help="--pipeline workloads: B_mu x seq (Fig. 11: batch 16-128, sequence 2K-16K)")
+    ap.add_argument("--pipe-sms", default="148,132,116,100,84", help="attend SM budgets tried by --pipeline / --sm-sweep")
+    ap.add_argument("--pipe-layers", type=int, default=8, help="layers per step in --pipeline")
+    ap.add_argument("--sm-sweep", action="store_true", help="kf_attend GB/s against its SM budget")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     if args.route_install:
         return run_route_install(args)
+    if args.pipeline:
+        return run_pipeline(args)
+    if args.sm_sweep:
+        return run_sm_sweep(args)
     args.warmup = max(args.warmup, 3)
 
     import torch

@@ -354,6 +354,9 @@ size_t kf_wside_weight_offset(const kf_wside_config *cfg, int32_t layer, int32_t
 size_t kf_wside_workspace_bytes(const kf_wside_config *cfg);
 int kf_wside_create(kf_wside **out, const kf_wside_config *cfg, void *weights, void *workspace, size_t workspace_bytes);
 int kf_wside_destroy(kf_wside *w);
+/* kf_wside_set_sms: SM budget of the GEMM kernels = CTAs of their persistent grid (0 => all SMs); takes effect for the
+ *   calls that follow.  Together with kf_config.attend_sms it partitions the GPU between the W side and the A side. */
+int kf_wside_set_sms(kf_wside *w, int32_t n_sms);
 const char *kf_wside_last_error(const kf_wside *w);
 int64_t kf_wside_launch_count(const kf_wside *w);
 int kf_w_project_q(kf_wside *w, int32_t layer, const void *x, int32_t batch, void *q, kf_stream stream);

@@ -23,7 +23,7 @@ EXPORTS = [
     "kf_set_active_partitions", "kf_partition_state", "kf_set_active_requests",
     "kf_policy_bytes_per_token", "kf_policy_threshold", "kf_policy_initial_nodes", "kf_policy_step",
     "kf_wside_weight_bytes", "kf_wside_weight_offset", "kf_wside_workspace_bytes", "kf_wside_create", "kf_wside_destroy",
-    "kf_wside_last_error", "kf_wside_launch_count", "kf_w_project_q", "kf_w_project_kv", "kf_w_post_attention",
+    "kf_wside_last_error", "kf_wside_launch_count", "kf_wside_set_sms", "kf_w_project_q", "kf_w_project_kv", "kf_w_post_attention",
     "kf_pipeline_step",
 ]
 KF_W_Q, KF_W_KV, KF_W_O, KF_W_GATE, KF_W_UP, KF_W_DOWN = range(6)
@@ -125,6 +125,7 @@ def load_library():
     L.kf_wside_workspace_bytes.argtypes, L.kf_wside_workspace_bytes.restype = [wcp], sz
     L.kf_wside_create.argtypes = [ctypes.POINTER(vp), wcp, vp, vp, sz]
     L.kf_wside_destroy.argtypes = [vp]
+    L.kf_wside_set_sms.argtypes = [vp, i32]
     L.kf_wside_last_error.argtypes, L.kf_wside_last_error.restype = [vp], ctypes.c_char_p
     L.kf_wside_launch_count.argtypes, L.kf_wside_launch_count.restype = [vp], i64
     L.kf_w_project_q.argtypes = [vp, i32, vp, i32, vp, vp]
@@ -536,6 +537,10 @@ class WSide:
                                               arr(o), arr(lse), 1 if pipelined else 0,
                                               ctypes.c_void_p(w_stream.cuda_stream), ctypes.c_void_p(a_stream.cuda_stream)),
                     "kf_pipeline_step")
+
+    def set_sms(self, n_sms: int):
+        """kf_wside_set_sms: CTAs of the persistent GEMM grid (0 = all SMs)."""
+        self._check(self.lib.kf_wside_set_sms(self.h, n_sms), "kf_wside_set_sms")
 
     def launch_count(self) -> int:
         return int(self.lib.kf_wside_launch_count(self.h))

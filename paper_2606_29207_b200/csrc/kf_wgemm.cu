@@ -14,8 +14,11 @@
 //     shared-memory descriptors), accumulators in TMEM; tcgen05.commit releases the ring stages;
 //   * warps 2..5 read the accumulators back with tcgen05.ld (32x32b: one output feature per thread, the batch along
 //     the registers) and store fp16;
-//   * N / 128 tiles rarely fill 148 SMs (Q projection of Llama-3.1-8B: 32 tiles), so K is split across CTAs; partial
-//     sums go through L2 as fp32 and the LAST CTA of a tile adds them in split order (deterministic) and writes fp16;
+//   * persistent, stream-K: N / 128 tiles rarely fill 148 SMs (Q projection of Llama-3.1-8B: 32 tiles), so the flat
+//     sequence of (tile, k-block) pairs is cut into one contiguous span per CTA; the TMA ring runs through a span
+//     without draining at tile boundaries, two TMEM accumulator buffers let the epilogue of one tile overlap the MMAs
+//     of the next; a tile that several spans share goes through L2 as fp32 pieces which a small fix-up kernel adds
+//     in k order (deterministic; no CTA ever waits for another one, so any SM budget is safe) and writes as fp16;
 //   * the gate and up projections of the FFN run as two accumulators of the same CTA (two weight tiles per stage,
 //     one shared activation tile), so SwiGLU is applied in the epilogue and g, u never exist in memory.
 #include <cuda.h>
@@ -100,6 +103,20 @@ __host__ __device__ constexpr int tmem_cols(int n) { return n <= 32 ? 32 : n <= 
 
 }  // namespace
 
+// One span of the stream-K decomposition: CTA c owns the k-blocks [c * per, (c + 1) * per) of the flat sequence
+// (tile 0: k-blocks 0 .. nkb-1, tile 1: ...).  A maximal run of k-blocks inside one tile is a SEGMENT: one accumulator.
+struct Span {
+    int k0, k1;
+};
+__device__ __forceinline__ Span span_of(const WGemmArgs &a, int cta, int n_ctas) {
+    const int total = (a.N / kWgTileN) * a.nkb;
+    const int per = (total + n_ctas - 1) / n_ctas;
+    Span sp;
+    sp.k0 = min(total, cta * per);
+    sp.k1 = min(total, sp.k0 + per);
+    return sp;
+}
+
 template <int NB, bool DUAL>
 __global__ void __launch_bounds__(kWgThreads, 1)
     wgemm_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmX, const WGemmArgs a) {
@@ -108,15 +125,15 @@ __global__ void __launch_bounds__(kWgThreads, 1)
     constexpr int kNW = DUAL ? 2 : 1;
     constexpr int kStageBytes = kWBytes * kNW + kXBytes;
     constexpr int kStages = wgemm_stages(NB, DUAL);
-    constexpr int kCols = tmem_cols(NB * kNW);
+    constexpr int kAccCols = NB * kNW;               // TMEM columns of one accumulator buffer
+    constexpr int kCols = tmem_cols(2 * kAccCols);   // two buffers: the epilogue of a segment overlaps the next one's MMAs
     extern __shared__ unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t full_bar[kStages], empty_bar[kStages], acc_bar;
+    __shared__ __align__(8) uint64_t full_bar[kStages], empty_bar[kStages], acc_full[2], acc_empty[2];
     __shared__ uint32_t tmem_base_s;
-    __shared__ int last_s;
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int tile = blockIdx.x / a.splits, split = blockIdx.x - tile * a.splits;
-    const int nkb = a.kb_per_split, kb0 = split * nkb;
+    const int nkb = a.nkb;
+    const Span sp = span_of(a, blockIdx.x, gridDim.x);
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmW) : "memory");
@@ -126,7 +143,11 @@ __global__ void __launch_bounds__(kWgThreads, 1)
             mbar_init(smem_u32(&full_bar[s]), 1);
             mbar_init(smem_u32(&empty_bar[s]), 1);
         }
-        mbar_init(smem_u32(&acc_bar), 1);
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(smem_u32(&acc_full[s]), 1);
+            mbar_init(smem_u32(&acc_empty[s]), 4);  // one arrival per epilogue warp
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -143,19 +164,25 @@ __global__ void __launch_bounds__(kWgThreads, 1)
 
     if (warp == 0) {
         if (lane == 0) {
-            // ---- TMA producer: weights are read once -> evict-first; the activation tile is re-read by every CTA ----
+            // ---- TMA producer: runs through the whole span, across tile boundaries; weights are read once ->
+            //      evict-first; the activation tile is re-read by every CTA -> evict-last ----
             uint64_t pol_w = 0, pol_x = 0;
             asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_w));
             asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_x));
-            for (int i = 0; i < nkb; ++i) {
+            int tile = sp.k0 / nkb, kb = sp.k0 - tile * nkb;
+            for (int i = 0; i < sp.k1 - sp.k0; ++i) {
                 const int s = i % kStages;
                 mbar_wait(smem_u32(&empty_bar[s]), ((i / kStages) & 1) ^ 1);
                 const uint32_t sb = base + s * kStageBytes, bar = smem_u32(&full_bar[s]);
-                const int kx = (kb0 + i) * kWgBK;
+                const int kx = kb * kWgBK;
                 mbar_expect_tx(bar, kStageBytes);
                 tma_load_2d_hint(sb, &tmW, kx, tile * kWgTileN, bar, pol_w);
                 if (DUAL) tma_load_2d_hint(sb + kWBytes, &tmW, kx, a.up_row_offset + tile * kWgTileN, bar, pol_w);
                 tma_load_2d_hint(sb + kWBytes * kNW, &tmX, kx, 0, bar, pol_x);
+                if (++kb == nkb) {
+                    kb = 0;
+                    ++tile;
+                }
             }
         }
         __syncwarp();
@@ -163,83 +190,83 @@ __global__ void __launch_bounds__(kWgThreads, 1)
         if (lane == 0) {
             // ---- MMA issuer: instruction descriptor: D fp32, A/B fp16 K-major, N = NB, M = 128 ----
             constexpr uint32_t idesc = (1u << 4) | ((uint32_t)(NB >> 3) << 17) | ((uint32_t)(kWgTileN >> 4) << 24);
-            for (int i = 0; i < nkb; ++i) {
-                const int s = i % kStages;
-                mbar_wait(smem_u32(&full_bar[s]), (i / kStages) & 1);
+            int i = 0, seg = 0;
+            for (int pos = sp.k0; pos < sp.k1; ++seg) {
+                const int kb = pos % nkb;
+                const int len = min(nkb - kb, sp.k1 - pos);
+                const int buf = seg & 1;
+                mbar_wait(smem_u32(&acc_empty[buf]), ((seg >> 1) & 1) ^ 1);  // the epilogue has drained this buffer
                 tc_fence_after();
-                const uint32_t sa = base + s * kStageBytes, sx = sa + kWBytes * kNW;
+                const uint32_t acc = tmem + buf * kAccCols;
+                for (int j = 0; j < len; ++j, ++i) {
+                    const int s = i % kStages;
+                    mbar_wait(smem_u32(&full_bar[s]), (i / kStages) & 1);
+                    tc_fence_after();
+                    const uint32_t sa = base + s * kStageBytes, sx = sa + kWBytes * kNW;
 #pragma unroll
-                for (int k = 0; k < kWgBK / 16; ++k) {
-                    const uint64_t db = umma_desc(sx + k * 32);
-                    umma_f16(tmem, umma_desc(sa + k * 32), db, idesc, (uint32_t)((i | k) != 0));
-                    if (DUAL) umma_f16(tmem + NB, umma_desc(sa + kWBytes + k * 32), db, idesc, (uint32_t)((i | k) != 0));
+                    for (int k = 0; k < kWgBK / 16; ++k) {
+                        const uint64_t db = umma_desc(sx + k * 32);
+                        umma_f16(acc, umma_desc(sa + k * 32), db, idesc, (uint32_t)((j | k) != 0));
+                        if (DUAL) umma_f16(acc + NB, umma_desc(sa + kWBytes + k * 32), db, idesc, (uint32_t)((j | k) != 0));
+                    }
+                    umma_commit(smem_u32(&empty_bar[s]));  // the stage is free once these MMAs have read it
                 }
-                umma_commit(smem_u32(&empty_bar[s]));  // the stage is free once these MMAs have read it
+                umma_commit(smem_u32(&acc_full[buf]));  // this segment's accumulator is complete
+                pos += len;
             }
-            umma_commit(smem_u32(&acc_bar));  // accumulators complete
         }
         __syncwarp();
     } else {
         // ---- epilogue: thread = one output feature (TMEM lane), registers run along the batch ----
         const int slice = warp & 3;  // a warp may only touch TMEM lanes 32 * (warp % 4) ..
         const int row = slice * 32 + lane;
-        const int n = tile * kWgTileN + row;
-        const uint32_t taddr = tmem + ((uint32_t)(slice * 32) << 16);
-        const int seg = (tile * kWgTileN >= a.seg_end[0]) + (tile * kWgTileN >= a.seg_end[1]);
-        const int nn = n - (seg == 0 ? 0 : a.seg_end[seg - 1]);
-        __half *out = a.out[seg] + nn;
-        const int ld = a.ld[seg];
-        mbar_wait(smem_u32(&acc_bar), 0);
-        tc_fence_after();
-        if (a.splits == 1) {
+        const size_t slot_floats = (size_t)NB * kWgTileN * kNW;  // one partial: [kNW][NB][128] fp32
+        int seg = 0;
+        for (int pos = sp.k0; pos < sp.k1; ++seg) {
+            const int tile = pos / nkb, kb = pos - tile * nkb;
+            const int len = min(nkb - kb, sp.k1 - pos);
+            const int buf = seg & 1;
+            const int n = tile * kWgTileN + row;
+            const int sg = (tile * kWgTileN >= a.seg_end[0]) + (tile * kWgTileN >= a.seg_end[1]);
+            __half *out = a.out[sg] + (n - (sg == 0 ? 0 : a.seg_end[sg - 1]));
+            const int ld = a.ld[sg];
+            const uint32_t taddr = tmem + ((uint32_t)(slice * 32) << 16) + buf * kAccCols;
+            mbar_wait(smem_u32(&acc_full[buf]), (seg >> 1) & 1);
+            tc_fence_after();
+            const bool whole = len == nkb;
+            if (whole) {
 #pragma unroll 1
-            for (int c0 = 0; c0 < NB; c0 += 16) {
-                float g[16], u[16];
-                tmem_ld16(taddr + c0, g);
-                if (DUAL) tmem_ld16(taddr + NB + c0, u);
-#pragma unroll
-                for (int j = 0; j < 16; ++j)
-                    if (c0 + j < a.B) out[(size_t)(c0 + j) * ld] = __float2half_rn(DUAL ? silu_mul(g[j], u[j]) : g[j]);
-            }
-        } else {
-            float *part = a.partial + ((size_t)split * NB) * a.N + n;
-            const size_t dual_off = (size_t)a.splits * NB * a.N;
-#pragma unroll 1
-            for (int c0 = 0; c0 < NB; c0 += 16) {
-                float g[16];
-                tmem_ld16(taddr + c0, g);
-#pragma unroll
-                for (int j = 0; j < 16; ++j)
-                    if (c0 + j < a.B) __stcg(part + (size_t)(c0 + j) * a.N, g[j]);
-                if (DUAL) {
-                    tmem_ld16(taddr + NB + c0, g);
+                for (int c0 = 0; c0 < NB; c0 += 16) {
+                    float g[16], u[16];
+                    tmem_ld16(taddr + c0, g);
+                    if (DUAL) tmem_ld16(taddr + NB + c0, u);
 #pragma unroll
                     for (int j = 0; j < 16; ++j)
-                        if (c0 + j < a.B) __stcg(part + dual_off + (size_t)(c0 + j) * a.N, g[j]);
+                        if (c0 + j < a.B) out[(size_t)(c0 + j) * ld] = __float2half_rn(DUAL ? silu_mul(g[j], u[j]) : g[j]);
                 }
-            }
-            asm volatile("bar.sync 1, 128;" ::: "memory");  // the 128 epilogue threads
-            if (threadIdx.x == 64) {
-                asm volatile("fence.acq_rel.gpu;" ::: "memory");
-                const int old = atomicAdd(a.counters + tile, 1);
-                const int last = old == a.splits - 1;
-                if (last) a.counters[tile] = 0;  // ready for the next launch
-                asm volatile("fence.acq_rel.gpu;" ::: "memory");
-                last_s = last;
-            }
-            asm volatile("bar.sync 1, 128;" ::: "memory");
-            if (last_s) {
-                // the last CTA of this tile adds the partial sums in split order and applies the epilogue
-                const float *p0 = a.partial + n;
-                for (int b = 0; b < a.B; ++b) {
-                    float g = 0.f, u = 0.f;
-                    for (int s = 0; s < a.splits; ++s) {
-                        g += __ldcg(p0 + ((size_t)s * NB + b) * a.N);
-                        if (DUAL) u += __ldcg(p0 + dual_off + ((size_t)s * NB + b) * a.N);
+            } else {
+                // a piece of a tile: fp32 partial into this CTA's slot (0: the span's first segment, 1: any later one)
+                float *part = a.partial + ((size_t)blockIdx.x * 2 + (seg == 0 ? 0 : 1)) * slot_floats + row;
+#pragma unroll 1
+                for (int c0 = 0; c0 < NB; c0 += 16) {
+                    float g[16];
+                    tmem_ld16(taddr + c0, g);
+#pragma unroll
+                    for (int j = 0; j < 16; ++j)
+                        if (c0 + j < a.B) __stcg(part + (size_t)(c0 + j) * kWgTileN, g[j]);
+                    if (DUAL) {
+                        tmem_ld16(taddr + NB + c0, g);
+#pragma unroll
+                        for (int j = 0; j < 16; ++j)
+                            if (c0 + j < a.B) __stcg(part + (size_t)(NB + c0 + j) * kWgTileN, g[j]);
                     }
-                    out[(size_t)b * ld] = __float2half_rn(DUAL ? silu_mul(g, u) : g);
                 }
             }
+            // the accumulator buffer is free again
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&acc_empty[buf])) : "memory");
+            pos += len;
         }
         tc_fence_before();
     }
@@ -248,6 +275,40 @@ __global__ void __launch_bounds__(kWgThreads, 1)
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kCols) : "memory");
     }
+}
+
+// Fix-up of the tiles that several spans share: out[b][n] = epilogue(sum over the pieces, in k order = ascending CTA).
+// One thread per (feature, batch row); every piece is read once, coalesced along the features.  grid (tiles, ceil(B / 8)).
+template <bool DUAL>
+__global__ void __launch_bounds__(kWgTileN * 8) wgemm_fixup_kernel(const WGemmArgs a, int nb) {
+    const int tile = blockIdx.x, row = threadIdx.x, b = blockIdx.y * 8 + threadIdx.y;
+    const int nkb = a.nkb;
+    const int total = (a.N / kWgTileN) * nkb;
+    const int per = (total + a.n_ctas - 1) / a.n_ctas;
+    const int c_first = (tile * nkb) / per, c_last = ((tile + 1) * nkb - 1) / per;
+    if (c_first == c_last || b >= a.B) return;  // the tile was whole: its CTA stored the result itself
+    const size_t slot_floats = (size_t)nb * kWgTileN * (DUAL ? 2 : 1);
+    float g = 0.f, u = 0.f;
+    for (int c0 = c_first; c0 <= c_last; c0 += 8) {
+        float t[8], tu[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            const int c = c0 + e;
+            const int slot = ((c * per) / nkb == tile) ? 0 : 1;  // slot 0 holds the span's first segment
+            const float *pp = a.partial + ((size_t)c * 2 + slot) * slot_floats + row;
+            t[e] = c <= c_last ? __ldcg(pp + (size_t)b * kWgTileN) : 0.f;
+            if (DUAL) tu[e] = c <= c_last ? __ldcg(pp + (size_t)(nb + b) * kWgTileN) : 0.f;
+        }
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            g += t[e];
+            if (DUAL) u += tu[e];
+        }
+    }
+    const int n = tile * kWgTileN + row;
+    const int sg = (tile * kWgTileN >= a.seg_end[0]) + (tile * kWgTileN >= a.seg_end[1]);
+    __half *out = a.out[sg] + (n - (sg == 0 ? 0 : a.seg_end[sg - 1]));
+    out[(size_t)b * a.ld[sg]] = __float2half_rn(DUAL ? silu_mul(g, u) : g);
 }
 
 // o [rows][cols] fp32 -> fp16 (the attention output that feeds W_O)
@@ -271,8 +332,12 @@ static int launch_one(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGem
             return KF_ECUDA;
         configured = true;
     }
-    wgemm_kernel<NB, DUAL><<<(a.N / kWgTileN) * a.splits, kWgThreads, smem, s>>>(tmW, tmX, a);
-    return 1;
+    wgemm_kernel<NB, DUAL><<<a.n_ctas, kWgThreads, smem, s>>>(tmW, tmX, a);
+    // tiles shared between spans exist unless every span boundary is a tile boundary
+    const int tiles = a.N / kWgTileN, total = tiles * a.nkb, per = (total + a.n_ctas - 1) / a.n_ctas;
+    if (per % a.nkb == 0) return 1;
+    wgemm_fixup_kernel<DUAL><<<dim3(tiles, (a.B + 7) / 8), dim3(kWgTileN, 8), 0, s>>>(a, NB);
+    return 2;
 }
 
 int launch_wgemm(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGemmArgs &a, int nb, bool dual, cudaStream_t s) {

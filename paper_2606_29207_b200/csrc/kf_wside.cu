@@ -22,6 +22,8 @@ struct kf_wside {
     CUtensorMap *maps;        // [L][5] weight maps (host copies, passed to kernels by value)
     cudaEvent_t ev[64];       // cross-stream dependencies of kf_pipeline_step
     int n_ev;
+    int n_ctas;               // persistent GEMM grid (<= SM count; kf_wside_set_sms)
+    int sm_count;
     int64_t launches;
     char cuda_err[256];
 };
@@ -83,28 +85,9 @@ size_t mat_offset(const kf_wside_config *c, int layer, int m) {
 }
 inline size_t up(size_t x) { return (x + 255) / 256 * 256; }
 int nb_of(int batch) { return batch <= 16 ? 16 : batch <= 32 ? 32 : batch <= 64 ? 64 : 128; }
-// K splits: the smallest divisor of the k-block count that gives at least ~120 CTAs (148 SMs), keeping >= 4 k-blocks each
-int splits_of(int tiles, int nkb) {
-    int best = 1;
-    for (int d = 1; d <= nkb; ++d) {
-        if (nkb % d) continue;
-        if (nkb / d < 4) break;
-        best = d;
-        if (tiles * d >= 120) break;
-    }
-    return best;
-}
-size_t partial_floats(const kf_wside_config *c) {
-    // the largest splits * NB * N * (dual ? 2 : 1) over the five contractions at NB = 128
-    size_t mx = 0;
-    for (int m = 0; m < 5; ++m) {
-        const bool dual = m == kMatGU;
-        const size_t N = dual ? (size_t)c->ffn : rows_of(c, m);
-        const int sp = splits_of((int)(N / kWgTileN), (int)(cols_of(c, m) / kWgBK));
-        const size_t f = (size_t)sp * kWgMaxBatch * N * (dual ? 2 : 1);
-        if (sp > 1 && f > mx) mx = f;
-    }
-    return mx;
+size_t partial_floats(const kf_wside_config *) {
+    // every CTA of the persistent grid owns two slots of one (dual) accumulator tile [2][NB = 128][128] fp32
+    return (size_t)kWgMaxCtas * 2 * 2 * kWgMaxBatch * kWgTileN;
 }
 size_t max_tiles(const kf_wside_config *c) {
     size_t mx = 0;
@@ -156,9 +139,8 @@ int gemm(kf_wside *w, int layer, int m, const void *x, int batch, __half *o0, in
     a.K = K;
     a.N = N;
     a.B = batch;
-    const int nkb = K / kWgBK;
-    a.splits = splits_of(N / kWgTileN, nkb);
-    a.kb_per_split = nkb / a.splits;
+    a.nkb = K / kWgBK;
+    a.n_ctas = w->n_ctas;
     a.seg_end[0] = e0;
     a.seg_end[1] = N;
     a.seg_end[2] = N;
@@ -169,7 +151,6 @@ int gemm(kf_wside *w, int layer, int m, const void *x, int batch, __half *o0, in
     a.out[2] = a.out[1];
     a.ld[2] = a.ld[1];
     a.partial = w->partial;
-    a.counters = w->counters;
     a.up_row_offset = dual ? c->ffn : 0;
     rc = launch_wgemm(w->maps[layer * 5 + m], tmX, a, nb, dual, s);
     if (rc < 0) return rc;
@@ -245,6 +226,13 @@ int kf_wside_create(kf_wside **out, const kf_wside_config *cfg, void *weights, v
                                   cols_of(cfg, m), kWgTileN);
             if (rc != KF_OK) return rc;
         }
+    int dev_id = 0;
+    cudaDeviceProp prop;
+    e = cudaGetDevice(&dev_id);
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev_id);
+    if (e != cudaSuccess) return fail(w, e);
+    w->sm_count = prop.multiProcessorCount < kWgMaxCtas ? prop.multiProcessorCount : kWgMaxCtas;
+    w->n_ctas = w->sm_count;
     w->n_ev = 64;
     for (int i = 0; i < w->n_ev; ++i) {
         e = cudaEventCreateWithFlags(&w->ev[i], cudaEventDisableTiming);
@@ -261,6 +249,12 @@ int kf_wside_destroy(kf_wside *w) {
     for (int i = 0; i < w->n_ev; ++i) cudaEventDestroy(w->ev[i]);
     delete[] w->maps;
     delete w;
+    return KF_OK;
+}
+
+int kf_wside_set_sms(kf_wside *w, int32_t n_sms) {
+    if (!w || n_sms < 0) return KF_EINVAL;
+    w->n_ctas = n_sms == 0 || n_sms > w->sm_count ? w->sm_count : n_sms;
     return KF_OK;
 }
 
@@ -341,6 +335,10 @@ int kf_pipeline_step(kf_wside *w, kf_ctx *const *ctxs, int32_t n_micro, int32_t 
         if (rc != KF_OK) return;
         rc = kf_w_post_attention(w, layers[l], o[m], B(m), x[m], (kf_stream)ws);
     };
+    // fork: the A stream joins the step after everything enqueued on the W stream so far (this also makes the whole
+    // step capturable into one CUDA graph from the W stream); joined again at the end
+    record(2 * n_micro, ws);
+    wait(2 * n_micro, as);
     // a1 on the A side: one token boundary per microbatch and step
     for (int m = 0; m < n_micro && rc == KF_OK; ++m) rc = kf_token_boundary(ctxs[m], (kf_stream)as);
     if (!pipelined) {
@@ -369,6 +367,8 @@ int kf_pipeline_step(kf_wside *w, kf_ctx *const *ctxs, int32_t n_micro, int32_t 
                 attend(m, l + 1);
             }
         }
+    record(2 * n_micro + 1, as);  // join
+    wait(2 * n_micro + 1, ws);
     return rc;
 }
 

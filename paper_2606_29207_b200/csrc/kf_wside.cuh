@@ -15,6 +15,7 @@ constexpr int kWgBK = 64;        // halfs per k-block = one 128-byte swizzle row
 constexpr int kWgTileN = 128;    // output features per CTA = UMMA M = TMEM lanes
 constexpr int kWgThreads = 192;  // warp 0: TMA producer; warp 1: TMEM allocator + MMA issuer; warps 2..5: epilogue
 constexpr int kWgMaxBatch = 128;
+constexpr int kWgMaxCtas = 160;   // upper bound of the persistent grid (SM count)
 
 __host__ __device__ constexpr int wgemm_stages(int nb, bool dual) { return dual ? (nb > 64 ? 4 : 5) : (nb > 64 ? 6 : 8); }
 __host__ __device__ constexpr int wgemm_smem_bytes(int nb, bool dual) {
@@ -23,13 +24,12 @@ __host__ __device__ constexpr int wgemm_smem_bytes(int nb, bool dual) {
 
 struct WGemmArgs {
     int K, N, B;          // reduction length, output features (per accumulator), valid batch rows
-    int splits;           // K is cut into `splits` equal parts, one CTA each
-    int kb_per_split;     // k-blocks (of 64) per split
+    int nkb;              // k-blocks (of 64) per tile = K / 64
+    int n_ctas;           // persistent grid: CTA c owns k-blocks [c * per, (c + 1) * per) of the (tile, k-block) sequence
     int seg_end[3];       // output segments: features [seg_end[i-1], seg_end[i]) go to out[i] (boundaries % 128 == 0)
     int ld[3];            // row stride (halfs) of each output
     __half *out[3];
-    float *partial;       // [splits][NB][N] fp32 (x 2 for the dual kernel); only used when splits > 1
-    int *counters;        // [N / 128] arrival counters, zero between launches
+    float *partial;       // [n_ctas][2 slots][1 or 2][NB][128] fp32: pieces of tiles shared between spans
     int up_row_offset;    // dual kernel: row of the first `up` weight in the weight tensor (gate rows come first)
 };
 
