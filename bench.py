@@ -69,7 +69,7 @@ def traffic_record(wl_name, args):
     if cap is None:
         return None, "no committed ncu capture for this workload"
     nbytes, src, rev = cap
-    if args.attend_impl == 1 or args.min_tiles or args.kv_l2_policy or args.no_graph:
+    if args.attend_impl == 1 or args.min_tiles or args.kv_l2_policy or args.no_graph or args.workers_per_sm or args.stages:
         return None, f"{src}: not applicable (non-default --attend-impl / --min-tiles / --kv-l2-policy / --no-graph)"
     if rev != kernel_rev():
         return None, f"{src}: stale (captured at kernel_rev {rev}, running {kernel_rev()})"
@@ -566,7 +566,8 @@ def measure(args, wl_name, steps, warmup, e2e_steps, dev, dist, rank, world, loc
         per_layer = wl.slots_per_partition(total_steps) * wl.n_partitions * wl.range_tokens * wl.kv_bytes_per_token()
         L_phys = max(1, min(n_layers, int(0.85 * free // per_layer)))
     ses = Session(wl, impl=args.attend_impl, n_layers_phys=L_phys, steps=total_steps, min_tiles=args.min_tiles,
-                  device=str(dev), kv_l2_policy=args.kv_l2_policy)
+                  device=str(dev), kv_l2_policy=args.kv_l2_policy, workers_per_sm=args.workers_per_sm,
+                  pipeline_stages=args.stages)
     kf = ses.kf
     ses.prepare()
     assert kf.status() == 0
@@ -867,6 +868,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 50)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--min-tiles", type=int, default=0)
+    ap.add_argument("--workers-per-sm", type=int, default=0, help="kf_config.workers_per_sm (0 = default)")
+    ap.add_argument("--stages", type=int, default=0, help="kf_config.pipeline_stages (0 = default)")
     ap.add_argument("--kv-l2-policy", type=int, default=0, help="kf_config.kv_l2_policy: 0 default, 1 evict-first, 2 normal")
     ap.add_argument("--route-install", action="store_true", help="measure the latency of a scale event (route "
                     "install) and of the token boundary instead of the decode benchmark")

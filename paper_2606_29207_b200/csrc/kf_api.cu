@@ -61,7 +61,9 @@ bool valid_config(const kf_config *c) {
     if (!(c->softmax_scale >= 0.f) || !isfinite(c->softmax_scale)) return false;
     if (c->attend_impl < KF_IMPL_AUTO || c->attend_impl > KF_IMPL_TMA) return false;
     if (c->min_tiles_per_worker < 0) return false;
-    if (c->workers_per_sm != 0 && c->workers_per_sm != 4 && c->workers_per_sm != 8) return false;
+    if (c->workers_per_sm != 0 && c->workers_per_sm != 4 && c->workers_per_sm != 8 && c->workers_per_sm != 12 &&
+        c->workers_per_sm != 16)
+        return false;
     if (c->pipeline_stages != 0 &&
         !attend_tma_shape_ok(c->workers_per_sm ? c->workers_per_sm : kDefaultWarps, c->pipeline_stages))
         return false;

@@ -28,9 +28,11 @@ constexpr int kTicketAhead = 3;                 // tiles before the end of a chu
 constexpr int kRing = 8;                        // chunk descriptors in flight between the load and compute cursors
 // P is rounded to fp16 for the P.V MMA.  With p = exp2(s - m) in (0, 1] every weight below 2^-25 would flush to zero
 // there while the fp32 row sum l keeps it: on a long, peaked context (1M tokens, each 2^-25 below the maximum) that
-// is up to 3% of the mass missing from o but present in l.  So P (and l with it) is carried scaled by 2^kPShift:
-// p' = exp2(s - m + 14) in (0, 16384], flush threshold 2^-39 relative to the maximum; o'/l' = o/l, lse = m + log2(l') - 14.
-constexpr float kPShift = 14.f;
+// is up to 3% of the mass missing from o but present in l.  So P (and l with it) is carried scaled up:
+// p' = exp2(s - m_ref + kPShift), where m_ref trails the true maximum by at most kLazy, so p' <= 2^14;
+// o'/l' = o/l, lse = m_ref + log2(l') - kPShift.
+constexpr float kLazy = 8.f;     // the reference maximum of a head moves only when a score exceeds it by 2^8
+constexpr float kPShift = 6.f;   // p = exp2(s - m_ref + 6) <= 2^14: fits fp16; flush threshold 2^-31 .. 2^-39 below the maximum
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -77,13 +79,19 @@ __device__ __forceinline__ void ldsm_x4_trans(uint32_t addr, uint32_t &r0, uint3
                  : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
                  : "r"(addr));
 }
-// D(16x8,f32) += A(16x16,f16,row) * B(16x8,f16,col); rows 8..15 of A are zero (a1 = a3 = 0): G <= 8 heads
-__device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a2, uint32_t b0, uint32_t b1) {
-    const uint32_t z = 0u;
+// D(16x8,f32) += A(16x16,f16,row) * B(16x8,f16,col)
+__device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
+                                         uint32_t b1) {
     asm volatile(
         "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
         : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-        : "r"(a0), "r"(z), "r"(a2), "r"(z), "r"(b0), "r"(b1));
+        : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+// transpose an 8x8 matrix of 16-bit elements held as one C / A-style fragment register per lane
+__device__ __forceinline__ uint32_t movmatrix_trans(uint32_t x) {
+    uint32_t y;
+    asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(y) : "r"(x));
+    return y;
 }
 __device__ __forceinline__ float fast_exp2(float x) {
     float y;
@@ -222,21 +230,24 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) try_issue();
 
-        // ---- per-lane shared-memory offsets of the ldmatrix rows (128B hardware swizzle: chunk ^= row & 7) ----
-        const int l7 = lane & 7, mi = lane >> 3;
-        const uint32_t k_row = l7 * 128;
-        const uint32_t k_x0 = ((mi) ^ l7) << 4, k_x1 = ((4 + mi) ^ l7) << 4;
-        const uint32_t v_row = ((mi & 1) * 8 + l7) * 128;
-        const int v_c = mi >> 1;
-        const int qrow = lane >> 2, qcol = (lane & 3) * 2;
+        // ---- fragment addressing.  TOKENS are the M rows of both MMAs (S^T = K Q^T, O^T = V^T P^T), the <= 8 query
+        //      heads of the group are the N = 8 columns: no padding rows for G = 8, half as many HMMAs and accumulator
+        //      registers as heads-as-M.  128B hardware swizzle: 16-byte chunk index ^= row & 7. ----
+        const int l7 = lane & 7;
+        const uint32_t ka_row = (l7 + ((lane >> 3) & 1) * 8) * 128;  // K as A operand (ldmatrix x4: matrix lane / 8)
+        const int ka_kc = lane >> 4;                                  // which 8-half chunk of the 16-wide k-step
+        const uint32_t va_row = (l7 + (lane >> 4) * 8) * 128;         // V as A operand through ldmatrix.trans
+        const int va_dc = (lane >> 3) & 1;                            // which 8-wide half of the 16 output dims
+        const int tq = lane >> 2;                                     // C fragments: token rows tq, tq + 8; B: head
+        const int hp = (lane & 3) * 2;                                // C fragments: heads hp, hp + 1
 
         // ---- compute cursor ------------------------------------------------------------------------------
         int cu = 0, ct = 0, c_left = 0, piece = 0, c_cnt = 0;
         Unit cun;
         cun.cnt = 0;
-        uint32_t qa[8][2];  // A fragments of Q: [k-step][a0, a2]
-        float o[16][4];
-        float m_run = -INFINITY, l_run = 0.f;
+        uint32_t qb[8][2];  // B fragments of Q^T: [k-step][b0, b1] = Q[head tq][16 ks + hp, +1] and [.. + 8, +9]
+        float o[8][4];      // O^T: [16-dim tile][c0..c3] = (dim 16 mt + tq, heads hp, hp+1), (dim + 8, heads hp, hp+1)
+        float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;  // reference maximum (base 2) and row sum of heads hp, hp+1
 
         while (consumed < issued) {
             if (c_left == 0) {
@@ -250,16 +261,16 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
                 piece = c4.w;
                 cun = load_unit(d.units, cu);
                 c_cnt = live_cnt(d, cun);
-                const __half *qg = p.q + ((size_t)cun.req * d.Hq + (size_t)(cu % Hkv) * G + qrow) * kHeadDim + qcol;
+                const __half *qg = p.q + ((size_t)cun.req * d.Hq + (size_t)(cu % Hkv) * G + tq) * kHeadDim + hp;
 #pragma unroll
                 for (int ks = 0; ks < 8; ++ks) {
-                    qa[ks][0] = qrow < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16)) : 0u;
-                    qa[ks][1] = qrow < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16 + 8)) : 0u;
+                    qb[ks][0] = tq < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16)) : 0u;
+                    qb[ks][1] = tq < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16 + 8)) : 0u;
                 }
-                m_run = -INFINITY;
-                l_run = 0.f;
+                m0 = m1 = -INFINITY;
+                l0 = l1 = 0.f;
 #pragma unroll
-                for (int n = 0; n < 16; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
+                for (int n = 0; n < 8; ++n) o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f;
             }
             const int stage = consumed % STAGES;
             const uint32_t sb = wbase + stage * kStageBytes;
@@ -278,58 +289,61 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
                 __syncwarp();
             }
 
-            // ---- S = Q K^T : 16 (heads, padded) x 16 tokens ------------------------------------------------
-            float s[2][4];
+            // ---- S^T = K Q^T : 16 tokens x 8 heads; two accumulators (even / odd k-steps) halve the HMMA chain ----
+            float sa[4] = {0.f, 0.f, 0.f, 0.f}, sc[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-            for (int j = 0; j < 2; ++j) s[j][0] = s[j][1] = s[j][2] = s[j][3] = 0.f;
-#pragma unroll
-            for (int ii = 0; ii < 4; ++ii) {
-#pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    uint32_t b0, b1, b2, b3;
-                    ldsm_x4(sb + (ii >> 1) * kSubTile + j * 1024 + k_row + ((ii & 1) ? k_x1 : k_x0), b0, b1, b2, b3);
-                    mma16816(s[j], qa[2 * ii][0], qa[2 * ii][1], b0, b1);
-                    mma16816(s[j], qa[2 * ii + 1][0], qa[2 * ii + 1][1], b2, b3);
-                }
+            for (int ks = 0; ks < 8; ++ks) {
+                uint32_t a0, a1, a2, a3;
+                ldsm_x4(sb + (ks >> 2) * kSubTile + ka_row + (((((ks & 3) << 1) + ka_kc) ^ l7) << 4), a0, a1, a2, a3);
+                mma16816(ks & 1 ? sc : sa, a0, a1, a2, a3, qb[ks][0], qb[ks][1]);
             }
 
-            // ---- online softmax on row `qrow` (c0, c1 of each n-tile), base 2 ------------------------------
-            float mx = -INFINITY;
+            // ---- online softmax, base 2, per head column; the reference maximum is LAZY: it only moves (and the
+            //      accumulators are only rescaled) when a score exceeds it by more than 2^kLazy, so the cross-lane
+            //      maximum and the rescale cost nothing on most tiles; p = exp2(s - m + kPShift) <= 2^(kLazy + kPShift)
 #pragma unroll
-            for (int j = 0; j < 2; ++j) {
+            for (int i = 0; i < 4; ++i) sc[i] = (sa[i] + sc[i]) * d.scale_log2;
+            if (ragged) {
+                if (tq >= valid) sc[0] = sc[1] = -INFINITY;
+                if (tq + 8 >= valid) sc[2] = sc[3] = -INFINITY;
+            }
+            const float t0 = fmaxf(sc[0], sc[2]), t1 = fmaxf(sc[1], sc[3]);
+            if (__any_sync(0xffffffffu, t0 > m0 + kLazy || t1 > m1 + kLazy)) {
+                float x0 = t0, x1 = t1;
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const float v = s[j][e] * d.scale_log2;
-                    s[j][e] = (8 * j + qcol + e < valid) ? v : -INFINITY;
-                    mx = fmaxf(mx, s[j][e]);
+                for (int sh = 4; sh < 32; sh <<= 1) {
+                    x0 = fmaxf(x0, __shfl_xor_sync(0xffffffffu, x0, sh));
+                    x1 = fmaxf(x1, __shfl_xor_sync(0xffffffffu, x1, sh));
+                }
+                const float n0 = fmaxf(m0, x0), n1 = fmaxf(m1, x1);
+                const float al0 = fast_exp2(m0 - n0), al1 = fast_exp2(m1 - n1);
+                m0 = n0;
+                m1 = n1;
+                l0 *= al0;
+                l1 *= al1;
+#pragma unroll
+                for (int n = 0; n < 8; ++n) {
+                    o[n][0] *= al0;
+                    o[n][1] *= al1;
+                    o[n][2] *= al0;
+                    o[n][3] *= al1;
                 }
             }
-            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
-            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
-            const float m_new = fmaxf(m_run, mx);
-            const float alpha = fast_exp2(m_run - m_new);
-            const float m_off = m_new - kPShift;
-            const float p00 = fast_exp2(s[0][0] - m_off), p01 = fast_exp2(s[0][1] - m_off);
-            const float p10 = fast_exp2(s[1][0] - m_off), p11 = fast_exp2(s[1][1] - m_off);
-            l_run = l_run * alpha + ((p00 + p01) + (p10 + p11));
-            m_run = m_new;
-            if (__any_sync(0xffffffffu, alpha != 1.f)) {
-#pragma unroll
-                for (int n = 0; n < 16; ++n) {
-                    o[n][0] *= alpha;
-                    o[n][1] *= alpha;
-                }
-            }
-            const uint32_t pa0 = pack_half2(p00, p01), pa2 = pack_half2(p10, p11);
+            const float f0 = m0 - kPShift, f1 = m1 - kPShift;
+            const float p0 = fast_exp2(sc[0] - f0), p1 = fast_exp2(sc[1] - f1);
+            const float p2 = fast_exp2(sc[2] - f0), p3 = fast_exp2(sc[3] - f1);
+            l0 += p0 + p2;
+            l1 += p1 + p3;
+            // P (tokens x heads, C-fragment layout) -> B fragments of P^T... of the product O^T = V^T P: movmatrix
+            const uint32_t pb0 = movmatrix_trans(pack_half2(p0, p1)), pb1 = movmatrix_trans(pack_half2(p2, p3));
 
-            // ---- O += P V : 16 x 128 -----------------------------------------------------------------------
+            // ---- O^T += V^T P : 128 dims x 8 heads -----------------------------------------------------------
 #pragma unroll
-            for (int nd = 0; nd < 16; nd += 2) {
-                uint32_t b0, b1, b2, b3;
-                ldsm_x4_trans(sb + 2 * kSubTile + (nd >> 3) * kSubTile + v_row + ((((nd & 7) + v_c) ^ l7) << 4), b0, b1,
-                              b2, b3);
-                mma16816(o[nd], pa0, pa2, b0, b1);
-                mma16816(o[nd + 1], pa0, pa2, b2, b3);
+            for (int mt = 0; mt < 8; ++mt) {
+                uint32_t a0, a1, a2, a3;
+                ldsm_x4_trans(sb + (2 + (mt >> 2)) * kSubTile + va_row + (((((mt & 3) << 1) + va_dc) ^ l7) << 4), a0, a1, a2,
+                              a3);
+                mma16816(o[mt], a0, a1, a2, a3, pb0, pb1);
             }
 
             // the zero-stores above went through the generic proxy: every lane that wrote orders them before the
@@ -344,23 +358,36 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
             if (c_left == 0) {
                 // ---- end of the piece: emit its partial (o, lse) -------------------------------------------
                 const int g = cu % Hkv;
-                float lt = l_run + __shfl_xor_sync(0xffffffffu, l_run, 1);
-                lt += __shfl_xor_sync(0xffffffffu, lt, 2);
+                float lt0 = l0, lt1 = l1;
+#pragma unroll
+                for (int sh = 4; sh < 32; sh <<= 1) {
+                    lt0 += __shfl_xor_sync(0xffffffffu, lt0, sh);
+                    lt1 += __shfl_xor_sync(0xffffffffu, lt1, sh);
+                }
                 const PieceDest pd = piece_dest(p, cun, cu, g, piece);
-                if (qrow < G) {
-                    const float inv = 1.f / lt;
-                    float *dst = pd.o + (size_t)qrow * kHeadDim + qcol;
+                const float inv0 = 1.f / lt0, inv1 = 1.f / lt1;
+                const float lse0 = (m0 + log2f(lt0) - kPShift) * 0.6931471805599453f;
+                const float lse1 = (m1 + log2f(lt1) - kPShift) * 0.6931471805599453f;
 #pragma unroll
-                    for (int n = 0; n < 16; ++n)
-                        *reinterpret_cast<float2 *>(dst + 8 * n) = make_float2(o[n][0] * inv, o[n][1] * inv);
-                    const float lse = (m_run + log2f(lt) - kPShift) * 0.6931471805599453f;
-                    if ((lane & 3) == 0) pd.lse[qrow] = lse;
-                    if (pd.o2) {
-                        float *dst2 = pd.o2 + (size_t)qrow * kHeadDim + qcol;
+                for (int e = 0; e < 2; ++e) {
+                    if (hp + e < G) {
+                        const float inv = e ? inv1 : inv0;
+                        float *dst = pd.o + (size_t)(hp + e) * kHeadDim + tq;
 #pragma unroll
-                        for (int n = 0; n < 16; ++n)
-                            *reinterpret_cast<float2 *>(dst2 + 8 * n) = make_float2(o[n][0] * inv, o[n][1] * inv);
-                        if ((lane & 3) == 0) pd.lse2[qrow] = lse;
+                        for (int n = 0; n < 8; ++n) {
+                            dst[16 * n] = o[n][e] * inv;
+                            dst[16 * n + 8] = o[n][2 + e] * inv;
+                        }
+                        if (tq == 0) pd.lse[hp + e] = e ? lse1 : lse0;
+                        if (pd.o2) {
+                            float *dst2 = pd.o2 + (size_t)(hp + e) * kHeadDim + tq;
+#pragma unroll
+                            for (int n = 0; n < 8; ++n) {
+                                dst2[16 * n] = o[n][e] * inv;
+                                dst2[16 * n + 8] = o[n][2 + e] * inv;
+                            }
+                            if (tq == 0) pd.lse2[hp + e] = e ? lse1 : lse0;
+                        }
                     }
                 }
                 if (p.fused) piece_done(p, ctr, cu, cun, g, lane);
@@ -409,7 +436,7 @@ static int launch_one(const AttendParams &p, int n_ctas, cudaStream_t s) {
     return 1;
 }
 
-#define KF_TMA_SHAPES(X) X(4, 2) X(4, 3) X(4, 4) X(4, 5) X(4, 6) X(8, 2) X(8, 3)
+#define KF_TMA_SHAPES(X) X(4, 2) X(4, 3) X(4, 4) X(4, 5) X(4, 6) X(8, 2) X(8, 3) X(12, 2) X(16, 1)
 
 bool attend_tma_shape_ok(int warps, int stages) {
 #define X(Wp, St) \

@@ -13,8 +13,8 @@ namespace kf {
 constexpr int kHeadDim = 128;
 constexpr int kTileTokens = 16;       // work-plan granule = one MMA k-step of tokens
 constexpr int kWarpsPerCta = 8;       // default workers (warps) per CTA; one worker = one warp
-constexpr int kMaxWarpsPerCta = 8;
-constexpr int kMaxWorkers = 2048;     // >= SMs * kMaxWarpsPerCta on any Blackwell part (148 * 8 = 1184)
+constexpr int kMaxWarpsPerCta = 16;
+constexpr int kMaxWorkers = 2560;     // >= SMs * kMaxWarpsPerCta on any Blackwell part (148 * 16 = 2368)
 constexpr int kMaxLevels = 16;        // levels of the guided self-scheduling chunk list
 constexpr int kChunkSlack = 16 * kMaxWorkers;  // chunk capacity = units + kChunkSlack
 constexpr int kMaxGroup = 8;          // G = H_q / H_kv
