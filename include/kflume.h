@@ -209,6 +209,14 @@ int kf_attend(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, f
  *   (the step boundary; a request waiting for a slot stays where it is, see kf_token_boundary). */
 int kf_step_commit(kf_ctx *ctx, kf_stream stream);
 
+/* (a2+a3+a4) kf_layer_step -- one layer-step in ONE launch: kf_kv_append(k_new, v_new) followed by kf_attend(q, ...),
+ *   same arguments, same results, same device errors.  With the TMA kernel the append rides in the attend launch: the
+ *   worker that attends the tail tile of (request, kv head) writes the new K/V row to the pool and patches it into its
+ *   shared-memory copy of that tile (the tail node "appends (K_new, V_new), then computes attention");
+ *   the static step graph uses the same launch.  With KF_IMPL_SIMPLE it is the two launches one after the other. */
+int kf_layer_step(kf_ctx *ctx, int32_t layer, const void *q, const void *k_new, const void *v_new, float *o, float *lse,
+                  float *o_part, float *lse_part, kf_stream stream);
+
 /* One layer-step with HOST buffers (end-to-end path): q / k_new / v_new [host, fp16, shapes as above] in,
  * o [B][H_q][128] and lse [B][H_q] (fp32) out [host].  With PINNED host memory (16-byte aligned) nothing is copied
  * by a copy engine: the append kernel reads k_new / v_new over the bus and stages q, kf_attend writes o / lse
@@ -223,6 +231,8 @@ int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const voi
  * fixed grid and reads lengths, routes and the work plan from device memory, so ONE captured graph of
  *     kf_token_boundary -> for i < n: { kf_kv_append(layers[i], k_new[i], v_new[i]);
  *                                       kf_attend(layers[i], q[i], o[i], lse[i]) } -> kf_step_commit
+ * (device buffers + TMA kernel: n + 1 kernel nodes -- each layer-step is the single launch of kf_layer_step, the commit
+ * rides in the last one)
  * is replayed for every decode step, across range fills, route updates and kf_open/close_request, without
  * re-capture.  A replay also removes the submission latency between the small kernels of a step.
  * kf_step_graph_create: captures on `stream` (must not be the legacy default stream; nothing executes) and

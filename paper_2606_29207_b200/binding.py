@@ -16,7 +16,7 @@ KF_IMPL_AUTO, KF_IMPL_SIMPLE, KF_IMPL_TMA = 0, 1, 2
 EXPORTS = [
     "kf_version", "kf_strerror", "kf_last_cuda_error", "kf_pool_bytes", "kf_workspace_bytes", "kf_pool_offset",
     "kf_create", "kf_destroy", "kf_open_request", "kf_close_request", "kf_load_context", "kf_token_boundary",
-    "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_step_commit", "kf_layer_step_host",
+    "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_step_commit", "kf_layer_step", "kf_layer_step_host",
     "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count", "kf_worker_times",
     "kf_step_graph_create", "kf_step_graph_launch", "kf_step_graph_destroy", "kf_probe_read",
     "kf_step_graph_flags", "kf_step_graph_seq", "kf_step_graph_release", "kf_signal_roundtrip",
@@ -94,6 +94,7 @@ def load_library():
     L.kf_merge_partials.argtypes = [vp, vp, vp, vp, vp, vp]
     L.kf_attend.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
     L.kf_step_commit.argtypes = [vp, vp]
+    L.kf_layer_step.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
     L.kf_layer_step_host.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
     L.kf_route_snapshot.argtypes = [vp] + [ctypes.POINTER(i32)] * 6 + [vp]
     L.kf_status.argtypes = [vp, vp]
@@ -280,6 +281,16 @@ class KFlume:
 
     def step_commit(self, stream=None):
         self._check(self.lib.kf_step_commit(self.h, self._stream(stream)), "kf_step_commit")
+
+    def layer_step(self, layer: int, q, k_new, v_new, o, lse, o_part=None, lse_part=None, stream=None):
+        if o_part is not None:
+            self._f32(o_part, (self.B, self.Jmax, self.Hq, 128))
+            self._f32(lse_part, (self.B, self.Jmax, self.Hq))
+        shp = (self.B, self.Hkv, 128)
+        self._check(self.lib.kf_layer_step(self.h, layer, self._f16(q, (self.B, self.Hq, 128)), self._f16(k_new, shp),
+                                           self._f16(v_new, shp), self._f32(o, (self.B, self.Hq, 128)),
+                                           self._f32(lse, (self.B, self.Hq)), _ptr(o_part), _ptr(lse_part),
+                                           self._stream(stream)), "kf_layer_step")
 
     def layer_step_host(self, layer: int, q_host, k_new_host, v_new_host, o_host, lse_host, stream=None):
         for t in (q_host, k_new_host, v_new_host, o_host, lse_host):

@@ -41,7 +41,7 @@ size_t max_chunks_of(const kf_config *c) {
 inline size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t len, n_ranges, route_part, route_slot, rr_cursor, rr_last, req_active, active, part_tokens, part_tails, free_head, free_cnt, free_stack, error, plan, units, chunks, plan_age, sched,
+    size_t len, n_ranges, route_part, route_slot, rr_cursor, rr_last, req_active, active, part_tokens, part_tails, free_head, free_cnt, free_stack, error, plan, units, chunks, recs, plan_age, sched,
         scratch, unit_counter, group_counter, piece_o, piece_lse, range_o, range_lse, stage_q, stage_k, stage_v,
         stage_o, stage_lse, tmaps, gates, worker_times, total;
 };
@@ -107,6 +107,7 @@ Layout make_layout(const kf_config *c) {
     L.plan = take(sizeof(PlanHeader));
     L.units = take(U * sizeof(Unit));
     L.chunks = take(max_piece_slots * sizeof(Chunk));
+    L.recs = take(max_piece_slots * sizeof(ChunkRec));
     L.plan_age = take(4);
     L.sched = take(8 * 4);
     L.scratch = take((B + B + (B + 1) + E + (E + 1) + (E + 1) + 3 * ((size_t)kMaxLevels * E + 1)) * 4);
@@ -330,6 +331,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.plan = (PlanHeader *)(ws + L.plan);
     d.units = (Unit *)(ws + L.units);
     d.chunks = (Chunk *)(ws + L.chunks);
+    d.recs = (ChunkRec *)(ws + L.recs);
     d.plan_age = (int32_t *)(ws + L.plan_age);
     d.sched = (int32_t *)(ws + L.sched);
     d.scratch = (int32_t *)(ws + L.scratch);
@@ -426,6 +428,8 @@ int kf_partial_attend(kf_ctx *ctx, int32_t layer, const void *q, const uint8_t *
     ap.lse = nullptr;
     ap.fused = 0;
     ap.commit = 0;
+    ap.k_new = nullptr;
+    ap.v_new = nullptr;
     ap.part_mask = 0;
     for (int p = 0; p < ctx->cfg.n_partitions; ++p)
         if (!partition_mask || partition_mask[p]) ap.part_mask |= 1ull << p;
@@ -443,8 +447,10 @@ int kf_merge_partials(kf_ctx *ctx, const float *o_part, const float *lse_part, f
 }
 
 int kf_attend_impl(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, float *o_part, float *lse_part,
-                   int commit, kf_stream stream) {
+                   int commit, const void *k_new, const void *v_new, kf_stream stream) {
     if (!ctx || bad_layer(ctx, layer) || !q || !o || !lse || ((uintptr_t)q & 15) || ((uintptr_t)o & 15)) return KF_EINVAL;
+    if ((k_new == nullptr) != (v_new == nullptr) || ((uintptr_t)k_new & 15) || ((uintptr_t)v_new & 15)) return KF_EINVAL;
+    if (k_new && ctx->impl != KF_IMPL_TMA) return KF_EINVAL;  // only the TMA kernel carries the fused append
     if ((o_part == nullptr) != (lse_part == nullptr) || ((uintptr_t)o_part & 15)) return KF_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_plan(ctx, s);
@@ -460,6 +466,8 @@ int kf_attend_impl(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *l
     ap.fused = 1;
     ap.commit = commit;
     ap.part_mask = ~0ull;
+    ap.k_new = (const __half *)k_new;
+    ap.v_new = (const __half *)v_new;
     rc = run_attend(ctx, ap, s);
     if (rc == KF_OK && commit) ctx->plan_dirty = true;  // lengths moved
     return rc;
@@ -467,7 +475,7 @@ int kf_attend_impl(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *l
 
 int kf_attend(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, float *o_part, float *lse_part,
               kf_stream stream) {
-    return kf_attend_impl(ctx, layer, q, o, lse, o_part, lse_part, 0, stream);
+    return kf_attend_impl(ctx, layer, q, o, lse, o_part, lse_part, 0, nullptr, nullptr, stream);
 }
 
 int kf_step_commit(kf_ctx *ctx, kf_stream stream) {
@@ -490,21 +498,32 @@ int kf_layer_step_host_impl(kf_ctx *ctx, int32_t layer, const void *q_host, cons
         int rc = after_launch(ctx, launch_kv_append_stage(d, layer, (const __half *)k_new_host, (const __half *)v_new_host,
                                                           (const __half *)q_host, d.stage_q, s));
         if (rc != KF_OK) return rc;
-        return kf_attend_impl(ctx, layer, d.stage_q, o_host, lse_host, nullptr, nullptr, commit, stream);
+        return kf_attend_impl(ctx, layer, d.stage_q, o_host, lse_host, nullptr, nullptr, commit, nullptr, nullptr, stream);
     }
     const size_t qb = (size_t)d.B * d.Hq * kHeadDim * 2, kb = (size_t)d.B * d.Hkv * kHeadDim * 2;
     cudaError_t e = cudaMemcpyAsync(d.stage_q, q_host, qb, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d.stage_k, k_new_host, kb, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d.stage_v, v_new_host, kb, cudaMemcpyHostToDevice, s);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
-    int rc = kf_kv_append(ctx, layer, d.stage_k, d.stage_v, stream);
+    const bool fused = ctx->impl == KF_IMPL_TMA;  // the append rides in the attend launch
+    int rc = fused ? KF_OK : kf_kv_append(ctx, layer, d.stage_k, d.stage_v, stream);
     if (rc != KF_OK) return rc;
-    rc = kf_attend_impl(ctx, layer, d.stage_q, d.stage_o, d.stage_lse, nullptr, nullptr, commit, stream);
+    rc = kf_attend_impl(ctx, layer, d.stage_q, d.stage_o, d.stage_lse, nullptr, nullptr, commit,
+                        fused ? d.stage_k : nullptr, fused ? d.stage_v : nullptr, stream);
     if (rc != KF_OK) return rc;
     e = cudaMemcpyAsync(o_host, d.stage_o, (size_t)d.B * d.Hq * kHeadDim * 4, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(lse_host, d.stage_lse, (size_t)d.B * d.Hq * 4, cudaMemcpyDeviceToHost, s);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     return KF_OK;
+}
+
+int kf_layer_step(kf_ctx *ctx, int32_t layer, const void *q, const void *k_new, const void *v_new, float *o, float *lse,
+                  float *o_part, float *lse_part, kf_stream stream) {
+    if (!ctx || !k_new || !v_new) return KF_EINVAL;
+    if (ctx->impl == KF_IMPL_TMA) return kf_attend_impl(ctx, layer, q, o, lse, o_part, lse_part, 0, k_new, v_new, stream);
+    const int rc = kf_kv_append(ctx, layer, k_new, v_new, stream);
+    if (rc != KF_OK) return rc;
+    return kf_attend_impl(ctx, layer, q, o, lse, o_part, lse_part, 0, nullptr, nullptr, stream);
 }
 
 int kf_layer_step_host(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host, const void *v_new_host,

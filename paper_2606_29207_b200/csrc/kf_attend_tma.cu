@@ -24,7 +24,6 @@ namespace kf {
 
 constexpr int kSubTile = kTileTokens * 128;     // 16 rows x 128 B (64 halfs): one TMA box
 constexpr int kStageBytes = 4 * kSubTile;       // K lo | K hi | V lo | V hi = 8 KB
-constexpr int kTicketAhead = 3;                 // tiles before the end of a chunk at which the next ticket is taken
 constexpr int kRing = 8;                        // chunk descriptors in flight between the load and compute cursors
 // P is rounded to fp16 for the P.V MMA.  With p = exp2(s - m) in (0, 1] every weight below 2^-25 would flush to zero
 // there while the fp32 row sum l keeps it: on a long, peaked context (1M tokens, each 2^-25 below the maximum) that
@@ -128,12 +127,18 @@ __device__ __forceinline__ Unit load_unit(const Unit *units, int u) {
 }
 
 
+// Ring slot handed from a worker's load cursor to its compute cursor: the chunk's record with the live tile / token
+// counts filled in.  Word layout = ChunkRec; pad[0] = 1 when the chunk's q rows were staged into the warp's q slot.
+constexpr int kQRowBytes = kHeadDim * 2 + 16;  // q rows in shared memory, padded: B-fragment loads hit 32 distinct banks
+constexpr int kPfStart = 3;                    // the next chunk is requested when this many tiles of the current one are left
+
 template <int WARPS, int STAGES>
 __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendParams p) {
     constexpr int kWarpSmem = STAGES * kStageBytes;
     extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bars[WARPS][STAGES];
-    __shared__ int4 ring[WARPS][kRing];
+    __shared__ __align__(16) int4 ring[WARPS][kRing][4];
+    __shared__ __align__(16) unsigned char q_stage[WARPS][kMaxGroup * kQRowBytes];
     const Dev &d = p.d;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = gridDim.x * WARPS;
@@ -141,7 +146,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
     const int n_chunks = __ldg(&d.plan->n_pieces);
     const long long t_start = d.diag ? global_ns() : 0;
     long long t_first = 0, t_stream = 0;
-    const Counters ctr = launch_prologue(d, w, W, lane);
+    Counters ctr;
     int m_first = -1;  // lane 0: pre-taken first merge ticket
 
     if (w < n_chunks) {
@@ -159,45 +164,95 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
         uint64_t policy = 0;  // K/V is read once per launch: evict-first keeps the partials resident in L2
         asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
         const unsigned char *tmaps = reinterpret_cast<const unsigned char *>(d.tmaps);
+        const int layer_row = p.layer * d.slots * Hkv * d.R;
+        const uint32_t q_s = smem_u32(&q_stage[warp][0]);
 
-        // ---- load cursor: runs up to STAGES tiles ahead of the compute cursor, across chunk boundaries ----
+        // ---- load cursor: runs up to STAGES tiles ahead of the compute cursor, across chunk boundaries.  The NEXT
+        //      chunk is fetched in the background, one step per issued tile: ticket (atomic) -> 64-byte record (one
+        //      coalesced load by lanes 0..3) -> ring slot in shared memory; by the time the current chunk runs out,
+        //      its successor is a shared-memory read away. ----
         int issued = 0, consumed = 0;
         int l_left = 0, l_row = 0, l_part = 0;
         int ring_w = 0, ring_r = 0;
-        int pre = 0;  // lane 0: ticket of the dynamic part of the chunk list, taken shortly before it is needed
-        bool l_first = true, l_done = false, has_pre = false;
-        auto grab = [&]() -> bool {
-            for (;;) {
-                int id;
-                if (l_first) {
-                    id = w;  // the first W chunks are handed out statically: no atomic storm at launch
-                    l_first = false;
-                } else {
-                    if (!has_pre && lane == 0) pre = atomicAdd(d.sched, 1);
-                    has_pre = false;
-                    id = W + __shfl_sync(0xffffffffu, pre, 0);
+        int pf_state = 1, pf_id = w;  // 0 idle | 1 ticket requested (pf_id valid: the first chunk is static) | 2 record requested | 3 record in the ring
+        int pf_tk = 0;                // lane 0: the ticket
+        bool pf_static = true;        // pf_id already holds the chunk id (worker w starts with chunk w: no atomic storm)
+        int4 pf_rec = make_int4(0, 0, 0, 0);
+        bool l_done = false, q_busy = false;
+        auto pf_step = [&]() {
+            if (pf_state == 0) {
+                if (lane == 0) pf_tk = atomicAdd(d.sched, 1);
+                pf_state = 1;
+            } else if (pf_state == 1) {
+                if (!pf_static) pf_id = W + __shfl_sync(0xffffffffu, pf_tk, 0);
+                pf_static = false;
+                if (pf_id < n_chunks) {
+                    if (lane < 4) pf_rec = __ldg(reinterpret_cast<const int4 *>(d.recs + pf_id) + lane);
+                } else if (p.fused && lane == 0 && m_first < 0) {
+                    m_first = merge_first_ticket(d, W);  // nothing left to load: reserve the first merge tasks now
                 }
-                if (id >= n_chunks) {
+                pf_state = 2;
+            } else if (pf_state == 2) {
+                if (pf_id < n_chunks && lane < 4) ring[warp][ring_w & (kRing - 1)][lane] = pf_rec;
+                __syncwarp();
+                pf_state = 3;
+            }
+        };
+        // next chunk -> load cursor; false when the list is exhausted
+        auto advance = [&]() -> bool {
+            for (;;) {
+                while (pf_state < 3) pf_step();
+                pf_state = 0;
+                if (pf_id >= n_chunks) {
                     l_done = true;
-                    // nothing left to load: reserve the first merge tasks now, STAGES tiles before they are needed
-                    if (p.fused && lane == 0) m_first = merge_first_ticket(d, W);
                     return false;
                 }
-                int4 c4 = __ldg(reinterpret_cast<const int4 *>(d.chunks + id));
-                const Unit un = load_unit(d.units, c4.x);
-                if (!((p.part_mask >> un.part) & 1ull)) continue;  // partition not selected: nothing to load
-                if (un.tail) c4.z = live_tiles(un, live_cnt(d, un), c4.y, c4.z);  // the plan may be older than this step
-                l_left = c4.z;
-                l_part = un.part;
-                l_row = ((p.layer * d.slots + un.slot) * Hkv + (c4.x % Hkv)) * d.R + c4.y * kTileTokens;
-                if (lane == 0) ring[warp][ring_w & (kRing - 1)] = c4;
+                int4 *slot = ring[warp][ring_w & (kRing - 1)];
+                const int4 a = slot[0], b = slot[1], c = slot[2];  // {unit, tile_begin, n_tiles, piece} {part, row0, req, range} {cnt, flags, n_pieces, J}
+                if (!((p.part_mask >> b.x) & 1ull)) continue;     // partition not selected: nothing to load
+                int n_tiles = a.z, cnt = c.x, app = -1;
+                if (c.y & kRecTail) {  // the plan may be older than this step: a tail unit has grown since
+                    const int raw = __ldg(d.len + b.z) + 1 - b.w * d.R;  // tokens of the tail range, this step's included
+                    cnt = min(d.R, raw);
+                    if (c.y & kRecStretch) {
+                        n_tiles = (cnt + kTileTokens - 1) / kTileTokens - a.y;
+                        if (p.k_new) {  // fused (a2): this chunk ends with the tile that receives the new token
+                            if (raw <= d.R)
+                                app = raw - 1;
+                            else if (lane == 0)
+                                set_error(d, KF_ESTATE);  // no route for the tail position (the request waits for a slot)
+                        }
+                    }
+                }
+                // q rows of the chunk's head group -> the warp's q slot (if the previous chunk has picked its q up)
+                const bool stage_q = !q_busy;
+                if (stage_q) {
+                    const unsigned char *qg =
+                        reinterpret_cast<const unsigned char *>(p.q + ((size_t)b.z * d.Hq + (size_t)(a.x % Hkv) * G) * kHeadDim);
+                    for (int i = lane; i < G * 16; i += 32) {
+                        const uint32_t dst = q_s + (i >> 4) * kQRowBytes + (i & 15) * 16;
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(qg + (size_t)i * 16) : "memory");
+                    }
+                    asm volatile("cp.async.commit_group;" ::: "memory");
+                    q_busy = true;
+                }
+                __syncwarp();  // every lane has read the slot
+                if (lane == 0) {
+                    slot[0].z = n_tiles;
+                    slot[2].x = cnt;
+                    slot[3].x = stage_q ? 1 : 0;
+                    slot[3].y = app;
+                }
+                l_left = n_tiles;
+                l_part = b.x;
+                l_row = layer_row + b.y;
                 ++ring_w;
                 return true;
             }
         };
         auto try_issue = [&]() {
             if (l_done) return;
-            if (l_left == 0 && !grab()) return;
+            if (l_left == 0 && !advance()) return;
             if (lane == 0) {
                 const int stage = issued % STAGES;
                 const uint32_t sb = wbase + stage * kStageBytes, bar = bar0 + 8 * stage;
@@ -218,17 +273,13 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
             l_row += kTileTokens;
             --l_left;
             ++issued;
-            // take the next ticket a few tiles before the end of this chunk: late enough that a slow worker does
-            // not reserve work long before it can start it, early enough to hide the atomic's round trip
-            if (l_left == kTicketAhead - 1 || (l_left < kTicketAhead - 1 && !has_pre && l_left >= 0)) {
-                if (!has_pre) {
-                    if (lane == 0) pre = atomicAdd(d.sched, 1);
-                    has_pre = true;
-                }
-            }
+            // late enough that a slow worker does not reserve work long before it can start it, early enough to hide
+            // the round trips of the atomic and of the record
+            if (l_left < kPfStart && pf_state < 3) pf_step();
         };
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) try_issue();
+        ctr = launch_prologue(d, w, W, lane);  // one more L2 round trip, now in the shadow of the first tiles
 
         // ---- fragment addressing.  TOKENS are the M rows of both MMAs (S^T = K Q^T, O^T = V^T P^T), the <= 8 query
         //      heads of the group are the N = 8 columns: no padding rows for G = 8, half as many HMMAs and accumulator
@@ -242,30 +293,70 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
         const int hp = (lane & 3) * 2;                                // C fragments: heads hp, hp + 1
 
         // ---- compute cursor ------------------------------------------------------------------------------
-        int cu = 0, ct = 0, c_left = 0, piece = 0, c_cnt = 0;
-        Unit cun;
-        cun.cnt = 0;
+        int cu = 0, ct = 0, c_left = 0, piece = 0, c_cnt = 0, c_req = 0, c_range = 0, c_np = 0, c_J = 0;
+        int c_app = -1, c_part = 0, c_row = 0;  // fused append: token offset of the new row in the unit (-1: none)
         uint32_t qb[8][2];  // B fragments of Q^T: [k-step][b0, b1] = Q[head tq][16 ks + hp, +1] and [.. + 8, +9]
         float o[8][4];      // O^T: [16-dim tile][c0..c3] = (dim 16 mt + tq, heads hp, hp+1), (dim + 8, heads hp, hp+1)
         float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;  // reference maximum (base 2) and row sum of heads hp, hp+1
+        // completion signal of the piece written last, deferred by one tile: the release fence then finds the partial's
+        // stores already performed instead of waiting ~1 us for them
+        int32_t *sig_ptr = nullptr;  // lane 0
+        int sig_val = 0;
+        bool sig_pending = false;    // warp-uniform
+        auto flush_signal = [&]() {
+            // release: barrier first, THEN lane 0 fences and publishes -- the fence is cumulative over the stores of
+            // the other lanes that the barrier ordered before it
+            __syncwarp();
+            if (lane == 0 && sig_pending) {
+                release_fence();
+                atomicAdd(sig_ptr, sig_val);
+            }
+            sig_pending = false;
+        };
 
         while (consumed < issued) {
             if (c_left == 0) {
                 // ---- next chunk (= one piece of one unit) ----
                 __syncwarp();
-                const int4 c4 = ring[warp][ring_r & (kRing - 1)];
+                const int4 *slot = ring[warp][ring_r & (kRing - 1)];
+                const int4 a = slot[0], b = slot[1], c = slot[2];
+                const int staged = slot[3].x;
+                c_app = slot[3].y;
+                c_part = b.x;
+                c_row = layer_row + b.y - a.y * kTileTokens;  // pool row of the unit's first token
                 ++ring_r;
-                cu = c4.x;
-                ct = c4.y;
-                c_left = c4.z;
-                piece = c4.w;
-                cun = load_unit(d.units, cu);
-                c_cnt = live_cnt(d, cun);
-                const __half *qg = p.q + ((size_t)cun.req * d.Hq + (size_t)(cu % Hkv) * G + tq) * kHeadDim + hp;
+                cu = a.x;
+                ct = a.y;
+                c_left = a.z;
+                piece = a.w;
+                c_req = b.z;
+                c_range = b.w;
+                c_cnt = c.x;
+                c_np = c.z;
+                c_J = c.w;
+                if (staged) {
+                    asm volatile("cp.async.wait_all;" ::: "memory");
+                    __syncwarp();
+                    const uint32_t qa = q_s + tq * kQRowBytes + hp * 2;
 #pragma unroll
-                for (int ks = 0; ks < 8; ++ks) {
-                    qb[ks][0] = tq < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16)) : 0u;
-                    qb[ks][1] = tq < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16 + 8)) : 0u;
+                    for (int ks = 0; ks < 8; ++ks) {
+                        uint32_t x0 = 0u, x1 = 0u;
+                        if (tq < G) {
+                            asm volatile("ld.shared.b32 %0, [%1];" : "=r"(x0) : "r"(qa + ks * 32));
+                            asm volatile("ld.shared.b32 %0, [%1];" : "=r"(x1) : "r"(qa + ks * 32 + 16));
+                        }
+                        qb[ks][0] = x0;
+                        qb[ks][1] = x1;
+                    }
+                    __syncwarp();  // every lane has its fragments: the slot may be refilled
+                    q_busy = false;
+                } else {
+                    const __half *qg = p.q + ((size_t)c_req * d.Hq + (size_t)(cu % Hkv) * G + tq) * kHeadDim + hp;
+#pragma unroll
+                    for (int ks = 0; ks < 8; ++ks) {
+                        qb[ks][0] = tq < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16)) : 0u;
+                        qb[ks][1] = tq < G ? __ldg(reinterpret_cast<const uint32_t *>(qg + ks * 16 + 8)) : 0u;
+                    }
                 }
                 m0 = m1 = -INFINITY;
                 l0 = l1 = 0.f;
@@ -278,8 +369,22 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
             if (d.diag && consumed == 0) t_first = global_ns();
 
             const int valid = min(kTileTokens, c_cnt - ct * kTileTokens);
-            const bool ragged = valid < kTileTokens;
-            if (ragged) {
+            const bool patched = c_app >= 0 && ct == (c_app >> 4);
+            const bool ragged = valid < kTileTokens || patched;
+            if (patched) {
+                // (a2) this tile receives the step's new token: lanes 0..15 carry the 16-byte chunks of its K row,
+                // lanes 16..31 those of its V row -- into the pool (what kf_kv_append does) and into this tile's
+                // shared-memory copy, whatever the TMA load found at that position
+                const int row = c_app & 15, is_v = lane >> 4, ch = lane & 15;
+                const int4 val = __ldg(reinterpret_cast<const int4 *>((is_v ? p.v_new : p.k_new) +
+                                                                      ((size_t)c_req * Hkv + cu % Hkv) * kHeadDim) + ch);
+                const uint32_t a = sb + (2 * is_v + (ch >> 3)) * kSubTile + row * 128 + (((ch & 7) ^ (row & 7)) << 4);
+                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(val.x), "r"(val.y), "r"(val.z), "r"(val.w) : "memory");
+                unsigned char *dst = d.pool[c_part] + (is_v ? d.v_off : 0) + ((size_t)c_row + c_app) * (kHeadDim * 2) + ch * 16;
+                *reinterpret_cast<int4 *>(dst) = val;
+                __syncwarp();
+            }
+            if (valid < kTileTokens) {
                 // rows >= valid hold whatever the pool holds (maybe NaN patterns): zero them in V so 0 * V = 0
                 for (int idx = lane; idx < (kTileTokens - valid) * 16; idx += 32) {
                     const int row = valid + (idx >> 4), rem = idx & 15;
@@ -351,6 +456,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
             if (ragged) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncwarp();  // every lane is done reading this stage
             try_issue();   // refills this very stage: issued == consumed + STAGES whenever it issues
+            if (sig_pending) flush_signal();
 
             ++consumed;
             ++ct;
@@ -364,7 +470,22 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
                     lt0 += __shfl_xor_sync(0xffffffffu, lt0, sh);
                     lt1 += __shfl_xor_sync(0xffffffffu, lt1, sh);
                 }
-                const PieceDest pd = piece_dest(p, cun, cu, g, piece);
+                PieceDest pd;
+                pd.o2 = nullptr;
+                pd.lse2 = nullptr;
+                if (c_np == 1) {
+                    const size_t row = range_row(d, c_req, c_range, g * G);
+                    pd.o = p.o_part + row * kHeadDim;
+                    pd.lse = p.lse_part + row;
+                    if (p.fused && c_J == 1) {  // this piece is the final result
+                        const size_t frow = (size_t)c_req * d.Hq + g * G;
+                        pd.o2 = p.o + frow * kHeadDim;
+                        pd.lse2 = p.lse + frow;
+                    }
+                } else {
+                    pd.o = d.piece_o + (size_t)piece * G * kHeadDim;
+                    pd.lse = d.piece_lse + (size_t)piece * G;
+                }
                 const float inv0 = 1.f / lt0, inv1 = 1.f / lt1;
                 const float lse0 = (m0 + log2f(lt0) - kPShift) * 0.6931471805599453f;
                 const float lse1 = (m1 + log2f(lt1) - kPShift) * 0.6931471805599453f;
@@ -390,10 +511,25 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
                         }
                     }
                 }
-                if (p.fused) piece_done(p, ctr, cu, cun, g, lane);
+                if (p.fused) {
+                    // publish: pieces of a cut unit count on the unit, a whole range partial counts G heads on its group
+                    if (c_np > 1) {
+                        sig_ptr = &ctr.unit[cu];
+                        sig_val = 1;
+                        sig_pending = true;
+                    } else if (c_J > 1) {
+                        sig_ptr = &ctr.group[c_req * Hkv + g];
+                        sig_val = G;
+                        sig_pending = true;
+                    }
+                    if (sig_pending && consumed == issued) flush_signal();  // nothing left to hide it behind
+                }
             }
         }
+        if (sig_pending) flush_signal();
         if (d.diag) t_stream = global_ns();
+    } else {
+        ctr = launch_prologue(d, w, W, lane);
     }
     if (p.fused) merge_phase(p, ctr, W, lane, m_first);
 

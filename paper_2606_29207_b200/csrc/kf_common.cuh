@@ -45,6 +45,23 @@ struct Chunk {
     int32_t piece;      // global piece index (unit-major)
 };
 
+// The same chunk as the TMA kernel wants it: ONE 64-byte record holds everything its load cursor (route, first pool
+// row, tile count) and its compute cursor (request, head group, token count, piece bookkeeping, J_r) need, so a
+// worker that has a ticket is one L2 load away from its first TMA -- no dependent chunk -> unit -> length chain.
+struct alignas(64) ChunkRec {
+    int32_t unit, tile_begin, n_tiles, piece;  // as in Chunk
+    int32_t part;      // partition that holds the unit's range
+    int32_t row0;      // pool row of the chunk's first token in physical layer 0: (slot * H_kv + g) * R + tile_begin * 16
+    int32_t req, range;
+    int32_t cnt;       // tokens of the unit when the plan was built
+    int32_t flags;     // kRecTail: the unit is its request's last range; kRecStretch: this chunk holds the planned
+                       // last tile of a tail unit -- the one chunk that grows while the plan is kept (live_tiles())
+    int32_t n_pieces;  // pieces of the unit
+    int32_t J;         // ranges of the request in this plan
+    int32_t pad[4];
+};
+constexpr int kRecTail = 1, kRecStretch = 2;
+
 struct PlanHeader {
     int32_t n_units;
     int32_t n_tiles;
@@ -87,6 +104,7 @@ struct Dev {
     PlanHeader *plan;
     Unit *units;            // [B*Jmax*Hkv]
     Chunk *chunks;          // [max_chunks]
+    ChunkRec *recs;         // [max_chunks]  the chunk list again, self-contained records for the TMA kernel
     int32_t *plan_age;      // [0] token boundaries served by the current plan
     int32_t *sched;         // [0] chunk counter (dynamic part of the list), [1] finished-worker counter
     int32_t *scratch;       // plan scratch: [B] J, [B] S, [B+1] entry prefix, [E] tiles, [E+1] tile prefix,
@@ -120,6 +138,10 @@ struct AttendParams {
     uint64_t part_mask;
     int32_t fused;
     int32_t commit;  // 1: the last worker of this launch performs the step commit (static step graph only)
+    // (a2) fused into the launch (static step graph, TMA kernel): [B][H_kv][128] or nullptr.  The worker that attends
+    // the tail tile of (request, kv head) writes the new K/V row to the pool and patches it into its shared-memory
+    // copy of that tile, so the step needs no separate kf_kv_append launch in front of the attention.
+    const __half *k_new, *v_new;
 };
 
 __device__ __forceinline__ void set_error(const Dev &d, int code) { atomicCAS(d.error, 0, code); }

@@ -21,7 +21,8 @@ struct kf_ctx {
 #define KF_INTERNAL __attribute__((visibility("hidden")))
 extern "C" {
 KF_INTERNAL int kf_attend_impl(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, float *o_part, float *lse_part,
-                   int commit, kf_stream stream);                      // commit != 0: + kf_step_commit in the same launch
+                   int commit, const void *k_new, const void *v_new,   // commit != 0: + kf_step_commit in the same launch
+                   kf_stream stream);                                  // k_new / v_new != NULL: + kf_kv_append, ditto
 KF_INTERNAL int kf_layer_step_host_impl(kf_ctx *ctx, int32_t layer, const void *q_host, const void *k_new_host,
                                         const void *v_new_host, float *o_host, float *lse_host, int commit,
                                         kf_stream stream);

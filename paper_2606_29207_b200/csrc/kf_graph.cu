@@ -26,6 +26,7 @@ struct kf_graph {
     int n;                                  // layer-steps per launch
     int host_io;                            // 1: q/k/v/o/lse are pinned host buffers
     bool zero_copy;                         // host_io graph made of kernels only (no copy nodes): re-bindable
+    bool fused_append;                      // device graph with the TMA kernel: the append rides in the attend launch
     int kernels_per_launch;
     std::vector<int32_t> layers;
     std::vector<cudaGraphNode_t> append_nodes, attend_nodes;   // [n] (device-pointer graphs only)
@@ -118,12 +119,14 @@ int kernel_chain(cudaGraph_t g, std::vector<cudaGraphNode_t> &out, std::vector<c
             if (cudaGraphNodeGetType(cur, &t) != cudaSuccess) return -2;
             if (t == cudaGraphNodeTypeKernel) out.push_back(cur);
         }
+        // the _v2 query also reports programmatic (PDL) edges, which the plain one refuses
         size_t nd = 0;
-        if (cudaGraphNodeGetDependentNodes(cur, nullptr, &nd) != cudaSuccess) return -1;
+        if (cudaGraphNodeGetDependentNodes_v2(cur, nullptr, nullptr, &nd) != cudaSuccess) return -1;
         if (nd == 0) break;
         if (nd != 1) return -4;
         cudaGraphNode_t next;
-        if (cudaGraphNodeGetDependentNodes(cur, &next, &nd) != cudaSuccess) return -1;
+        cudaGraphEdgeData edge;
+        if (cudaGraphNodeGetDependentNodes_v2(cur, &next, &edge, &nd) != cudaSuccess) return -1;
         cur = next;
     }
     return 0;
@@ -174,9 +177,11 @@ int build_graph(kf_graph *g, cudaStream_t s) {
         if (g->host_io) {
             rc = kf_layer_step_host_impl(ctx, g->layers[i], g->q[i], g->k[i], g->v[i], g->o[i], g->lse[i], commit, stream);
         } else {
-            rc = kf_kv_append(ctx, g->layers[i], g->k[i], g->v[i], stream);
+            // with the TMA kernel the append rides in the attend launch (n + 1 kernels per step instead of 2n + 1)
+            if (!g->fused_append) rc = kf_kv_append(ctx, g->layers[i], g->k[i], g->v[i], stream);
             if (rc == KF_OK)
-                rc = kf_attend_impl(ctx, g->layers[i], g->q[i], g->o[i], g->lse[i], nullptr, nullptr, commit, stream);
+                rc = kf_attend_impl(ctx, g->layers[i], g->q[i], g->o[i], g->lse[i], nullptr, nullptr, commit,
+                                    g->fused_append ? g->k[i] : nullptr, g->fused_append ? g->v[i] : nullptr, stream);
         }
         if (rc == KF_OK && g->ready) {  // o[i] / lse[i] are complete: signal the host (default flags: the write is
                                         // ordered after all prior writes of the stream, system-wide)
@@ -204,22 +209,23 @@ int build_graph(kf_graph *g, cudaStream_t s) {
     // a host-io graph whose layer-steps all took the zero-copy path consists of kernels (and mem-ops) only: same
     // shape as a device graph (the staging kernel in place of the append kernel), so it can be re-bound the same way
     g->zero_copy = g->host_io && rc == KF_OK && n_nodes == (size_t)(2 * n + 1) + n_mem && (int)chain.size() == 2 * n + 1;
+    const int per = g->fused_append ? 1 : 2;  // kernels per layer-step
     if (rc == KF_OK && mem.size() != n_mem) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "step graph: %zu mem-op nodes captured, %zu expected", mem.size(), n_mem);
         rc = KF_ECUDA;
     }
     if (rc == KF_OK && (!g->host_io || g->zero_copy)) {
-        // kernel order of the capture: plan, n x (append or stage, attend)
-        if ((int)chain.size() != 2 * n + 1) {
+        // kernel order of the capture: plan, n x ([append or stage,] attend)
+        if ((int)chain.size() != per * n + 1) {
             snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "unexpected step-graph topology");
             rc = KF_ECUDA;
         } else {
             for (int i = 0; i < n && rc == KF_OK; ++i) {
-                g->append_nodes.push_back(chain[1 + 2 * i]);
-                g->attend_nodes.push_back(chain[2 + 2 * i]);
+                g->append_nodes.push_back(chain[1 + per * i]);  // (the attend node itself when the append is fused)
+                g->attend_nodes.push_back(chain[per + per * i]);
                 cudaKernelNodeParams pa, pt;
-                e = cudaGraphKernelNodeGetParams(chain[1 + 2 * i], &pa);
-                if (e == cudaSuccess) e = cudaGraphKernelNodeGetParams(chain[2 + 2 * i], &pt);
+                e = cudaGraphKernelNodeGetParams(chain[1 + per * i], &pa);
+                if (e == cudaSuccess) e = cudaGraphKernelNodeGetParams(chain[per + per * i], &pt);
                 if (e != cudaSuccess) rc = cuda_fail(ctx, e);
                 g->append_params.push_back(pa);
                 g->attend_params.push_back(pt);
@@ -265,6 +271,7 @@ int kf_step_graph_create(kf_ctx *ctx, int32_t n_layer_steps, const int32_t *laye
     g->n = n_layer_steps;
     g->host_io = host_io ? 1 : 0;
     g->zero_copy = false;
+    g->fused_append = !g->host_io && ctx->impl == KF_IMPL_TMA;
     g->ready = nullptr;
     g->gates = false;
     g->n_launches = 0;
@@ -347,7 +354,7 @@ int kf_step_graph_launch(kf_graph *g, const void *const *q, const void *const *k
                     g->k[i] = k_new[i];
                     g->v[i] = v_new[i];
                 }
-            } else if (k_new[i] != g->k[i] || v_new[i] != g->v[i]) {
+            } else if (!g->fused_append && (k_new[i] != g->k[i] || v_new[i] != g->v[i])) {
                 // kv_append_kernel(Dev d, int layer, const __half *k_new, const __half *v_new)
                 int layer = g->layers[i];
                 const void *kk = k_new[i], *vv = v_new[i];
@@ -360,7 +367,8 @@ int kf_step_graph_launch(kf_graph *g, const void *const *q, const void *const *k
                 g->k[i] = k_new[i];
                 g->v[i] = v_new[i];
             }
-            if ((!g->host_io && q[i] != g->q[i]) || o[i] != g->o[i] || lse[i] != g->lse[i]) {
+            if ((!g->host_io && q[i] != g->q[i]) || o[i] != g->o[i] || lse[i] != g->lse[i] ||
+                (g->fused_append && (k_new[i] != g->k[i] || v_new[i] != g->v[i]))) {
                 // attend_*_kernel(AttendParams p): same struct as kf_attend builds, new q / o / lse
                 AttendParams ap;
                 ap.d = ctx->dev;
@@ -373,6 +381,8 @@ int kf_step_graph_launch(kf_graph *g, const void *const *q, const void *const *k
                 ap.fused = 1;
                 ap.commit = i == g->n - 1;
                 ap.part_mask = ~0ull;
+                ap.k_new = g->fused_append ? (const __half *)k_new[i] : nullptr;
+                ap.v_new = g->fused_append ? (const __half *)v_new[i] : nullptr;
                 void *args[1] = {&ap};
                 cudaKernelNodeParams p = g->attend_params[i];
                 p.kernelParams = args;
@@ -381,6 +391,10 @@ int kf_step_graph_launch(kf_graph *g, const void *const *q, const void *const *k
                 if (e != cudaSuccess) return cuda_fail(ctx, e);
                 g->o[i] = o[i];
                 g->lse[i] = lse[i];
+                if (g->fused_append) {
+                    g->k[i] = k_new[i];
+                    g->v[i] = v_new[i];
+                }
             }
             g->q[i] = q[i];
         }

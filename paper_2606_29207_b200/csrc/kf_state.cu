@@ -401,6 +401,19 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
         const int piece0 = ppre[e] * Hkv + g * pu + before;
         const int chunk0 = lpre[k * E + e] + g * c;
         const int cq = len / c, cr = len - cq * c;  // the first cr chunks hold cq + 1 tiles
+        const int r = last_le(epre, B + 1, e);
+        const int j = e - epre[r];
+        ChunkRec rec;
+        rec.unit = e * Hkv + g;
+        rec.part = d.route_part[(size_t)r * d.Jmax + j];
+        const int slot = d.route_slot[(size_t)r * d.Jmax + j];
+        rec.req = r;
+        rec.range = j;
+        rec.cnt = min(d.R, Sr[r] - j * d.R);
+        rec.n_pieces = pu;
+        rec.J = Jr[r];
+        rec.pad[0] = rec.pad[1] = rec.pad[2] = rec.pad[3] = 0;
+        const int tail = j == Jr[r] - 1 ? kRecTail : 0;
         for (int i = 0; i < c; ++i) {
             const int t0 = b0 + i * cq + min(i, cr);
             const int t1 = b0 + (i + 1) * cq + min(i + 1, cr);
@@ -410,6 +423,12 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
             ch.n_tiles = t1 - t0;
             ch.piece = piece0 + i;
             d.chunks[chunk0 + i] = ch;
+            rec.tile_begin = t0;
+            rec.n_tiles = t1 - t0;
+            rec.piece = piece0 + i;
+            rec.row0 = (slot * Hkv + g) * d.R + t0 * T;
+            rec.flags = tail | (tail && t1 == etiles[e] ? kRecStretch : 0);
+            d.recs[chunk0 + i] = rec;
         }
     }
 

@@ -325,9 +325,13 @@ int kf_pipeline_step(kf_wside *w, kf_ctx *const *ctxs, int32_t n_micro, int32_t 
         wait(2 * m, as);
         if (rc != KF_OK) return;
         const int lp = layers[l] % ctxs[m]->cfg.n_layers;
-        rc = kf_kv_append(ctxs[m], lp, k_new[m], v_new[m], (kf_stream)as);
-        if (rc == KF_OK)  // the last layer's attend also performs the step commit a5 of its microbatch
-            rc = kf_attend_impl(ctxs[m], lp, q[m], o[m], lse[m], nullptr, nullptr, l == n_layers - 1 ? 1 : 0, (kf_stream)as);
+        // the last layer's attend also performs the step commit a5 of its microbatch; with the TMA kernel the append
+        // a2 rides in the attend launch as well
+        const bool fused = ctxs[m]->impl == KF_IMPL_TMA;
+        if (!fused) rc = kf_kv_append(ctxs[m], lp, k_new[m], v_new[m], (kf_stream)as);
+        if (rc == KF_OK)
+            rc = kf_attend_impl(ctxs[m], lp, q[m], o[m], lse[m], nullptr, nullptr, l == n_layers - 1 ? 1 : 0,
+                                fused ? k_new[m] : nullptr, fused ? v_new[m] : nullptr, (kf_stream)as);
         record(2 * m + 1, as);
     };
     auto post = [&](int m, int l) {

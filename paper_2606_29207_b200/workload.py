@@ -77,8 +77,15 @@ class Session:
         return k, v
 
     # ---- one layer-step through the C ABI -------------------------------------------------------------
-    def layer_step(self, layer: int, q, k_new, v_new, fused: bool = True, want_partials: bool = False):
+    def layer_step(self, layer: int, q, k_new, v_new, fused: bool = True, want_partials: bool = False,
+                   one_launch: bool = False):
         kf = self.kf
+        if one_launch:          # kf_layer_step: append + attend + merge in ONE launch (what the step graph replays)
+            if want_partials:
+                kf.layer_step(layer, q, k_new, v_new, self.o, self.lse, self.o_part, self.lse_part)
+            else:
+                kf.layer_step(layer, q, k_new, v_new, self.o, self.lse)
+            return
         kf.kv_append(layer, k_new, v_new)
         if fused:
             if want_partials:

@@ -29,6 +29,7 @@ def _one_case(rnd, case):
     steps = rnd.randrange(1, 6)
     impl = KF_IMPL_SIMPLE if case % 7 == 6 else KF_IMPL_TMA
     fused = rnd.random() < 0.7
+    one_launch = fused and rnd.random() < 0.5      # kf_layer_step: append + attend + merge in one launch
     wl = Workload(f"fuzz{case}", Hkv * G, Hkv, R, P, ctx)
     ses = Session(wl, impl=impl, steps=steps, min_tiles=rnd.choice([0, 0, 1, 2]),
                   plan_refresh_steps=rnd.choice([0, 0, 1, 2]), sched_decay_pct=rnd.choice([0, 30, 70]))
@@ -37,7 +38,7 @@ def _one_case(rnd, case):
     model = RoutingModel(P, R, B, kf.Jmax, kf.cfg.slots_per_partition)
     for r, n in enumerate(ses.len0):
         model.open_request(r, n)
-    what = f"case {case}: Hkv={Hkv} G={G} R={R} P={P} ctx={ctx} steps={steps} impl={impl} fused={fused}"
+    what = f"case {case}: Hkv={Hkv} G={G} R={R} P={P} ctx={ctx} steps={steps} impl={impl} fused={fused} one_launch={one_launch}"
     for t in range(steps):
         kf.token_boundary()
         model.token_boundary()
@@ -45,7 +46,7 @@ def _one_case(rnd, case):
         k_new, v_new = ses.kv_new_for(0, t)
         ses.o.fill_(float("nan"))
         ses.lse.fill_(float("nan"))
-        ses.layer_step(0, q, k_new, v_new, fused=fused)
+        ses.layer_step(0, q, k_new, v_new, fused=fused, one_launch=one_launch)
         kf.step_commit()
         model.step_commit()
         assert kf.status() == KF_OK, what

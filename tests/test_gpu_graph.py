@@ -7,6 +7,7 @@ pytestmark = pytest.mark.gpu
 
 torch = pytest.importorskip("torch")
 
+from kf_inputs import gen, gen_device  # noqa: E402
 from kf_inputs.workloads import Workload  # noqa: E402
 from kf_testlib import check_close, oracle_request  # noqa: E402
 from oracle.routing import RoutingModel  # noqa: E402
@@ -50,13 +51,25 @@ def test_step_graph_replay_across_route_updates_with_rebinding():
             side.synchronize()
             for l in range(2):
                 _check_step(ses, wl, l, t, o[l].cpu().numpy(), lse[l].cpu().numpy(), "graph")
-        # plan, 2 x (append, attend); the commit rides in the last attend launch
-        assert kf.launch_count() - launches0 == steps * 5
+        # plan, 2 x attend: the append of each layer-step and the commit of the step ride in the attend launches
+        assert kf.launch_count() - launches0 == steps * 3
         assert kf.status() == KF_OK
         snap, ms = kf.route_snapshot(), model.snapshot()
         for key in ("len", "n_ranges", "part", "slot", "free_head", "rr_cursor"):
             assert snap[key] == ms[key], key
         assert sum(ms["n_ranges"]) > sum(-(-n // 64) for n in ses.len0)     # ranges were opened during replay
+        # (a2) rides in the attend launch of the graph: every appended row of every step / layer / request / kv head
+        # sits bit-exact where the integer model puts it
+        for l in range(2):
+            for r, n0 in enumerate(ses.len0):
+                K = gen_device.fill(gen.STREAM_K, l, r, n0, steps, wl.n_kv_heads, seed=wl.seed)
+                V = gen_device.fill(gen.STREAM_V, l, r, n0, steps, wl.n_kv_heads, seed=wl.seed)
+                for t in range(steps):
+                    p, sl, off = model.locate(r, n0 + t)
+                    for gk in range(wl.n_kv_heads):
+                        for is_v, src in ((False, K), (True, V)):
+                            o0 = kf.pool_offset(l, sl, gk, off, is_v)
+                            assert torch.equal(kf.pools[p][o0:o0 + 256].view(torch.float16), src[gk, t]), (l, r, t, gk, is_v)
         g.destroy()
     ses.close()
 

@@ -17,7 +17,7 @@ from paper_2606_29207_b200.workload import Session  # noqa: E402
 IMPLS = [KF_IMPL_SIMPLE, KF_IMPL_TMA]
 
 
-def _decode_loop(wl, impl, steps, refresh, fused=True, min_tiles=0, check_every=1):
+def _decode_loop(wl, impl, steps, refresh, fused=True, min_tiles=0, check_every=1, one_launch=False):
     ses = Session(wl, impl=impl, steps=steps, min_tiles=min_tiles, plan_refresh_steps=refresh)
     ses.prepare()
     kf = ses.kf
@@ -32,7 +32,7 @@ def _decode_loop(wl, impl, steps, refresh, fused=True, min_tiles=0, check_every=
         k_new, v_new = ses.kv_new_for(0, step)
         ses.o.fill_(float("nan"))
         ses.lse.fill_(float("nan"))
-        ses.layer_step(0, q, k_new, v_new, fused=fused)
+        ses.layer_step(0, q, k_new, v_new, fused=fused, one_launch=one_launch)
         kf.step_commit()
         model.step_commit()
         assert kf.status() == KF_OK
@@ -57,6 +57,18 @@ def test_kept_plan_decode_loop_matches_oracle(impl, refresh):
     # sits one token before a tile edge, and the plan ages past `refresh` (0 = default 128: never, 1: every step)
     wl = Workload("kept_plan", 32, 8, 64, 3, [200, 125, 33, 65, 16, 1])
     _decode_loop(wl, impl, steps=40, refresh=refresh)
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_layer_step_one_launch_equals_append_then_attend(impl):
+    # kf_layer_step (append + attend + merge in ONE launch: the new K/V row is written to the pool AND patched into the
+    # shared-memory copy of the tail tile) must give the bits of kf_kv_append followed by kf_attend, at every step of a
+    # loop whose tails cross tile edges, fill ranges and sit in 1-token ranges; and it matches the oracle
+    wl = Workload("one_launch", 32, 8, 64, 3, [200, 125, 33, 65, 16, 1])
+    a = _decode_loop(wl, impl, steps=40, refresh=0, one_launch=True)
+    b = _decode_loop(wl, impl, steps=40, refresh=0, one_launch=False, check_every=40)
+    for step, ((oa, la), (ob, lb)) in enumerate(zip(a, b)):
+        assert np.array_equal(oa, ob) and np.array_equal(la, lb), step
 
 
 def test_kept_plan_many_pieces_and_unfused():

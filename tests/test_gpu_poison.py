@@ -70,7 +70,7 @@ def test_poisoned_pools_fused_through_the_step_graph(impl, pattern, min_tiles):
 
 @pytest.mark.parametrize("impl", [KF_IMPL_SIMPLE, KF_IMPL_TMA])
 @pytest.mark.parametrize("pattern", list(PATTERNS), ids=list(PATTERNS))
-@pytest.mark.parametrize("fused", [True, False])
+@pytest.mark.parametrize("fused", [True, False, "one_launch"])
 def test_poisoned_pools_eager_with_partials(impl, pattern, fused):
     wl = Workload("poison", 32, 8, 64, 3, CONTEXTS)
     ses = Session(wl, impl=impl, steps=STEPS, min_tiles=1)
@@ -83,7 +83,7 @@ def test_poisoned_pools_eager_with_partials(impl, pattern, fused):
         k_new, v_new = ses.kv_new_for(0, t)
         for x in (ses.o, ses.lse, ses.o_part, ses.lse_part):
             x.fill_(float("nan"))
-        ses.layer_step(0, q, k_new, v_new, fused=fused, want_partials=True)
+        ses.layer_step(0, q, k_new, v_new, fused=bool(fused), want_partials=True, one_launch=fused == "one_launch")
         kf.step_commit()
         assert kf.status() == KF_OK
         _check_all(wl, t, ses.o.cpu().numpy(), ses.lse.cpu().numpy(), ses.o_part.cpu().numpy(),
@@ -105,7 +105,7 @@ def test_poisoned_pools_g8_and_long_ragged_units():
             k_new, v_new = ses.kv_new_for(0, t)
             for x in (ses.o, ses.lse, ses.o_part, ses.lse_part):
                 x.fill_(float("nan"))
-            ses.layer_step(0, q, k_new, v_new, fused=True, want_partials=True)
+            ses.layer_step(0, q, k_new, v_new, fused=True, want_partials=True, one_launch=t == 1)
             kf.step_commit()
             assert kf.status() == KF_OK
             _check_all(wl, t, ses.o.cpu().numpy(), ses.lse.cpu().numpy(), ses.o_part.cpu().numpy(),
