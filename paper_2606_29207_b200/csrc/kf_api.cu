@@ -602,7 +602,7 @@ int kf_plan_info(kf_ctx *ctx, int32_t *out, kf_stream stream) {
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_plan(ctx, s);
     if (rc != KF_OK) return rc;
-    cudaError_t e = cudaMemcpyAsync(out, ctx->dev.plan, sizeof(PlanHeader), cudaMemcpyDeviceToHost, s);
+    cudaError_t e = cudaMemcpyAsync(out, ctx->dev.plan, 8 * sizeof(int32_t), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     return KF_OK;

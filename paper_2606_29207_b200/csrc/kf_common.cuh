@@ -71,6 +71,8 @@ struct PlanHeader {
     int32_t tile_tokens;
     int32_t max_workers;
     int32_t n_levels;
+    int32_t max_unit_pieces;  // largest n_pieces of any unit / largest J_r of any request: the fused merge sizes its
+    int32_t max_J;            // tasks from them (how many heads one warp merges per round trip, kf_merge.cuh)
 };
 
 // Device pointers into the caller's workspace + immutable config.  Passed BY VALUE to every kernel.

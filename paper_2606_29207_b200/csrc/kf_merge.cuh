@@ -138,6 +138,100 @@ static __device__ __noinline__ void merge_rows(const float *src_o, size_t o_stri
     }
 }
 
+// The same reduction for up to HC = min(8, 32 / N2) CONSECUTIVE query heads at once, n <= N2 partials each (N2 a power
+// of two): all HC * N2 <= 32 rows are requested before anything is computed, so a warp merges HC heads in the ONE L2
+// round trip that merge_rows spends on one.  The fused merge tail is a chain of dependent round trips per task (unit
+// record, counter, rows, store, fence, signal); with G = 8 heads and 4 ranges per request it was 25 us of a 645 us
+// launch at one head per task.  Head h reads src_o + h * 128 / src_lse + h and writes dst + h * 128 / dst_lse + h.
+// Same arithmetic, same order (j ascending; the lse sum is the same shuffle tree, restricted to the N2 lanes of the
+// head), so the result is bit-identical to merge_rows.
+template <int N2>
+static __device__ __noinline__ void merge_heads(const float *src_o, size_t o_stride, const float *src_lse, size_t lse_stride,
+                                            int n, int heads, float *dst_o, float *dst_lse, float *dst2_o,
+                                            float *dst2_lse, int lane) {
+    constexpr int HC = 32 / N2 < 8 ? 32 / N2 : 8;
+    const int hl = lane / N2, jl = lane % N2;  // this lane's (head, partial) in the lse phase
+    const bool have = hl < heads && hl < HC && jl < n;
+    const float lj = have ? __ldcg(src_lse + hl + (size_t)jl * lse_stride) : -INFINITY;
+    float4 v[HC * N2];
+#pragma unroll
+    for (int k = 0; k < HC * N2; ++k) {
+        const int h = k / N2, j = k % N2;
+        v[k] = (h < heads && j < n)
+                   ? __ldcg(reinterpret_cast<const float4 *>(src_o + (size_t)h * kHeadDim + (size_t)j * o_stride) + lane)
+                   : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    float M = lj;
+#pragma unroll
+    for (int o = N2 / 2; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+    float sum = M != -INFINITY ? expf(lj - M) : 0.f;  // exp(-inf) = 0 for the padding
+#pragma unroll
+    for (int o = N2 / 2; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    const float lse = M != -INFINITY ? M + logf(sum) : -INFINITY;
+    const float wl = (have && lse != -INFINITY) ? expf(lj - lse) : 0.f;
+    float4 acc[HC];
+#pragma unroll
+    for (int h = 0; h < HC; ++h) acc[h] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int k = 0; k < HC * N2; ++k) {
+        const int h = k / N2, j = k % N2;
+        const float w = __shfl_sync(0xffffffffu, wl, k);
+        if (h < heads && j < n && w != 0.f) {  // w == 0 (lse_j = -inf): ignore its o_j, whatever it holds
+            acc[h].x = fmaf(w, v[k].x, acc[h].x);
+            acc[h].y = fmaf(w, v[k].y, acc[h].y);
+            acc[h].z = fmaf(w, v[k].z, acc[h].z);
+            acc[h].w = fmaf(w, v[k].w, acc[h].w);
+        }
+    }
+#pragma unroll
+    for (int h = 0; h < HC; ++h) {
+        if (h < heads) {
+            reinterpret_cast<float4 *>(dst_o + (size_t)h * kHeadDim)[lane] = acc[h];
+            if (dst2_o) reinterpret_cast<float4 *>(dst2_o + (size_t)h * kHeadDim)[lane] = acc[h];
+        }
+    }
+    if (have && jl == 0) {
+        dst_lse[hl] = lse;
+        if (dst2_o) dst2_lse[hl] = lse;
+    }
+}
+
+// heads merged per task when no head has more than n_max partials; the padded partial count N2 that goes with it
+__device__ __forceinline__ int merge_n2(int n_max) { return n_max <= 8 ? 8 : n_max <= 16 ? 16 : 32; }
+__device__ __forceinline__ int merge_hc(int n2, int G) { return min(G, 32 / n2); }  // 4, 2 or 1 heads per task
+
+// `heads` consecutive heads, n partials each: one merge_heads call when n fits its N2, else head by head
+__device__ __forceinline__ void merge_group(int n2, const float *src_o, size_t o_stride, const float *src_lse,
+                                            size_t lse_stride, int n, int heads, float *dst_o, float *dst_lse,
+                                            float *dst2_o, float *dst2_lse, int lane) {
+    if (n > n2 || n2 > 16) {  // more partials than one round trip of merge_heads holds: head by head
+        for (int h = 0; h < heads; ++h)
+            merge_rows(src_o + (size_t)h * kHeadDim, o_stride, src_lse + h, lse_stride, n, dst_o + (size_t)h * kHeadDim,
+                       dst_lse + h, dst2_o ? dst2_o + (size_t)h * kHeadDim : nullptr, dst2_o ? dst2_lse + h : nullptr, lane);
+        return;
+    }
+    // two instantiations only: this code runs at the very end of a launch with a cold instruction cache
+    if (n2 <= 8)
+        merge_heads<8>(src_o, o_stride, src_lse, lse_stride, n, heads, dst_o, dst_lse, dst2_o, dst2_lse, lane);
+    else
+        merge_heads<16>(src_o, o_stride, src_lse, lse_stride, n, heads, dst_o, dst_lse, dst2_o, dst2_lse, lane);
+}
+
+__device__ __forceinline__ Unit load_unit_g(const Unit *units, int u) {
+    const int4 *q = reinterpret_cast<const int4 *>(units + u);
+    const int4 a = __ldg(q), b = __ldg(q + 1);
+    Unit un;
+    un.req = a.x;
+    un.range = a.y;
+    un.part = a.z;
+    un.slot = a.w;
+    un.cnt = b.x;
+    un.tail = b.y;
+    un.piece_begin = b.z;
+    un.n_pieces = b.w;
+    return un;
+}
+
 // merge the pieces of unit u, query head i of its group, into the range partial (and into the final output if
 // the request has a single range and `to_final`)
 __device__ __forceinline__ void merge_unit_head(const AttendParams &p, const Unit &un, int g, int i, bool to_final,
@@ -244,16 +338,35 @@ __device__ __forceinline__ void wait_counter(const int32_t *ctr, int target, int
 }
 
 // Fused tail: once the chunk list is exhausted every worker turns into a merge worker.
-// One ticket stream covers both levels: tasks [0, nA) = (unit, head of its group): pieces -> range partial;
-// tasks [nA, nA + nB) = (request, query head): range partials -> output.  A task waits until its inputs are
+// One ticket stream covers both levels: tasks [0, nA) = (unit, chunk of heads of its group): pieces -> range partial;
+// tasks [nA, total) = (request, kv head, chunk of heads): range partials -> output.  A chunk holds as many heads as
+// fit one round trip of merge_heads, given the launch's largest piece count / range count (plan header).  A task
+// waits until its inputs are
 // complete; its producers are either chunks (taken by resident workers of this launch: the grid never exceeds
 // the SM count) or tasks with a LOWER ticket, and every worker serves its tickets in ascending order, so the
 // waits cannot deadlock.  Tickets are taken in batches (bounded atomic traffic on one word) and the next batch
 // is requested before the current one is processed, which keeps the atomic's round trip off the critical path.
 // `first` is lane 0's pre-taken first ticket (merge_first_ticket) or -1.
+struct MergeShape {
+    int n2A, hcA, caA;  // A level (pieces -> range partial): padded partials per head, heads per task, tasks per unit
+    int n2B, hcB, caB;  // B level (range partials -> output): ditto per (request, kv head)
+    int nA, total;
+};
+__device__ __forceinline__ MergeShape merge_shape(const Dev &d) {
+    MergeShape m;
+    // ONE N2 for both levels: the tail of a launch runs this code with a cold instruction cache, and a second
+    // instantiation of merge_heads costs more in instruction fetches than the heads it would add per task
+    m.n2A = m.n2B = merge_n2(max(__ldg(&d.plan->max_unit_pieces), __ldg(&d.plan->max_J)));
+    m.hcA = merge_hc(m.n2A, d.G);
+    m.caA = (d.G + m.hcA - 1) / m.hcA;
+    m.hcB = merge_hc(m.n2B, d.G);
+    m.caB = (d.G + m.hcB - 1) / m.hcB;
+    m.nA = __ldg(&d.plan->n_units) * m.caA;
+    m.total = m.nA + d.B * d.Hkv * m.caB;
+    return m;
+}
 __device__ __forceinline__ int merge_batch(const Dev &d, int W) {
-    const int total = __ldg(&d.plan->n_units) * d.G + d.B * d.Hq;
-    return max(1, total / (4 * W));
+    return max(1, merge_shape(d).total / (4 * W));
 }
 __device__ __forceinline__ int merge_first_ticket(const Dev &d, int W) {  // call from ONE lane
     return atomicAdd(d.sched + 2, merge_batch(d, W));
@@ -262,38 +375,52 @@ __device__ __forceinline__ int merge_first_ticket(const Dev &d, int W) {  // cal
 __device__ __forceinline__ void merge_phase(const AttendParams &p, const Counters &c, int W, int lane, int first = -1) {
     const Dev &d = p.d;
     const int G = d.G, Hkv = d.Hkv;
-    const int nA = __ldg(&d.plan->n_units) * G;
-    const int total = nA + d.B * d.Hq;
-    const int batch = merge_batch(d, W);
+    const MergeShape ms = merge_shape(d);
+    const int batch = max(1, ms.total / (4 * W));
     int next = first;
     if (lane == 0 && next < 0) next = atomicAdd(d.sched + 2, batch);
     for (;;) {
         const int t0 = __shfl_sync(0xffffffffu, next, 0);
-        if (t0 >= total) break;
+        if (t0 >= ms.total) break;
         if (lane == 0) next = atomicAdd(d.sched + 2, batch);  // in flight while this batch is processed
-        const int t1 = min(total, t0 + batch);
+        const int t1 = min(ms.total, t0 + batch);
         for (int t = t0; t < t1; ++t) {
-            if (t < nA) {
-                const int u = t / G, i = t - u * G;
-                const Unit un = d.units[u];
+            if (t < ms.nA) {
+                // task = (unit, chunk of hcA heads of its group): pieces -> range partial (and the output if J_r = 1)
+                const int u = t / ms.caA, i0 = (t - u * ms.caA) * ms.hcA;
+                const int heads = min(ms.hcA, G - i0);
+                const Unit un = load_unit_g(d.units, u);
                 if (un.n_pieces <= 1) continue;
-                const int g = u % Hkv;
+                const int g = u % Hkv, head = g * G + i0;
+                const int J = d.scratch[un.req];
                 wait_counter(&c.unit[u], un.n_pieces, lane);
-                merge_unit_head(p, un, g, i, true, lane);
-                if (d.scratch[un.req] > 1) {
+                const size_t row = range_row(d, un.req, un.range, head);
+                const size_t frow = (size_t)un.req * d.Hq + head;
+                merge_group(ms.n2A, d.piece_o + ((size_t)un.piece_begin * G + i0) * kHeadDim, (size_t)G * kHeadDim,
+                            d.piece_lse + (size_t)un.piece_begin * G + i0, G, un.n_pieces, heads,
+                            p.o_part + row * kHeadDim, p.lse_part + row, J == 1 ? p.o + frow * kHeadDim : nullptr,
+                            J == 1 ? p.lse + frow : nullptr, lane);
+                if (J > 1) {
                     __syncwarp();
                     if (lane == 0) {
                         release_fence();
-                        atomicAdd(&c.group[un.req * Hkv + g], 1);
+                        atomicAdd(&c.group[un.req * Hkv + g], heads);
                     }
                 }
             } else {
-                const int tb = t - nA;
-                const int req = tb / d.Hq, h = tb - req * d.Hq;
+                // task = (request, kv head, chunk of hcB heads): range partials -> output
+                const int tb = t - ms.nA;
+                const int grp = tb / ms.caB, i0 = (tb - grp * ms.caB) * ms.hcB;
+                const int heads = min(ms.hcB, G - i0);
+                const int req = grp / Hkv, g = grp - req * Hkv;
                 const int J = d.scratch[req];  // 0 for closed requests
                 if (J <= 1) continue;          // a single range: its partial was also written to the output
-                wait_counter(&c.group[req * Hkv + h / G], J * G, lane);
-                merge_request_head(d, p.o_part, p.lse_part, p.o, p.lse, req, h, J, lane);
+                wait_counter(&c.group[grp], J * G, lane);
+                const int h = g * G + i0;
+                const size_t row = range_row(d, req, 0, h);
+                const size_t frow = (size_t)req * d.Hq + h;
+                merge_group(ms.n2B, p.o_part + row * kHeadDim, (size_t)d.Hq * kHeadDim, p.lse_part + row, d.Hq, J, heads,
+                            p.o + frow * kHeadDim, p.lse + frow, nullptr, nullptr, lane);
             }
         }
     }

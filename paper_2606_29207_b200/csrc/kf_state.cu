@@ -252,7 +252,7 @@ constexpr int kPlanSmemInts = 48 * 1024;  // 192 KB of dynamic shared memory
 __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
     extern __shared__ int plan_smem[];
     __shared__ Levels lv;
-    __shared__ int s_m, s_keep;
+    __shared__ int s_m, s_keep, s_max_pieces, s_max_J;
     const int tid = threadIdx.x, nt = blockDim.x;
     const int B = d.B, Emax = d.B * d.Jmax, T = kTileTokens, Hkv = d.Hkv;
     if (do_boundary) {
@@ -289,6 +289,8 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
     int *epre = take(B + 1, g_epre);
     int *etiles = nullptr, *tpre = nullptr, *ppre = nullptr, *pos = nullptr, *ccnt = nullptr, *lpre = nullptr;
 
+    if (tid == 0) s_max_pieces = s_max_J = 0;
+    __syncthreads();
     // 1. per request: tokens attended this step S = len + 1, ranges J = ceil(S / R)
     for (int r = tid; r < B; r += nt) {
         const int len = d.len[r];
@@ -303,6 +305,7 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
         Jr[r] = J;
         Sr[r] = (int)S;
         epre[r] = J;
+        if (J > 1) atomicMax(&s_max_J, J);
     }
     __syncthreads();
     const int E = block_exclusive_scan(epre, B);
@@ -379,6 +382,7 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
         int pu = 0;
         for (int k = 0; k < K; ++k) pu += ccnt[k * E + e];
         ppre[e] = pu;
+        if (pu > 1) atomicMax(&s_max_pieces, pu);
     }
     __syncthreads();
     const int pieces_per_head = block_exclusive_scan(ppre, E);
@@ -460,6 +464,8 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
         h.tile_tokens = T;
         h.max_workers = W;
         h.n_levels = K;
+        h.max_unit_pieces = s_max_pieces;
+        h.max_J = s_max_J;
         *d.plan = h;
     }
 }
