@@ -21,6 +21,16 @@ attending).  Where the paper is silent the readings of DESIGN.md apply:
              the paper's "existing KV ranges remain in place ... future appends use the new A node" (:240) then
              holds again as soon as a slot is freed or a node is activated
 
+  reading 28: "publish the route and redirect active tails on i to prewarm[i]" (Algorithm 1 l.16-17, PAPER.md:216-219;
+             "at the next token boundary ... future appends use the new A node, while existing KV ranges remain in
+             place", :240), taken literally: redirect_tails(parts) marks partitions; at the NEXT token boundary every
+             active request whose tail range lives on a marked partition (and holds at least one token) CLOSES that
+             range at its current length and continues in a new range -- beginning at position len -- on the next
+             active partition.  So a range is [begin_j, begin_{j+1}) with begin_{j+1} - begin_j <= R; without
+             redirects begin_j = j*R and everything above is unchanged.  A redirect that finds no free slot (or no
+             free route entry) is simply not carried out: the tail stays where it is, no error.  The marks are
+             consumed by that one boundary.
+
 Pure Python, no numpy: written to be checked against the text by eye.
 """
 from __future__ import annotations
@@ -42,6 +52,8 @@ class RoutingModel:
         self.slots = slots_per_partition
         self.len: List[int] = [-1] * max_requests          # -1 = request closed
         self.route: List[List[Tuple[int, int]]] = [[] for _ in range(max_requests)]
+        self.begin: List[List[int]] = [[] for _ in range(max_requests)]    # first token position of every range
+        self.redirect = set()                               # partitions whose tails move at the next boundary
         self.rr_cursor = 0                                  # ranges allocated so far
         self.rr_last = -1                                   # partition of the last allocation
         self.active = [True] * n_partitions                 # partitions that receive new ranges
@@ -50,7 +62,7 @@ class RoutingModel:
         self.free_list: List[List[int]] = [[] for _ in range(n_partitions)]  # LIFO of released slots
 
     # -- allocation -----------------------------------------------------------------------------
-    def _alloc(self, req: int) -> Tuple[int, int]:
+    def _alloc(self, req: int, begin: int) -> Tuple[int, int]:
         if len(self.route[req]) >= self.Jmax:
             raise RoutingError("ENOSPC: max_ranges_per_request")
         p = None
@@ -70,6 +82,7 @@ class RoutingModel:
         else:
             self.free_head[p] += 1
         self.route[req].append((p, slot))
+        self.begin[req].append(begin)
         return p, slot
 
     # -- API mirror -----------------------------------------------------------------------------
@@ -80,8 +93,8 @@ class RoutingModel:
         if n_tokens < 0:
             raise RoutingError("EINVAL")
         self.len[req] = n_tokens
-        for _ in range(-(-n_tokens // self.R)):
-            self._alloc(req)
+        for j in range(-(-n_tokens // self.R)):
+            self._alloc(req, j * self.R)
 
     def token_boundary(self) -> List[Tuple[int, int, int, int]]:
         """Open a new range for every open request whose tail position has no route: its tail range is full
@@ -93,13 +106,22 @@ class RoutingModel:
         for r in range(self.B):
             if self.len[r] < 0 or not self.req_active[r]:
                 continue
-            if len(self.route[r]) * self.R <= self.len[r]:
+            n = self.len[r]
+            if not self.route[r] or n - self.begin[r][-1] >= self.R:     # no route for position n
                 try:
-                    p, s = self._alloc(r)
+                    p, s = self._alloc(r, n)
                 except RoutingError as e:
                     failed = failed or e
                     continue
                 events.append((r, len(self.route[r]) - 1, p, s))
+            elif self.route[r][-1][0] in self.redirect and n > self.begin[r][-1]:
+                # reading 28: the tail range is closed at its current length; the new one starts at position n
+                try:
+                    p, s = self._alloc(r, n)
+                except RoutingError:
+                    continue                                             # not carried out: the tail stays
+                events.append((r, len(self.route[r]) - 1, p, s))
+        self.redirect = set()
         self.last_events = events
         if failed is not None:
             raise failed
@@ -110,17 +132,17 @@ class RoutingModel:
         n = self.len[req]
         if n < 0:
             raise RoutingError("ESTATE: closed request")
-        j = n // self.R
-        if j >= len(self.route[req]):
+        if not self.route[req] or n - self.begin[req][-1] >= self.R:
             raise RoutingError("ESTATE: no route for the tail position (token_boundary not called)")
-        p, s = self.route[req][j]
-        return p, s, n - j * self.R
+        p, s = self.route[req][-1]
+        return p, s, n - self.begin[req][-1]
 
     def step_commit(self) -> None:
         """len += 1 for every open, active request whose tail position had a route in this step (reading 24: a
         request that is waiting for a slot appended nothing and stays where it is)."""
         for r in range(self.B):
-            if self.len[r] >= 0 and self.req_active[r] and len(self.route[r]) * self.R > self.len[r]:
+            if (self.len[r] >= 0 and self.req_active[r] and self.route[r]
+                    and self.len[r] - self.begin[r][-1] < self.R):
                 self.len[r] += 1
 
     def close_request(self, req: int) -> None:
@@ -129,6 +151,7 @@ class RoutingModel:
         for (p, s) in self.route[req]:       # ascending j
             self.free_list[p].append(s)
         self.route[req] = []
+        self.begin[req] = []
         self.len[req] = -1
 
     def set_active(self, active) -> None:
@@ -136,6 +159,18 @@ class RoutingModel:
         if len(active) != self.P or not any(active):
             raise RoutingError("EINVAL")
         self.active = [bool(a) for a in active]
+
+    def redirect_tails(self, parts) -> None:
+        """Mark partitions (reading 28): their tails move to a new range at the next token boundary."""
+        if len(parts) != self.P:
+            raise RoutingError("EINVAL")
+        self.redirect = {p for p in range(self.P) if parts[p]}
+
+    def range_tokens_held(self, req: int, j: int) -> int:
+        """Committed tokens of range j of an open request."""
+        b = self.begin[req]
+        end = b[j + 1] if j + 1 < len(b) else min(self.len[req], b[j] + self.R)
+        return max(0, end - b[j])
 
     def set_active_requests(self, active=None) -> None:
         """Requests that take part in the following decode steps; a paused request keeps its routes and tokens."""
@@ -148,7 +183,7 @@ class RoutingModel:
             if self.len[r] < 0:
                 continue
             for j, (p, _) in enumerate(self.route[r]):
-                tokens[p] += max(0, min(self.R, self.len[r] - j * self.R))
+                tokens[p] += self.range_tokens_held(r, j)
                 if j == len(self.route[r]) - 1 and self.req_active[r]:   # "r active" (Algorithm 1, l.7)
                     tails[p] += 1
         return {"active": [1 if a else 0 for a in self.active], "tokens": tokens, "tails": tails}
@@ -159,15 +194,16 @@ class RoutingModel:
 
     def locate(self, req: int, pos: int) -> Tuple[int, int, int]:
         """(partition, slot, offset) of logical token ``pos`` of a request."""
-        j = pos // self.R
+        j = max(i for i, b in enumerate(self.begin[req]) if b <= pos)
         p, s = self.route[req][j]
-        return p, s, pos - j * self.R
+        return p, s, pos - self.begin[req][j]
 
     def snapshot(self) -> Dict[str, object]:
         part = [[-1] * self.Jmax for _ in range(self.B)]
         slot = [[-1] * self.Jmax for _ in range(self.B)]
+        begin = [[-1] * self.Jmax for _ in range(self.B)]
         for r in range(self.B):
             for j, (p, s) in enumerate(self.route[r]):
-                part[r][j], slot[r][j] = p, s
+                part[r][j], slot[r][j], begin[r][j] = p, s, self.begin[r][j]
         return {"len": list(self.len), "n_ranges": [len(x) for x in self.route], "part": part,
-                "slot": slot, "free_head": list(self.free_head), "rr_cursor": self.rr_cursor}
+                "slot": slot, "begin": begin, "free_head": list(self.free_head), "rr_cursor": self.rr_cursor}

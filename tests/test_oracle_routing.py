@@ -276,3 +276,106 @@ def test_paused_requests_keep_routes_and_length():
     assert [e[:2] for e in ev if e[0] == 0] == [(0, 1)]
     m.step_commit()
     assert m.len[0] == 5 and sum(m.partition_state()["tails"]) == 3
+
+
+# ---- reading 28: Algorithm 1 l.16-17 taken literally -- a published route redirects ACTIVE TAILS at the next boundary ----
+def test_fig5_with_a_cut_at_t_plus_k_worked_by_hand():
+    # Fig. 5 continued: T = 16, R = 8, three nodes.  [0,8)->A0, [8,16)->A1, the boundary at len = 16 opens
+    # [16,..)->A2.  Three tokens later (len = 19) node A2 is over its threshold: the policy publishes a route without
+    # A2 and redirects its tails.  At the NEXT boundary the tail [16,19) is closed where it is
+    # and [19,..) opens on the first active node after A2 = A0; nothing older changes (:240).
+    m = RoutingModel(n_partitions=3, range_tokens=8, max_requests=1, max_ranges_per_request=6, slots_per_partition=3)
+    m.open_request(0, 16)
+    for _ in range(3):
+        m.token_boundary()
+        m.step_commit()
+    assert m.len[0] == 19 and m.route[0] == [(0, 0), (1, 0), (2, 0)] and m.begin[0] == [0, 8, 16]
+    m.set_active([1, 1, 0])
+    m.redirect_tails([0, 0, 1])
+    assert m.token_boundary() == [(0, 3, 0, 1)]                      # A0's slot 0 holds [0,8): bump allocator gives slot 1
+    assert m.route[0] == [(0, 0), (1, 0), (2, 0), (0, 1)] and m.begin[0] == [0, 8, 16, 19]
+    assert m.append_position(0) == (0, 1, 0)                         # token 19 is the first token of the new range
+    assert [m.range_tokens_held(0, j) for j in range(4)] == [8, 8, 3, 0]
+    assert m.locate(0, 18) == (2, 0, 2) and m.locate(0, 16) == (2, 0, 0) and m.locate(0, 15) == (1, 0, 7)
+    m.step_commit()
+    assert m.locate(0, 19) == (0, 1, 0)
+    # the marks are consumed: nothing moves at the following boundaries until the new tail is FULL (8 tokens: 19..26)
+    for n in range(20, 27):
+        assert m.token_boundary() == []
+        assert m.append_position(0) == (0, 1, n - 19)
+        m.step_commit()
+    assert m.len[0] == 27
+    assert m.token_boundary() == [(0, 4, 1, 1)]                      # 27 - 19 = 8 = R: next active node after A0 is A1
+    assert m.begin[0] == [0, 8, 16, 19, 27]
+    st = m.partition_state()
+    assert st["tokens"] == [8 + 8, 8 + 0, 3] and st["tails"] == [0, 1, 0]
+
+
+def test_redirect_moves_only_tails_on_marked_nodes_and_only_nonempty_ones():
+    m = RoutingModel(3, 4, 3, 6, 4)
+    m.open_request(0, 5)      # ranges -> A0, A1: tail on A1 holds token 4
+    m.open_request(1, 2)      # A2: tail on A2
+    m.open_request(2, 4)      # A0: tail full -> the boundary opens a range anyway
+    m.redirect_tails([0, 1, 0])
+    ev = m.token_boundary()
+    # request 0: tail on the marked node A1, one token in it -> cut at 5; request 1: not marked; request 2: ordinary fill
+    assert [(r, j) for r, j, _, _ in ev] == [(0, 2), (2, 1)]
+    assert m.begin[0] == [0, 4, 5] and m.begin[1] == [0] and m.begin[2] == [0, 4]
+    # a tail that holds no token yet (opened at the previous boundary, nothing committed since) is not cut again;
+    # request 1's tail on A2 holds two tokens and IS cut now that every node is marked
+    m.redirect_tails([1, 1, 1])
+    ev = m.token_boundary()
+    assert [(r, j) for r, j, _, _ in ev] == [(1, 1)]
+    assert m.begin[0] == [0, 4, 5] and m.begin[1] == [0, 2] and m.begin[2] == [0, 4]
+
+
+def test_redirect_without_a_free_slot_is_not_carried_out():
+    m = RoutingModel(2, 4, 2, 4, 1)
+    m.open_request(0, 2)      # A0 slot 0
+    m.open_request(1, 2)      # A1 slot 0: every slot is taken
+    m.redirect_tails([1, 0])
+    assert m.token_boundary() == []          # no error, the tail stays
+    assert m.append_position(0) == (0, 0, 2)
+    m.step_commit()
+    assert m.len == [3, 3]
+
+
+def test_redirect_invariants_random_walk():
+    import random
+    rnd = random.Random(28)
+    P, R, B = 4, 8, 6
+    m = RoutingModel(P, R, B, 64, 64)
+    for r in range(B):
+        m.open_request(r, rnd.randrange(0, 30))
+    history = [list(map(tuple, m.route))]
+    for step in range(200):
+        if rnd.random() < 0.2:
+            m.redirect_tails([rnd.random() < 0.4 for _ in range(P)])
+        if rnd.random() < 0.1:
+            act = [rnd.random() < 0.7 for _ in range(P)]
+            m.set_active(act if any(act) else [1] * P)
+        m.token_boundary()
+        for r in range(B):
+            b = m.begin[r]
+            assert b[0] == 0 and all(0 < b[j + 1] - b[j] <= R for j in range(len(b) - 1))     # ranges tile [0, len]
+            assert 0 <= m.len[r] - b[-1] < R                                                   # the tail has room
+            assert m.append_position(r)[2] == m.len[r] - b[-1]
+            assert sum(m.range_tokens_held(r, j) for j in range(len(b))) == m.len[r]
+            old = history[-1][r]
+            assert tuple(m.route[r][:len(old)]) == tuple(old)                                  # entries never change
+        history.append([tuple(x) for x in m.route])
+        m.step_commit()
+    assert sum(m.partition_state()["tokens"]) == sum(m.len)
+    used = [(p, s) for r in range(B) for (p, s) in m.route[r]]
+    assert len(used) == len(set(used)) == m.rr_cursor
+
+
+def test_no_redirect_means_begin_is_j_times_r():
+    m = RoutingModel(3, 4, 2, 16, 16)
+    m.open_request(0, 9)
+    m.open_request(1, 0)
+    for _ in range(20):
+        m.token_boundary()
+        m.step_commit()
+    for r in range(2):
+        assert m.begin[r] == [4 * j for j in range(len(m.route[r]))]
