@@ -140,15 +140,21 @@ int kf_close_request(kf_ctx *ctx, int32_t req, kf_stream stream);
  *   serving the ranges they hold.  Allocation order: the first active partition after the one used last, cyclically
  *   (with all P active: the k-th range ever allocated goes to partition k mod P).  All partitions start active.
  *   This call is the critical-path "route install" (paper: 7.2 us on the CPU): one tiny kernel.
- *   DEVIATION from Algorithm 1 l.16-17 / PAPER.md:240 ("redirect active tails on i to prewarm[i]" at the next token
- *   boundary): with fixed-size ranges (reading 20) a tail keeps appending to the node that holds its
- *   current range until that range is full -- up to R tokens per tail -- and only then moves to a node of the new
- *   active set.  A node that left the set can therefore still grow by (its tails) * R tokens: C_thresh may be
- *   overshot by n_i * R * bytes_per_token, and kf_policy_step keeps reporting want_publish for it meanwhile.
+ *   On its own it moves a tail only when its current range fills (reading 20): a node that left the set can
+ *   still grow by (its tails) * R tokens.  Algorithm 1 l.16-17 ("publish the route and redirect active tails on i to
+ *   prewarm[i]") is this call FOLLOWED BY kf_redirect_tails for node i.
+ * kf_redirect_tails -- partitions: [host] uint8[P], non-zero = marked.  At the NEXT kf_token_boundary every active request
+ *   whose tail range lives on a marked partition and holds at least one token closes that range at its current length
+ *   and continues in a new range, beginning at position len_r, on the next active partition (PAPER.md:216-219, :240:
+ *   "at the next token boundary ... future appends use the new A node, while existing KV ranges remain in place";
+ *   DESIGN.md reading 28).  Ranges are therefore [begin_j, begin_j+1) with at most R tokens each (kf_route_begins);
+ *   begin_j = j * R as long as no tail was redirected.  A redirect that finds no free slot or route entry is not carried
+ *   out (no error).  The marks are consumed by that one boundary.  One tiny kernel, like the route install.
  * kf_partition_state -- occupancy that the policy monitors (Algorithm 1, l.6-9): [host] active[P] (0/1),
  *   tokens[P] = committed tokens resident on each partition (x 2*H_kv*d*2 B*L = KV bytes),
  *   tails[P] = open requests whose tail range lives there.  Any pointer may be NULL.  Synchronises `stream`. */
 int kf_set_active_partitions(kf_ctx *ctx, const uint8_t *active, kf_stream stream);
+int kf_redirect_tails(kf_ctx *ctx, const uint8_t *partitions, kf_stream stream);
 /* kf_set_active_requests -- which OPEN requests take part in the following decode steps (continuous batching: a
  *   request may sit out steps without being closed; Algorithm 1 counts only "r active", l.7).  active: [device]
  *   uint8[B], non-zero = active, or NULL = all (the initial state).  A paused request keeps its routes and KV;
@@ -177,13 +183,13 @@ int kf_load_context(kf_ctx *ctx, int32_t layer, int32_t req, int32_t tok_begin, 
 int kf_token_boundary(kf_ctx *ctx, kf_stream stream);
 
 /* (a2) kf_kv_append -- the tail node appends (K_new, V_new).
- *   k_new, v_new: [device] fp16 [B][H_kv][128]; row r is written at token offset len_r - j*R of range
- *   j = len_r / R of open request r (rows of closed requests are ignored).  Does NOT advance len (all
+ *   k_new, v_new: [device] fp16 [B][H_kv][128]; row r is written at token offset len_r - begin_j of the tail range
+ *   j = n_ranges_r - 1 of open request r (begin_j = j*R unless a tail was redirected; rows of closed requests are ignored).  Does NOT advance len (all
  *   layers of a step append at the same position).  Device error ESTATE if that range has no route. */
 int kf_kv_append(kf_ctx *ctx, int32_t layer, const void *k_new, const void *v_new, kf_stream stream);
 
 /* (a3) kf_partial_attend -- local core attention per token range:
- *   for every open request r, range j < J_r = ceil((len_r+1)/R) whose partition is selected, and query
+ *   for every open request r, range j < J_r (= ceil((len_r+1)/R) unless a tail was redirected) whose partition is selected, and query
  *   head h (KV head h / G):  s_t = scale * q_h . K_t over the range's tokens,
  *       lse_part[r][j][h] = ln sum_t exp(s_t),   o_part[r][j][h][:] = sum_t exp(s_t - lse) V_t.
  *   q: [device] fp16 [B][H_q][128].  partition_mask: [host] uint8 [P] (non-zero = selected) or NULL = all.
@@ -292,6 +298,8 @@ int kf_step_graph_release(kf_graph *graph, int32_t layer_step, uint32_t seq, kf_
  * kf_launch_count: number of CUDA kernels this ctx has launched so far (host-side counter). */
 int kf_route_snapshot(kf_ctx *ctx, int32_t *len, int32_t *n_ranges, int32_t *part, int32_t *slot,
                       int32_t *free_head, int32_t *rr_cursor, kf_stream stream);
+/* kf_route_begins: begin[B][Jmax] [host] = first token position of every range (-1 where unused).  Synchronises. */
+int kf_route_begins(kf_ctx *ctx, int32_t *begin, kf_stream stream);
 int kf_status(kf_ctx *ctx, kf_stream stream);
 int64_t kf_launch_count(const kf_ctx *ctx);
 
@@ -306,8 +314,7 @@ int64_t kf_launch_count(const kf_ctx *ctx);
  *        tau_fill = (C_thresh - b_i) / g_i                                   (Eq. 2; +inf for nodes without tails)
  *        want_prewarm = tau_fill * T_step < T_prewarm and no prewarm pending or ready for i
  *        want_publish = b_i >= gamma * C_thresh and the prewarm for i is ready
- *      (want_publish stays asserted for a node that has already left the active set while its tails drain their
- *      current ranges: see the deviation note at kf_set_active_partitions)
+ *      (acting on want_publish = kf_set_active_partitions without node i, then kf_redirect_tails for node i)
  *      tokens, tails: [host] [P] as kf_partition_state returns them; prewarm_pending / prewarm_ready: [host] uint8[P]
  *      kept by the caller (a prewarm is the background bring-up of a fresh node); out: [host] [P]. */
 typedef struct kf_policy_config {

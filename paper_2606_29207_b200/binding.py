@@ -20,7 +20,7 @@ EXPORTS = [
     "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count", "kf_worker_times",
     "kf_step_graph_create", "kf_step_graph_launch", "kf_step_graph_destroy", "kf_probe_read",
     "kf_step_graph_flags", "kf_step_graph_seq", "kf_step_graph_release", "kf_signal_roundtrip",
-    "kf_set_active_partitions", "kf_partition_state", "kf_set_active_requests",
+    "kf_set_active_partitions", "kf_redirect_tails", "kf_route_begins", "kf_partition_state", "kf_set_active_requests",
     "kf_policy_bytes_per_token", "kf_policy_threshold", "kf_policy_initial_nodes", "kf_policy_step",
     "kf_wside_weight_bytes", "kf_wside_weight_offset", "kf_wside_workspace_bytes", "kf_wside_create", "kf_wside_destroy",
     "kf_wside_last_error", "kf_wside_launch_count", "kf_wside_set_sms", "kf_w_project_q", "kf_w_project_kv", "kf_w_post_attention",
@@ -110,6 +110,8 @@ def load_library():
     L.kf_step_graph_release.argtypes = [vp, i32, ctypes.c_uint32, vp]
     L.kf_signal_roundtrip.argtypes = [vp, i32, vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     L.kf_set_active_partitions.argtypes = [vp, ctypes.POINTER(ctypes.c_uint8), vp]
+    L.kf_redirect_tails.argtypes = [vp, ctypes.POINTER(ctypes.c_uint8), vp]
+    L.kf_route_begins.argtypes = [vp, ctypes.POINTER(ctypes.c_int32), vp]
     L.kf_set_active_requests.argtypes = [vp, vp, vp]
     L.kf_partition_state.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32), vp]
     pcp = ctypes.POINTER(kf_policy_config)
@@ -324,6 +326,11 @@ class KFlume:
         arr = (ctypes.c_uint8 * self.P)(*[1 if x else 0 for x in active])
         self._check(self.lib.kf_set_active_partitions(self.h, arr, self._stream(stream)), "kf_set_active_partitions")
 
+    def redirect_tails(self, partitions: Sequence[int], stream=None):
+        assert len(partitions) == self.P
+        arr = (ctypes.c_uint8 * self.P)(*[1 if x else 0 for x in partitions])
+        self._check(self.lib.kf_redirect_tails(self.h, arr, self._stream(stream)), "kf_redirect_tails")
+
     def set_active_requests(self, active=None, stream=None):
         """active: CUDA uint8 tensor [B] (non-zero = takes part in decode steps) or None = all."""
         if active is not None:
@@ -342,10 +349,13 @@ class KFlume:
         fh, cur = (i32 * self.P)(), (i32 * 1)()
         self._check(self.lib.kf_route_snapshot(self.h, ln, nr, part, slot, fh, cur, self._stream(stream)),
                     "kf_route_snapshot")
+        begin = (i32 * (self.B * self.Jmax))()
+        self._check(self.lib.kf_route_begins(self.h, begin, self._stream(stream)), "kf_route_begins")
         J = self.Jmax
         return {"len": list(ln), "n_ranges": list(nr),
                 "part": [list(part[r * J:(r + 1) * J]) for r in range(self.B)],
                 "slot": [list(slot[r * J:(r + 1) * J]) for r in range(self.B)],
+                "begin": [list(begin[r * J:(r + 1) * J]) for r in range(self.B)],
                 "free_head": list(fh), "rr_cursor": cur[0]}
 
     def status(self, stream=None) -> int:

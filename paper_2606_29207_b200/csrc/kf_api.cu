@@ -41,7 +41,7 @@ size_t max_chunks_of(const kf_config *c) {
 inline size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t len, n_ranges, route_part, route_slot, rr_cursor, rr_last, req_active, active, part_tokens, part_tails, free_head, free_cnt, free_stack, error, plan, units, chunks, recs, plan_age, sched,
+    size_t len, n_ranges, route_part, route_slot, range_begin, redirect, rr_cursor, rr_last, req_active, active, part_tokens, part_tails, free_head, free_cnt, free_stack, error, plan, units, chunks, recs, plan_age, sched,
         scratch, unit_counter, group_counter, piece_o, piece_lse, range_o, range_lse, stage_q, stage_k, stage_v,
         stage_o, stage_lse, tmaps, gates, worker_times, total;
 };
@@ -94,6 +94,8 @@ Layout make_layout(const kf_config *c) {
     L.n_ranges = take(B * 4);
     L.route_part = take(E * 4);
     L.route_slot = take(E * 4);
+    L.range_begin = take(E * 4);
+    L.redirect = take(P * 4);
     L.rr_cursor = take(4);
     L.rr_last = take(4);
     L.req_active = take(B * 4);
@@ -280,6 +282,7 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     e = cudaMemset(ws + L.len, 0xFF, (size_t)cfg->max_requests * 4);
     if (e == cudaSuccess) e = cudaMemset(ws + L.route_part, 0xFF, (size_t)cfg->max_requests * cfg->max_ranges_per_request * 4);
     if (e == cudaSuccess) e = cudaMemset(ws + L.route_slot, 0xFF, (size_t)cfg->max_requests * cfg->max_ranges_per_request * 4);
+    if (e == cudaSuccess) e = cudaMemset(ws + L.range_begin, 0xFF, (size_t)cfg->max_requests * cfg->max_ranges_per_request * 4);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     e = cudaMemset(ws + L.rr_last, 0xFF, 4);  // -1: nothing allocated yet
     if (e == cudaSuccess) {
@@ -318,6 +321,8 @@ int kf_create(kf_ctx **out, const kf_config *cfg, void *const *pool_ptrs, void *
     d.n_ranges = (int32_t *)(ws + L.n_ranges);
     d.route_part = (int32_t *)(ws + L.route_part);
     d.route_slot = (int32_t *)(ws + L.route_slot);
+    d.range_begin = (int32_t *)(ws + L.range_begin);
+    d.redirect = (int32_t *)(ws + L.redirect);
     d.rr_cursor = (int32_t *)(ws + L.rr_cursor);
     d.rr_last = (int32_t *)(ws + L.rr_last);
     d.req_active = (int32_t *)(ws + L.req_active);
@@ -556,6 +561,23 @@ int kf_set_active_partitions(kf_ctx *ctx, const uint8_t *active, kf_stream strea
         if (active[p]) mask |= 1ull << p;
     if (mask == 0) return KF_EINVAL;
     return after_launch(ctx, launch_set_active(ctx->dev, mask, (cudaStream_t)stream));
+}
+
+int kf_redirect_tails(kf_ctx *ctx, const uint8_t *partitions, kf_stream stream) {
+    if (!ctx || !partitions) return KF_EINVAL;
+    unsigned long long mask = 0;
+    for (int p = 0; p < ctx->cfg.n_partitions; ++p)
+        if (partitions[p]) mask |= 1ull << p;
+    return after_launch(ctx, launch_redirect(ctx->dev, mask, (cudaStream_t)stream));
+}
+
+int kf_route_begins(kf_ctx *ctx, int32_t *begin, kf_stream stream) {
+    if (!ctx || !begin) return KF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = cudaMemcpyAsync(begin, ctx->dev.range_begin, (size_t)ctx->dev.B * ctx->dev.Jmax * 4, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return KF_OK;
 }
 
 int kf_set_active_requests(kf_ctx *ctx, const uint8_t *active_dev, kf_stream stream) {

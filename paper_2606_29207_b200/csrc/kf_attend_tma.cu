@@ -212,7 +212,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) attend_tma_kernel(const AttendP
                 if (!((p.part_mask >> b.x) & 1ull)) continue;     // partition not selected: nothing to load
                 int n_tiles = a.z, cnt = c.x, app = -1;
                 if (c.y & kRecTail) {  // the plan may be older than this step: a tail unit has grown since
-                    const int raw = __ldg(d.len + b.z) + 1 - b.w * d.R;  // tokens of the tail range, this step's included
+                    const int raw = __ldg(d.len + b.z) + 1 - slot[3].z;  // tokens of the tail range, this step's included
                     cnt = min(d.R, raw);
                     if (c.y & kRecStretch) {
                         n_tiles = (cnt + kTileTokens - 1) / kTileTokens - a.y;

@@ -29,7 +29,7 @@ struct Unit {
     int32_t part;
     int32_t slot;
     int32_t cnt;         // tokens of this range when the plan was built (1..R); see live_extent() for tail units
-    int32_t tail;        // 1: this is the request's LAST range: it grows by one token per step
+    int32_t tail;        // != 0: this is the request's LAST range (it grows by one token per step); value = range_begin + 1
     int32_t piece_begin; // first global piece index of this unit (pieces of a unit are consecutive, tile order)
     int32_t n_pieces;    // pieces = chunks this unit is cut into
 };
@@ -58,7 +58,7 @@ struct alignas(64) ChunkRec {
                        // last tile of a tail unit -- the one chunk that grows while the plan is kept (live_tiles())
     int32_t n_pieces;  // pieces of the unit
     int32_t J;         // ranges of the request in this plan
-    int32_t pad[4];
+    int32_t pad[4];    // [2] = range_begin of the unit; [0], [1] are filled in by the worker (q staged, append offset)
 };
 constexpr int kRecTail = 1, kRecStretch = 2;
 
@@ -92,6 +92,8 @@ struct Dev {
     int32_t *n_ranges;   // [B]
     int32_t *route_part; // [B][Jmax]
     int32_t *route_slot; // [B][Jmax]
+    int32_t *range_begin; // [B][Jmax] first token position of range j (j * R unless a tail was redirected, reading 28)
+    int32_t *redirect;   // [P]   1: tails on this partition move to a new range at the next token boundary (one-shot)
     int32_t *rr_cursor;  // [1]   ranges allocated so far
     int32_t *rr_last;    // [1]   partition of the last allocation (-1: none yet)
     int32_t *req_active; // [B]   1: the request takes part in decode steps (kf_set_active_requests); 0: paused
@@ -154,7 +156,7 @@ __device__ __forceinline__ void set_error(const Dev &d, int code) { atomicCAS(d.
 // of a tail unit (always the last chunk of scheduling level 0: one of the first and largest chunks) is stretched
 // to the live end.  Every other chunk is exactly as planned.
 __device__ __forceinline__ int live_cnt(const Dev &d, const Unit &un) {
-    return un.tail ? min(d.R, __ldg(d.len + un.req) + 1 - un.range * d.R) : un.cnt;
+    return un.tail ? min(d.R, __ldg(d.len + un.req) + 1 - (un.tail - 1)) : un.cnt;
 }
 __device__ __forceinline__ int live_tiles(const Unit &un, int cnt_live, int tile_begin, int n_tiles) {
     const int planned = (un.cnt + kTileTokens - 1) / kTileTokens;
@@ -166,8 +168,8 @@ __device__ __forceinline__ int live_tiles(const Unit &un, int cnt_live, int tile
 // a request whose boundary could not get a slot (ENOSPC) appended nothing, so it must not move on -- the next
 // kf_token_boundary re-tries the allocation at the same position (reading 24).
 __device__ __forceinline__ bool commits(const Dev &d, int r) {
-    const int len = d.len[r];
-    return len >= 0 && d.req_active[r] && (long long)d.n_ranges[r] * d.R > len;
+    const int len = d.len[r], nr = d.n_ranges[r];
+    return len >= 0 && d.req_active[r] && nr > 0 && len - d.range_begin[(size_t)r * d.Jmax + nr - 1] < d.R;
 }
 
 // byte offset (within a partition pool) of K row (layer, slot, g, t)
@@ -183,6 +185,7 @@ int launch_plan(const Dev &d, int do_boundary, cudaStream_t s);  // (a1, optiona
 int plan_setup();        // cudaFuncSetAttribute for the plan kernel's dynamic shared memory; 0 or KF_ECUDA
 int launch_step_commit(const Dev &d, cudaStream_t s);
 int launch_set_active(const Dev &d, unsigned long long mask, cudaStream_t s);
+int launch_redirect(const Dev &d, unsigned long long mask, cudaStream_t s);
 int launch_set_req_active(const Dev &d, const unsigned char *mask_dev, cudaStream_t s);
 int launch_partition_state(const Dev &d, long long *tokens, int *tails, cudaStream_t s);
 int launch_load_context(const Dev &d, int layer, int req, int tok_begin, int n_tokens, const __half *k,

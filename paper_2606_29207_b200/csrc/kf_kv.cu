@@ -13,8 +13,13 @@ __global__ void __launch_bounds__(256) load_context_kernel(Dev d, int layer, int
     if (t >= n_tokens) return;
     const int g = blockIdx.y, is_v = blockIdx.z;
     const int pos = tok_begin + t;
-    const int j = pos / d.R, off = pos - j * d.R;
-    if (d.len[req] < 0 || j >= d.n_ranges[req]) {
+    // range that holds position pos: begin_j <= pos < begin_j+1 (j * R unless a tail was redirected, reading 28)
+    const int nr = d.len[req] < 0 ? 0 : d.n_ranges[req];
+    const int *bg = d.range_begin + (size_t)req * d.Jmax;
+    int j = min(pos / d.R, nr - 1);
+    while (j + 1 < nr && bg[j + 1] <= pos) ++j;
+    const int off = nr > 0 ? pos - bg[j] : 0;
+    if (nr == 0 || off >= d.R) {
         if (c == 0 && g == 0 && is_v == 0) set_error(d, KF_ESTATE);
         return;
     }
@@ -31,8 +36,9 @@ __global__ void __launch_bounds__(256) kv_append_kernel(Dev d, int layer, const 
     const int r = blockIdx.x;
     const int len = d.len[r];
     if (len < 0 || !d.req_active[r]) return;
-    const int j = len / d.R, off = len - j * d.R;
-    if (j >= d.n_ranges[r]) {
+    const int j = d.n_ranges[r] - 1;  // the tail range
+    const int off = j >= 0 ? len - d.range_begin[(size_t)r * d.Jmax + j] : d.R;
+    if (off >= d.R) {  // no route for position len
         if (threadIdx.x == 0) set_error(d, KF_ESTATE);
         return;
     }
@@ -64,8 +70,9 @@ __global__ void __launch_bounds__(256) kv_append_stage_kernel(Dev d, int layer, 
     if (blockIdx.y != 0) return;
     const int len = d.len[r];
     if (len < 0 || !d.req_active[r]) return;
-    const int j = len / d.R, off = len - j * d.R;
-    if (j >= d.n_ranges[r]) {
+    const int j = d.n_ranges[r] - 1;  // the tail range
+    const int off = j >= 0 ? len - d.range_begin[(size_t)r * d.Jmax + j] : d.R;
+    if (off >= d.R) {  // no route for position len
         if (threadIdx.x == 0) set_error(d, KF_ESTATE);
         return;
     }

@@ -9,10 +9,12 @@ namespace kf {
 // allocation: one global round-robin cursor, per-partition LIFO free list then bump allocator
 // (reading 9).  Called by a single thread.
 // ------------------------------------------------------------------------------------------------
-__device__ bool alloc_range(const Dev &d, int req) {
+// `begin` = first token position of the new range; `quiet`: a failure is not an error (a tail redirect that finds no
+// room is simply not carried out, reading 28).
+__device__ bool alloc_range(const Dev &d, int req, int begin, bool quiet = false) {
     const int j = d.n_ranges[req];
     if (j >= d.Jmax) {
-        set_error(d, KF_ENOSPC);
+        if (!quiet) set_error(d, KF_ENOSPC);
         return false;
     }
     // round-robin over the ACTIVE partitions: the first active one after the partition used last, cyclically
@@ -30,7 +32,7 @@ __device__ bool alloc_range(const Dev &d, int req) {
         }
     }
     if (p < 0) {
-        set_error(d, KF_ENOSPC);
+        if (!quiet) set_error(d, KF_ENOSPC);
         return false;
     }
     const int nfree = d.free_cnt[p];
@@ -43,6 +45,7 @@ __device__ bool alloc_range(const Dev &d, int req) {
         d.free_head[p] = slot + 1;
     d.route_part[(size_t)req * d.Jmax + j] = p;
     d.route_slot[(size_t)req * d.Jmax + j] = slot;
+    d.range_begin[(size_t)req * d.Jmax + j] = begin;
     d.n_ranges[req] = j + 1;
     return true;
 }
@@ -58,7 +61,7 @@ __global__ void open_request_kernel(Dev d, int req, int n_tokens) {
     d.n_ranges[req] = 0;
     const int J = (int)(((int64_t)n_tokens + d.R - 1) / d.R);
     for (int j = 0; j < J; ++j)
-        if (!alloc_range(d, req)) break;
+        if (!alloc_range(d, req, j * d.R)) break;
 }
 
 __global__ void close_request_kernel(Dev d, int req) {
@@ -76,6 +79,7 @@ __global__ void close_request_kernel(Dev d, int req) {
         d.free_cnt[p] += 1;
         d.route_part[(size_t)req * d.Jmax + j] = -1;
         d.route_slot[(size_t)req * d.Jmax + j] = -1;
+        d.range_begin[(size_t)req * d.Jmax + j] = -1;
     }
     d.n_ranges[req] = 0;
     d.len[req] = -1;
@@ -87,24 +91,35 @@ __device__ int token_boundary_warp(const Dev &d, int lane) {
     int opened = 0;
     for (int base = 0; base < d.B; base += 32) {
         const int r = base + lane;
-        bool need = false;
+        bool need = false, redir = false;
         if (r < d.B) {
             const int len = d.len[r];
-            // the tail position has no route yet: the tail range is full (len % R == 0) -- or an earlier boundary
-            // could not get a slot for it (ENOSPC) and the request has been waiting since (reading 24)
-            need = len >= 0 && d.req_active[r] && (long long)d.n_ranges[r] * d.R <= len;
+            if (len >= 0 && d.req_active[r]) {
+                const int nr = d.n_ranges[r];
+                const int bt = nr > 0 ? d.range_begin[(size_t)r * d.Jmax + nr - 1] : 0;
+                // the tail position has no route yet: the tail range is full (len - begin == R; len % R == 0 without
+                // redirects) -- or an earlier boundary could not get a slot for it (ENOSPC) and the request has been
+                // waiting since (reading 24)
+                need = nr == 0 || len - bt >= d.R;
+                // reading 28 (Algorithm 1 l.16-17): the tail lives on a node whose tails are being redirected and holds
+                // at least one token: close it here, continue in a new range that begins at position len
+                redir = !need && len > bt && d.redirect[d.route_part[(size_t)r * d.Jmax + nr - 1]] != 0;
+            }
         }
-        unsigned m = __ballot_sync(0xffffffffu, need);
+        const unsigned mr = __ballot_sync(0xffffffffu, redir);
+        unsigned m = __ballot_sync(0xffffffffu, need) | mr;
         opened += __popc(m);
         if (lane == 0) {
             while (m) {
                 const int b = __ffs(m) - 1;
                 m &= m - 1;
-                alloc_range(d, base + b);
+                alloc_range(d, base + b, d.len[base + b], (mr >> b) & 1u);
             }
         }
         __syncwarp();
     }
+    if (lane < d.P) d.redirect[lane] = 0;  // the marks are consumed by this boundary (P <= 64: two passes)
+    if (lane + 32 < d.P) d.redirect[lane + 32] = 0;
     return opened;
 }
 
@@ -112,6 +127,12 @@ __device__ int token_boundary_warp(const Dev &d, int lane) {
 __global__ void set_active_kernel(Dev d, unsigned long long mask) {
     const int p = threadIdx.x;
     if (p < d.P) d.active[p] = (int)((mask >> p) & 1ull);
+}
+
+// mark partitions whose tails move at the next token boundary (Algorithm 1 l.17, reading 28)
+__global__ void redirect_kernel(Dev d, unsigned long long mask) {
+    const int p = threadIdx.x;
+    if (p < d.P) d.redirect[p] = (int)((mask >> p) & 1ull);
 }
 
 // which open requests take part in the following decode steps (continuous batching: a request may pause);
@@ -132,7 +153,8 @@ __global__ void partition_state_kernel(Dev d, long long *tokens, int *tails) {
     const int J = d.n_ranges[r];
     for (int j = 0; j < J; ++j) {
         const int p = d.route_part[(size_t)r * d.Jmax + j];
-        const long long cnt = max(0, min(d.R, len - j * d.R));
+        const int bj = d.range_begin[(size_t)r * d.Jmax + j];
+        const long long cnt = j + 1 < J ? d.range_begin[(size_t)r * d.Jmax + j + 1] - bj : max(0, min(d.R, len - bj));
         atomicAdd(reinterpret_cast<unsigned long long *>(tokens + p), (unsigned long long)cnt);
         if (j == J - 1 && d.req_active[r]) atomicAdd(tails + p, 1);  // "r active" (Alg. 1 l.7)
     }
@@ -295,12 +317,14 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
     for (int r = tid; r < B; r += nt) {
         const int len = d.len[r];
         int64_t S = (len >= 0 && d.req_active[r]) ? (int64_t)len + 1 : 0;  // closed or paused: no work this step
-        int J = (int)((S + d.R - 1) / d.R);
         const int nr = d.n_ranges[r];
-        if (J > nr) {  // no route for the tail position: kf_token_boundary was not called
-            set_error(d, KF_ESTATE);
-            J = nr;
-            S = (int64_t)nr * d.R;
+        int J = S > 0 ? nr : 0;
+        if (S > 0) {
+            const int bt = nr > 0 ? d.range_begin[(size_t)r * d.Jmax + nr - 1] : 0;
+            if (nr == 0 || len - bt >= d.R) {  // no route for the tail position: kf_token_boundary was not called
+                set_error(d, KF_ESTATE);
+                S = nr == 0 ? 0 : (int64_t)bt + d.R;
+            }
         }
         Jr[r] = J;
         Sr[r] = (int)S;
@@ -319,7 +343,8 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
     for (int e = tid; e < E; e += nt) {
         const int r = last_le(epre, B + 1, e);
         const int j = e - epre[r];
-        const int cnt = min(d.R, Sr[r] - j * d.R);
+        const int *bg = d.range_begin + (size_t)r * d.Jmax;
+        const int cnt = (j + 1 < Jr[r] ? bg[j + 1] : Sr[r]) - bg[j];  // ranges are [begin_j, begin_j+1); the tail ends at S
         const int tiles = (cnt + T - 1) / T;
         etiles[e] = tiles;
         tpre[e] = tiles * Hkv;
@@ -413,10 +438,12 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
         const int slot = d.route_slot[(size_t)r * d.Jmax + j];
         rec.req = r;
         rec.range = j;
-        rec.cnt = min(d.R, Sr[r] - j * d.R);
+        const int *bg = d.range_begin + (size_t)r * d.Jmax;
+        rec.cnt = (j + 1 < Jr[r] ? bg[j + 1] : Sr[r]) - bg[j];
         rec.n_pieces = pu;
         rec.J = Jr[r];
-        rec.pad[0] = rec.pad[1] = rec.pad[2] = rec.pad[3] = 0;
+        rec.pad[0] = rec.pad[1] = rec.pad[3] = 0;
+        rec.pad[2] = bg[j];
         const int tail = j == Jr[r] - 1 ? kRecTail : 0;
         for (int i = 0; i < c; ++i) {
             const int t0 = b0 + i * cq + min(i, cr);
@@ -448,8 +475,9 @@ __global__ void __launch_bounds__(1024, 1) plan_kernel(Dev d, int do_boundary) {
         un.range = j;
         un.part = d.route_part[(size_t)r * d.Jmax + j];
         un.slot = d.route_slot[(size_t)r * d.Jmax + j];
-        un.cnt = min(d.R, Sr[r] - j * d.R);
-        un.tail = j == Jr[r] - 1 ? 1 : 0;
+        const int *bg = d.range_begin + (size_t)r * d.Jmax;
+        un.cnt = (j + 1 < Jr[r] ? bg[j + 1] : Sr[r]) - bg[j];
+        un.tail = j == Jr[r] - 1 ? bg[j] + 1 : 0;
         un.piece_begin = ppre[e] * Hkv + g * pu;
         un.n_pieces = pu;
         d.units[u] = un;
@@ -492,6 +520,10 @@ int plan_setup() {
 }
 int launch_set_active(const Dev &d, unsigned long long mask, cudaStream_t s) {
     set_active_kernel<<<1, kMaxPartitions, 0, s>>>(d, mask);
+    return 1;
+}
+int launch_redirect(const Dev &d, unsigned long long mask, cudaStream_t s) {
+    redirect_kernel<<<1, kMaxPartitions, 0, s>>>(d, mask);
     return 1;
 }
 int launch_set_req_active(const Dev &d, const unsigned char *mask_dev, cudaStream_t s) {

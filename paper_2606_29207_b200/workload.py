@@ -18,7 +18,7 @@ from .binding import (KF_IMPL_AUTO, KF_W_DOWN, KF_W_GATE, KF_W_KV, KF_W_O, KF_W_
 class Session:
     def __init__(self, wl: Workload, impl: int = KF_IMPL_AUTO, n_layers_phys: Optional[int] = None,
                  steps: Optional[int] = None, min_tiles: int = 0, device: str = "cuda:0", softmax_scale: float = 0.0,
-                 slack_slots: int = 0, **tuning):
+                 slack_slots: int = 0, slack_ranges: int = 0, **tuning):
         import torch
         self.torch = torch
         self.wl = wl
@@ -26,7 +26,7 @@ class Session:
         self.L_phys = wl.n_layers if n_layers_phys is None else n_layers_phys
         self.len0: List[int] = [s - 1 for s in wl.contexts]      # tokens resident before step 0
         cfg = make_config(wl.n_q_heads, wl.n_kv_heads, wl.range_tokens, wl.n_partitions, wl.batch,
-                          wl.max_ranges(self.steps), wl.slots_per_partition(self.steps) + slack_slots,
+                          wl.max_ranges(self.steps) + slack_ranges, wl.slots_per_partition(self.steps) + slack_slots,
                           n_layers=self.L_phys, softmax_scale=softmax_scale, attend_impl=impl,
                           min_tiles_per_worker=min_tiles, **tuning)
         self.kf = KFlume(cfg, device)
