@@ -94,7 +94,7 @@ def test_scale_up_and_down_during_graph_replay_matches_model_and_oracle():
 
 
 # ---- Algorithm 1 closed loop: the library's controller drives the device routing table -----------------------------
-def _controller_loop(steps, P, state_fn, decide_fn, publish_fn, step_fn, prewarm_steps=3):
+def _controller_loop(steps, P, state_fn, decide_fn, publish_fn, step_fn, prewarm_steps=3, redirect_fn=None):
     """The per-step monitor of Algorithm 1 around an abstract backend.  A node that reaches its watermark with a ready
     prewarm leaves the active set and the lowest-numbered idle node joins it: "redirect active tails on i to
     prewarm[i]" (l.17) under the fixed-R reading -- the tails move as their current ranges fill.  The joining node is a
@@ -117,6 +117,8 @@ def _controller_loop(steps, P, state_fn, decide_fn, publish_fn, step_fn, prewarm
                 active[i] = 0
                 ready[i] = False
                 publish_fn(active)
+                if redirect_fn is not None:   # l.17 literally (reading 28): node i's tails move at the next boundary
+                    redirect_fn([1 if p == i else 0 for p in range(P)])
         for i in range(P):
             if pending[i]:
                 countdown[i] -= 1
@@ -175,6 +177,65 @@ def test_algorithm1_closed_loop_device_equals_model():
     assert sum(1 for x in final_tokens if x > 0) >= 3
     # a node stops receiving ranges once published away; it may still grow until its tails' current ranges fill
     assert max(final_tokens[:3]) <= 400 + wl.batch * R        # (the last node has no successor to hand over to)
+    ses.close()
+
+
+def test_algorithm1_closed_loop_with_tail_redirect_stops_growth_at_once():
+    # the same controller, acting on want_publish as Algorithm 1 l.16-17 says: publish the route AND redirect the active
+    # tails of node i (kf_redirect_tails, reading 28).  Device == model every step, and a retired node holds exactly
+    # what it held at the boundary after the publish -- no overshoot of up to (tails * R) tokens as under reading 20.
+    from oracle import policy as opol
+    from paper_2606_29207_b200 import Policy
+    P, R, steps = 4, 32, 200
+    wl = Workload("alg1r", 32, 8, R, P, [70, 31, 33, 100, 64])
+    kw = dict(beta_mem=1.0, beta_slo=1.0, gamma=0.8, t_a_max_s=1.0, bw_hbm=1e30, c_kv_cap=4096.0 * 400,
+              t_step_s=1.0, t_prewarm_s=3.0, n_kv_heads=8, head_dim=128, n_layers=1)
+    pol, oc = Policy(**kw), opol.PolicyConstants(**kw)
+    ses = Session(wl, steps=steps, slack_slots=16, slack_ranges=8)
+    kf = ses.kf
+    kf.set_active_partitions([1, 0, 0, 0])
+    ses.prepare()
+
+    def gpu_step(t):
+        kf.token_boundary()
+        q, (kn, vn) = ses.q_for(0, t), ses.kv_new_for(0, t)
+        ses.layer_step(0, q, kn, vn, one_launch=True)
+        kf.step_commit()
+        if t % 9 == 0 or t == steps - 1:
+            o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+            for r, S0 in enumerate(wl.contexts):
+                o_ref, lse_ref = oracle_request(wl, 0, r, t, S0 + t)
+                check_close(o[r], lse[r], o_ref, lse_ref, f"alg1r step{t} r{r}")
+
+    h_gpu = _controller_loop(steps, P, kf.partition_state, pol.step, kf.set_active_partitions, gpu_step,
+                             redirect_fn=kf.redirect_tails)
+    model = RoutingModel(P, R, wl.batch, kf.Jmax, kf.cfg.slots_per_partition)
+    model.set_active([1, 0, 0, 0])
+    for r, n in enumerate(ses.len0):
+        model.open_request(r, n)
+
+    def model_step(t):
+        model.token_boundary()
+        model.step_commit()
+
+    h_model = _controller_loop(steps, P, model.partition_state,
+                               lambda tok, tails, pe, re: opol.monitor(oc, tok, tails, pe, re), model.set_active,
+                               model_step, redirect_fn=model.redirect_tails)
+    assert h_gpu == h_model
+    snap, ms = kf.route_snapshot(), model.snapshot()
+    for key in ("len", "n_ranges", "part", "slot", "begin", "free_head", "rr_cursor"):
+        assert snap[key] == ms[key], key
+    assert kf.status() == KF_OK
+    n_events = 0
+    for t in range(1, steps - 1):
+        a0, a1 = h_gpu[t - 1][0], h_gpu[t][0]
+        for i in range(P):
+            if a0[i] and not a1[i]:                       # node i was published away during iteration t - 1 ...
+                n_events += 1
+                assert h_gpu[t][2][i] > 0 or h_gpu[t][1][i] > 0
+                assert h_gpu[t + 1][2][i] == 0            # ... one boundary later it holds no tail any more
+                assert all(h[1][i] == h_gpu[t + 1][1][i] for h in h_gpu[t + 1:])   # and never grows again
+    assert n_events >= 2
     ses.close()
 
 
