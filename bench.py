@@ -902,7 +902,7 @@ def main():
                     "(PAPER.md:252-280) instead of the decode benchmark")
     ap.add_argument("--pipe-cases", default="16x2048,16x8192,16x16384,32x4096,64x2048,64x8192,128x2048,128x4096,128x16384",
                     help="--pipeline workloads: B_mu x seq (Fig. 11: batch 16-128, sequence 2K-16K)")
-    ap.add_argument("--pipe-sms", default="148,132,116,100,84", help="attend SM budgets tried by --pipeline / --sm-sweep")
+    ap.add_argument("--pipe-sms", default="148,116,100,84,68", help="attend SM budgets tried by --pipeline / --sm-sweep")
     ap.add_argument("--pipe-layers", type=int, default=8, help="layers per step in --pipeline")
     ap.add_argument("--sm-sweep", action="store_true", help="kf_attend GB/s against its SM budget")
     args = ap.parse_args()
