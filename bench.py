@@ -48,11 +48,12 @@ SUB_STEPS = {"cfg1": (200, 10, 50), "cfg2": (100, 10, 50), "cfg3": (100, 10, 40)
 # line carries `traffic` only when the running sources hash to the same value and no tuning flag is set.
 NCU_TRAFFIC = {
     # workload: (bytes per launch, committed summary, kernel_rev at capture time)
-    "cfg1": (16939392, "profiles/r01g_attend_full_cfg1.md", "r01"),
-    "cfg2": (1085991552, "profiles/r01g_attend_full_cfg2.md", "r01"),
-    "cfg3": (4782093992, "profiles/r01g_attend_full_cfg3.md", "r01"),
-    "cfg4": (4307839832, "profiles/r01g_attend_full_cfg4.md", "r01"),
-    "cfg5": (37122728208, "profiles/r01g_attend_full_cfg5.md", "r01"),
+    "cfg1": (16982400, "profiles/r02c_attend_full_cfg1.md", "a39d3ecfd9ff"),
+    "cfg2": (1086072536, "profiles/r02c_attend_full_cfg2.md", "a39d3ecfd9ff"),
+    "cfg3": (4782946188, "profiles/r02c_attend_full_cfg3.md", "a39d3ecfd9ff"),
+    "cfg4": (4306954112, "profiles/r02c_attend_full_cfg4.md", "a39d3ecfd9ff"),
+    "cfg5": (37122581380, "profiles/r02c_attend_full_cfg5.md", "a39d3ecfd9ff"),
+    "fig10_q64kv8_b32_s32k": (4311526756, "profiles/r02c_attend_full_fig10_q64kv8_b32_s32k.md", "a39d3ecfd9ff"),
 }
 
 
