@@ -19,6 +19,8 @@
 //     without draining at tile boundaries, two TMEM accumulator buffers let the epilogue of one tile overlap the MMAs
 //     of the next; a tile that several spans share goes through L2 as fp32 pieces which a small fix-up kernel adds
 //     in k order (deterministic; no CTA ever waits for another one, so any SM budget is safe) and writes as fp16;
+//   * programmatic dependent launch along the kernel chain of a W-side call: the set-up of a kernel (barriers, TMEM,
+//     descriptors) overlaps the tail of its predecessor;
 //   * the gate and up projections of the FFN run as two accumulators of the same CTA (two weight tiles per stage,
 //     one shared activation tile), so SwiGLU is applied in the epilogue and g, u never exist in memory.
 #include <cuda.h>
@@ -161,6 +163,11 @@ __global__ void __launch_bounds__(kWgThreads, 1)
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = tmem_base_s;
+    // Programmatic dependent launch along the chain of a W-side call: everything above (barriers, TMEM, descriptor
+    // prefetch) touches no global memory and overlaps the tail of the preceding kernel; nothing below runs before that
+    // kernel has completed.  The successor may set itself up from here on.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     if (warp == 0) {
         if (lane == 0) {
@@ -281,6 +288,8 @@ __global__ void __launch_bounds__(kWgThreads, 1)
 // One thread per (feature, batch row); every piece is read once, coalesced along the features.  grid (tiles, ceil(B / 8)).
 template <bool DUAL>
 __global__ void __launch_bounds__(kWgTileN * 8) wgemm_fixup_kernel(const WGemmArgs a, int nb) {
+    asm volatile("griddepcontrol.wait;" ::: "memory");  // launched while the GEMM is still running (PDL)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const int tile = blockIdx.x, row = threadIdx.x, b = blockIdx.y * 8 + threadIdx.y;
     const int nkb = a.nkb;
     const int total = (a.N / kWgTileN) * nkb;
@@ -313,6 +322,7 @@ __global__ void __launch_bounds__(kWgTileN * 8) wgemm_fixup_kernel(const WGemmAr
 
 // o [rows][cols] fp32 -> fp16 (the attention output that feeds W_O)
 __global__ void cast_o_kernel(const float *__restrict__ o, __half *__restrict__ o16, size_t n4) {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");  // the W_O GEMM may set itself up meanwhile
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
         const float4 v = __ldg(reinterpret_cast<const float4 *>(o) + i);
         __half2 a = __floats2half2_rn(v.x, v.y), b = __floats2half2_rn(v.z, v.w);
@@ -324,7 +334,7 @@ __global__ void cast_o_kernel(const float *__restrict__ o, __half *__restrict__ 
 }
 
 template <int NB, bool DUAL>
-static int launch_one(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGemmArgs &a, cudaStream_t s) {
+static int launch_one(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGemmArgs &a, bool pdl, cudaStream_t s) {
     const int smem = wgemm_smem_bytes(NB, DUAL);
     static bool configured = false;  // per instantiation
     if (!configured) {
@@ -332,17 +342,32 @@ static int launch_one(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGem
             return KF_ECUDA;
         configured = true;
     }
-    wgemm_kernel<NB, DUAL><<<a.n_ctas, kWgThreads, smem, s>>>(tmW, tmX, a);
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(a.n_ctas);
+    cfg.blockDim = dim3(kWgThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;  // only behind a kernel of the same W-side call (see the kernel's griddepcontrol.wait)
+    cudaLaunchKernelEx(&cfg, wgemm_kernel<NB, DUAL>, tmW, tmX, a);
     // tiles shared between spans exist unless every span boundary is a tile boundary
     const int tiles = a.N / kWgTileN, total = tiles * a.nkb, per = (total + a.n_ctas - 1) / a.n_ctas;
     if (per % a.nkb == 0) return 1;
-    wgemm_fixup_kernel<DUAL><<<dim3(tiles, (a.B + 7) / 8), dim3(kWgTileN, 8), 0, s>>>(a, NB);
+    cfg.gridDim = dim3(tiles, (a.B + 7) / 8);
+    cfg.blockDim = dim3(kWgTileN, 8);
+    cfg.dynamicSmemBytes = 0;
+    cfg.numAttrs = 1;            // the fix-up always follows its GEMM
+    cudaLaunchKernelEx(&cfg, wgemm_fixup_kernel<DUAL>, a, (int)NB);
     return 2;
 }
 
-int launch_wgemm(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGemmArgs &a, int nb, bool dual, cudaStream_t s) {
+int launch_wgemm(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGemmArgs &a, int nb, bool dual, bool pdl,
+                 cudaStream_t s) {
 #define KF_WG(NBv)                                                          \
-    if (nb == NBv) return dual ? launch_one<NBv, true>(tmW, tmX, a, s) : launch_one<NBv, false>(tmW, tmX, a, s);
+    if (nb == NBv) return dual ? launch_one<NBv, true>(tmW, tmX, a, pdl, s) : launch_one<NBv, false>(tmW, tmX, a, pdl, s);
     KF_WG(16) KF_WG(32) KF_WG(64) KF_WG(128)
 #undef KF_WG
     return KF_EINVAL;

@@ -125,7 +125,7 @@ int encode(kf_wside *w, CUtensorMap *map, const void *base, size_t rows, size_t 
 
 // out segments [0, e0) -> o0, [e0, e1) -> o1: one GEMM x [B][K] . W(m)^T
 int gemm(kf_wside *w, int layer, int m, const void *x, int batch, __half *o0, int ld0, int e0, __half *o1, int ld1,
-         cudaStream_t s) {
+         cudaStream_t s, bool pdl = false) {
     const kf_wside_config *c = &w->cfg;
     const bool dual = m == kMatGU;
     const int K = (int)cols_of(c, m);
@@ -152,7 +152,7 @@ int gemm(kf_wside *w, int layer, int m, const void *x, int batch, __half *o0, in
     a.ld[2] = a.ld[1];
     a.partial = w->partial;
     a.up_row_offset = dual ? c->ffn : 0;
-    rc = launch_wgemm(w->maps[layer * 5 + m], tmX, a, nb, dual, s);
+    rc = launch_wgemm(w->maps[layer * 5 + m], tmX, a, nb, dual, pdl, s);
     if (rc < 0) return rc;
     w->launches += rc;
     const cudaError_t e = cudaPeekAtLastError();
@@ -280,9 +280,10 @@ int kf_w_post_attention(kf_wside *w, int32_t layer, const float *o, int32_t batc
     const int qd = c->n_q_heads * 128;
     launch_cast_o(o, w->o16, (size_t)batch * qd, s);
     w->launches += 1;
-    int rc = gemm(w, layer, kMatO, w->o16, batch, w->y, c->hidden, c->hidden, nullptr, 0, s);
-    if (rc == KF_OK) rc = gemm(w, layer, kMatGU, w->y, batch, w->h, c->ffn, c->ffn, nullptr, 0, s);
-    if (rc == KF_OK) rc = gemm(w, layer, kMatD, w->h, batch, (__half *)x_next, c->hidden, c->hidden, nullptr, 0, s);
+    // the three GEMMs follow kernels of this very call: programmatic dependent launches (kf_wgemm.cu)
+    int rc = gemm(w, layer, kMatO, w->o16, batch, w->y, c->hidden, c->hidden, nullptr, 0, s, true);
+    if (rc == KF_OK) rc = gemm(w, layer, kMatGU, w->y, batch, w->h, c->ffn, c->ffn, nullptr, 0, s, true);
+    if (rc == KF_OK) rc = gemm(w, layer, kMatD, w->h, batch, (__half *)x_next, c->hidden, c->hidden, nullptr, 0, s, true);
     return rc;
 }
 
