@@ -285,39 +285,57 @@ __global__ void __launch_bounds__(kWgThreads, 1)
 }
 
 // Fix-up of the tiles that several spans share: out[b][n] = epilogue(sum over the pieces, in k order = ascending CTA).
-// One thread per (feature, batch row); every piece is read once, coalesced along the features.  grid (tiles, ceil(B / 8)).
+// One thread per (4 consecutive features, batch row): every piece is read once with 128-bit loads, coalesced along the
+// features, all pieces of the thread in flight at once; 8-byte stores.  grid (tiles, ceil(B / 32)), block (32, 32).
 template <bool DUAL>
-__global__ void __launch_bounds__(kWgTileN * 8) wgemm_fixup_kernel(const WGemmArgs a, int nb) {
+__global__ void __launch_bounds__(1024) wgemm_fixup_kernel(const WGemmArgs a, int nb) {
     asm volatile("griddepcontrol.wait;" ::: "memory");  // launched while the GEMM is still running (PDL)
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    const int tile = blockIdx.x, row = threadIdx.x, b = blockIdx.y * 8 + threadIdx.y;
+    const int tile = blockIdx.x, row = threadIdx.x * 4, b = blockIdx.y * 32 + threadIdx.y;
     const int nkb = a.nkb;
     const int total = (a.N / kWgTileN) * nkb;
     const int per = (total + a.n_ctas - 1) / a.n_ctas;
-    const int c_first = (tile * nkb) / per, c_last = ((tile + 1) * nkb - 1) / per;
+    const int k_lo = tile * nkb, k_hi = k_lo + nkb;  // the tile's k-blocks in the flat (tile, k-block) sequence
+    const int c_first = k_lo / per, c_last = (k_hi - 1) / per;
     if (c_first == c_last || b >= a.B) return;  // the tile was whole: its CTA stored the result itself
     const size_t slot_floats = (size_t)nb * kWgTileN * (DUAL ? 2 : 1);
-    float g = 0.f, u = 0.f;
+    float4 g = make_float4(0.f, 0.f, 0.f, 0.f), u = g;
     for (int c0 = c_first; c0 <= c_last; c0 += 8) {
-        float t[8], tu[8];
+        float4 t[8], tu[8];
 #pragma unroll
         for (int e = 0; e < 8; ++e) {
             const int c = c0 + e;
-            const int slot = ((c * per) / nkb == tile) ? 0 : 1;  // slot 0 holds the span's first segment
+            const int start = c * per;  // slot 0 holds the span's first segment: the span starts inside this tile
+            const int slot = (start >= k_lo && start < k_hi) ? 0 : 1;
             const float *pp = a.partial + ((size_t)c * 2 + slot) * slot_floats + row;
-            t[e] = c <= c_last ? __ldcg(pp + (size_t)b * kWgTileN) : 0.f;
-            if (DUAL) tu[e] = c <= c_last ? __ldcg(pp + (size_t)(nb + b) * kWgTileN) : 0.f;
+            t[e] = c <= c_last ? __ldcg(reinterpret_cast<const float4 *>(pp + (size_t)b * kWgTileN)) : make_float4(0.f, 0.f, 0.f, 0.f);
+            if (DUAL)
+                tu[e] = c <= c_last ? __ldcg(reinterpret_cast<const float4 *>(pp + (size_t)(nb + b) * kWgTileN))
+                                    : make_float4(0.f, 0.f, 0.f, 0.f);
         }
 #pragma unroll
         for (int e = 0; e < 8; ++e) {
-            g += t[e];
-            if (DUAL) u += tu[e];
+            g.x += t[e].x;
+            g.y += t[e].y;
+            g.z += t[e].z;
+            g.w += t[e].w;
+            if (DUAL) {
+                u.x += tu[e].x;
+                u.y += tu[e].y;
+                u.z += tu[e].z;
+                u.w += tu[e].w;
+            }
         }
     }
     const int n = tile * kWgTileN + row;
     const int sg = (tile * kWgTileN >= a.seg_end[0]) + (tile * kWgTileN >= a.seg_end[1]);
-    __half *out = a.out[sg] + (n - (sg == 0 ? 0 : a.seg_end[sg - 1]));
-    out[(size_t)b * a.ld[sg]] = __float2half_rn(DUAL ? silu_mul(g, u) : g);
+    __half *out = a.out[sg] + (n - (sg == 0 ? 0 : a.seg_end[sg - 1])) + (size_t)b * a.ld[sg];
+    const __half2 lo = __floats2half2_rn(DUAL ? silu_mul(g.x, u.x) : g.x, DUAL ? silu_mul(g.y, u.y) : g.y);
+    const __half2 hi = __floats2half2_rn(DUAL ? silu_mul(g.z, u.z) : g.z, DUAL ? silu_mul(g.w, u.w) : g.w);
+    uint2 w;
+    w.x = *reinterpret_cast<const uint32_t *>(&lo);
+    w.y = *reinterpret_cast<const uint32_t *>(&hi);
+    *reinterpret_cast<uint2 *>(out) = w;
 }
 
 // o [rows][cols] fp32 -> fp16 (the attention output that feeds W_O)
@@ -356,8 +374,8 @@ static int launch_one(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGem
     // tiles shared between spans exist unless every span boundary is a tile boundary
     const int tiles = a.N / kWgTileN, total = tiles * a.nkb, per = (total + a.n_ctas - 1) / a.n_ctas;
     if (per % a.nkb == 0) return 1;
-    cfg.gridDim = dim3(tiles, (a.B + 7) / 8);
-    cfg.blockDim = dim3(kWgTileN, 8);
+    cfg.gridDim = dim3(tiles, (a.B + 31) / 32);
+    cfg.blockDim = dim3(kWgTileN / 4, 32);
     cfg.dynamicSmemBytes = 0;
     cfg.numAttrs = 1;            // the fix-up always follows its GEMM
     cudaLaunchKernelEx(&cfg, wgemm_fixup_kernel<DUAL>, a, (int)NB);
