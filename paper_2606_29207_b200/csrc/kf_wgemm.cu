@@ -369,7 +369,7 @@ static int launch_one(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGem
     cfg.dynamicSmemBytes = smem;
     cfg.stream = s;
     cfg.attrs = attr;
-    cfg.numAttrs = pdl ? 1 : 0;  // only behind a kernel of the same W-side call (see the kernel's griddepcontrol.wait)
+    cfg.numAttrs = pdl ? 1 : 0;  // safe behind any kernel: nothing before the kernel's griddepcontrol.wait touches global memory
     cudaLaunchKernelEx(&cfg, wgemm_kernel<NB, DUAL>, tmW, tmX, a);
     // tiles shared between spans exist unless every span boundary is a tile boundary
     const int tiles = a.N / kWgTileN, total = tiles * a.nkb, per = (total + a.n_ctas - 1) / a.n_ctas;

@@ -125,7 +125,7 @@ int encode(kf_wside *w, CUtensorMap *map, const void *base, size_t rows, size_t 
 
 // out segments [0, e0) -> o0, [e0, e1) -> o1: one GEMM x [B][K] . W(m)^T
 int gemm(kf_wside *w, int layer, int m, const void *x, int batch, __half *o0, int ld0, int e0, __half *o1, int ld1,
-         cudaStream_t s, bool pdl = false) {
+         cudaStream_t s, bool pdl = true) {
     const kf_wside_config *c = &w->cfg;
     const bool dual = m == kMatGU;
     const int K = (int)cols_of(c, m);
@@ -280,7 +280,8 @@ int kf_w_post_attention(kf_wside *w, int32_t layer, const float *o, int32_t batc
     const int qd = c->n_q_heads * 128;
     launch_cast_o(o, w->o16, (size_t)batch * qd, s);
     w->launches += 1;
-    // the three GEMMs follow kernels of this very call: programmatic dependent launches (kf_wgemm.cu)
+    // every GEMM is a programmatic dependent launch (kf_wgemm.cu): before its griddepcontrol.wait it touches no global
+    // memory, so this is safe behind any kernel; the cast kernel has no such wait and is launched normally
     int rc = gemm(w, layer, kMatO, w->o16, batch, w->y, c->hidden, c->hidden, nullptr, 0, s, true);
     if (rc == KF_OK) rc = gemm(w, layer, kMatGU, w->y, batch, w->h, c->ffn, c->ffn, nullptr, 0, s, true);
     if (rc == KF_OK) rc = gemm(w, layer, kMatD, w->h, batch, (__half *)x_next, c->hidden, c->hidden, nullptr, 0, s, true);

@@ -34,8 +34,8 @@ struct WGemmArgs {
 };
 
 // returns the number of kernels launched (1) or a negative KF_E* code
-// pdl: launch programmatically dependent on the preceding kernel of the stream (which must be a kernel of the same
-// W-side call: cast_o_kernel, wgemm_kernel or its fix-up)
+// pdl: launch programmatically dependent on the preceding kernel of the stream (the kernel sets up barriers, TMEM and
+// descriptors, then waits for that kernel to complete before it touches global memory)
 int launch_wgemm(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGemmArgs &a, int nb, bool dual, bool pdl,
                  cudaStream_t s);
 int launch_cast_o(const float *o, __half *o16, size_t n, cudaStream_t s);
