@@ -234,9 +234,10 @@ __global__ void __launch_bounds__(kWgThreads, 1)
             const int len = min(nkb - kb, sp.k1 - pos);
             const int buf = seg & 1;
             const int n = tile * kWgTileN + row;
-            const int sg = (tile * kWgTileN >= a.seg_end[0]) + (tile * kWgTileN >= a.seg_end[1]);
-            __half *out = a.out[sg] + (n - (sg == 0 ? 0 : a.seg_end[sg - 1]));
-            const int ld = a.ld[sg];
+            // output segment of the tile (no dynamic indexing of the parameter struct: that would copy it to local memory)
+            const bool s1 = tile * kWgTileN >= a.seg_end[0], s2 = tile * kWgTileN >= a.seg_end[1];
+            __half *out = (s2 ? a.out[2] : s1 ? a.out[1] : a.out[0]) + (n - (s2 ? a.seg_end[1] : s1 ? a.seg_end[0] : 0));
+            const int ld = s2 ? a.ld[2] : s1 ? a.ld[1] : a.ld[0];
             const uint32_t taddr = tmem + ((uint32_t)(slice * 32) << 16) + buf * kAccCols;
             mbar_wait(smem_u32(&acc_full[buf]), (seg >> 1) & 1);
             tc_fence_after();
@@ -286,12 +287,12 @@ __global__ void __launch_bounds__(kWgThreads, 1)
 
 // Fix-up of the tiles that several spans share: out[b][n] = epilogue(sum over the pieces, in k order = ascending CTA).
 // One thread per (4 consecutive features, batch row): every piece is read once with 128-bit loads, coalesced along the
-// features, all pieces of the thread in flight at once; 8-byte stores.  grid (tiles, ceil(B / 32)), block (32, 32).
+// features, all pieces of the thread in flight at once; 8-byte stores.  grid (tiles, ceil(B / 8)), block (32, 8).
 template <bool DUAL>
-__global__ void __launch_bounds__(1024) wgemm_fixup_kernel(const WGemmArgs a, int nb) {
+__global__ void __launch_bounds__(256) wgemm_fixup_kernel(const WGemmArgs a, int nb) {
     asm volatile("griddepcontrol.wait;" ::: "memory");  // launched while the GEMM is still running (PDL)
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    const int tile = blockIdx.x, row = threadIdx.x * 4, b = blockIdx.y * 32 + threadIdx.y;
+    const int tile = blockIdx.x, row = threadIdx.x * 4, b = blockIdx.y * 8 + threadIdx.y;
     const int nkb = a.nkb;
     const int total = (a.N / kWgTileN) * nkb;
     const int per = (total + a.n_ctas - 1) / a.n_ctas;
@@ -328,8 +329,12 @@ __global__ void __launch_bounds__(1024) wgemm_fixup_kernel(const WGemmArgs a, in
         }
     }
     const int n = tile * kWgTileN + row;
-    const int sg = (tile * kWgTileN >= a.seg_end[0]) + (tile * kWgTileN >= a.seg_end[1]);
-    __half *out = a.out[sg] + (n - (sg == 0 ? 0 : a.seg_end[sg - 1])) + (size_t)b * a.ld[sg];
+    // output segment of the tile (no dynamic indexing of the parameter struct: that would copy it to local memory)
+    const bool s1 = tile * kWgTileN >= a.seg_end[0], s2 = tile * kWgTileN >= a.seg_end[1];
+    __half *base_out = s2 ? a.out[2] : s1 ? a.out[1] : a.out[0];
+    const int ldo = s2 ? a.ld[2] : s1 ? a.ld[1] : a.ld[0];
+    const int n0 = s2 ? a.seg_end[1] : s1 ? a.seg_end[0] : 0;
+    __half *out = base_out + (n - n0) + (size_t)b * ldo;
     const __half2 lo = __floats2half2_rn(DUAL ? silu_mul(g.x, u.x) : g.x, DUAL ? silu_mul(g.y, u.y) : g.y);
     const __half2 hi = __floats2half2_rn(DUAL ? silu_mul(g.z, u.z) : g.z, DUAL ? silu_mul(g.w, u.w) : g.w);
     uint2 w;
@@ -374,8 +379,8 @@ static int launch_one(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGem
     // tiles shared between spans exist unless every span boundary is a tile boundary
     const int tiles = a.N / kWgTileN, total = tiles * a.nkb, per = (total + a.n_ctas - 1) / a.n_ctas;
     if (per % a.nkb == 0) return 1;
-    cfg.gridDim = dim3(tiles, (a.B + 31) / 32);
-    cfg.blockDim = dim3(kWgTileN / 4, 32);
+    cfg.gridDim = dim3(tiles, (a.B + 7) / 8);
+    cfg.blockDim = dim3(kWgTileN / 4, 8);
     cfg.dynamicSmemBytes = 0;
     cfg.numAttrs = 1;            // the fix-up always follows its GEMM
     cudaLaunchKernelEx(&cfg, wgemm_fixup_kernel<DUAL>, a, (int)NB);
