@@ -76,6 +76,15 @@ def test_null_ctx_calls_return_einval():
     assert lib.kf_status(None, None) == -1
     assert lib.kf_destroy(None) == -1
     assert lib.kf_launch_count(None) == 0
+    # the calls added in round 2 follow the same convention: an error code, never a crash
+    assert lib.kf_layer_step(None, 0, None, None, None, None, None, None, None, None) == -1
+    assert lib.kf_redirect_tails(None, None, None) == -1
+    assert lib.kf_route_begins(None, None, None) == -1
+    assert lib.kf_set_active_partitions(None, None, None) == -1
+    assert lib.kf_step_graph_launch(None, None, None, None, None, None, None) == -1
+    assert lib.kf_step_graph_seq(None, 0) == 0
+    assert lib.kf_w_project_q(None, 0, None, 1, None, None) == -1
+    assert lib.kf_wside_launch_count(None) == 0
 
 
 def test_no_cpu_fallback():
