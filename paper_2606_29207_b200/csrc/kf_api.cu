@@ -26,6 +26,16 @@ bool device_can_read(const void *host_ptr) {
     }
     return a.type == cudaMemoryTypeHost && a.devicePointer == host_ptr;
 }
+// device_can_read() with a small per-ctx cache: the pinned buffers of an end-to-end loop are the same few pointers
+// every layer-step, and cudaPointerGetAttributes costs ~1 us each.  (A cached pointer is trusted for the lifetime of
+// the ctx: un-pinning a buffer that is still in use is the caller's error either way.)
+bool host_ptr_ok(kf_ctx *ctx, const void *p) {
+    const size_t slot = ((uintptr_t)p >> 6) % kf_ctx::kPinnedCache;  // direct-mapped
+    if (ctx->pinned[slot] == p) return true;
+    if (!device_can_read(p)) return false;
+    ctx->pinned[slot] = p;
+    return true;
+}
 }  // namespace kf
 
 namespace {
@@ -199,18 +209,6 @@ int ensure_plan(kf_ctx *ctx, cudaStream_t s) {
 int run_attend(kf_ctx *ctx, const AttendParams &ap, cudaStream_t s) {
     if (ctx->impl == KF_IMPL_SIMPLE) return after_launch(ctx, launch_attend_simple(ap, ctx->n_ctas, s));
     return after_launch(ctx, launch_attend_tma(ap, ctx->n_ctas, s));
-}
-
-// device_can_read() with a small per-ctx cache: the pinned buffers of an end-to-end loop are the same few pointers
-// every layer-step, and cudaPointerGetAttributes costs ~1 us each.  (A cached pointer is trusted for the lifetime of
-// the ctx: un-pinning a buffer that is still in use is the caller's error either way.)
-bool host_ptr_ok(kf_ctx *ctx, const void *p) {
-    for (int i = 0; i < kf_ctx::kPinnedCache; ++i)
-        if (ctx->pinned[i] == p) return true;
-    if (!device_can_read(p)) return false;
-    ctx->pinned[ctx->pinned_next] = p;
-    ctx->pinned_next = (ctx->pinned_next + 1) % kf_ctx::kPinnedCache;
-    return true;
 }
 
 bool bad_layer(const kf_ctx *ctx, int layer) { return layer < 0 || layer >= ctx->cfg.n_layers; }

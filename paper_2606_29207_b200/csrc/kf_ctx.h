@@ -11,9 +11,9 @@ struct kf_ctx {
     bool plan_dirty;  // lengths moved (step commit) or routes were edited since the plan kernel last ran
     int64_t launches;
     char cuda_err[256];
-    static constexpr int kPinnedCache = 16;
-    const void *pinned[kPinnedCache];  // host pointers already verified as device-readable (kf_layer_step_host)
-    int pinned_next;
+    static constexpr int kPinnedCache = 1024;
+    const void *pinned[kPinnedCache];  // host pointers already verified as device-readable (kf_layer_step_host,
+                                       // kf_step_graph_launch): direct-mapped by address
 };
 
 // library-internal entry points of the static step graph (kf_graph.cu); not exported through include/kflume.h:
@@ -31,4 +31,5 @@ KF_INTERNAL int kf_layer_step_host_impl(kf_ctx *ctx, int32_t layer, const void *
 namespace kf {
 int cuda_fail(kf_ctx *ctx, cudaError_t e);  // records the error text in the ctx, returns KF_ECUDA
 bool device_can_read(const void *host_ptr);  // pinned host memory the GPU can dereference as it is
+bool host_ptr_ok(kf_ctx *ctx, const void *p);  // the same through the ctx's cache of verified pointers
 }

@@ -338,8 +338,8 @@ int kf_step_graph_launch(kf_graph *g, const void *const *q, const void *const *k
                 // kv_append_stage_kernel(Dev d, int layer, k_new, v_new, q_src, q_dst); the attend node reads stage_q
                 const bool in_changed = q[i] != g->q[i] || k_new[i] != g->k[i] || v_new[i] != g->v[i];
                 const bool out_changed = o[i] != g->o[i] || lse[i] != g->lse[i];
-                if ((in_changed && !(device_can_read(q[i]) && device_can_read(k_new[i]) && device_can_read(v_new[i]))) ||
-                    (out_changed && !(device_can_read(o[i]) && device_can_read(lse[i]))))
+                if ((in_changed && !(host_ptr_ok(ctx, q[i]) && host_ptr_ok(ctx, k_new[i]) && host_ptr_ok(ctx, v_new[i]))) ||
+                    (out_changed && !(host_ptr_ok(ctx, o[i]) && host_ptr_ok(ctx, lse[i]))))
                     return KF_EINVAL;
                 if (in_changed) {
                     int layer = g->layers[i];
