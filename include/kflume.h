@@ -49,7 +49,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 100 /* 0.1.0 */
+#define KF_VERSION 200 /* 0.2.0: round 2 (kf_layer_step, kf_redirect_tails, graph flags, W-node stages; kf_config grew) */
 
 #define KF_OK 0
 #define KF_EINVAL (-1) /* bad argument / shape / alignment / null pointer */

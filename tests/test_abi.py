@@ -29,7 +29,7 @@ def test_every_declared_symbol_is_exported():
 
 def test_version_and_strerror():
     lib = load_library()
-    assert lib.kf_version() == 100
+    assert lib.kf_version() == 200
     assert lib.kf_strerror(0) == b"ok"
     for code in (-1, -2, -3, -4):
         assert lib.kf_strerror(code) not in (b"ok", b"unknown error")
