@@ -49,7 +49,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 200 /* 0.2.0: round 2 (kf_layer_step, kf_redirect_tails, graph flags, W-node stages; kf_config grew) */
+#define KF_VERSION 210 /* 0.2.1: + kf_attend_static (0.2.0: kf_layer_step, kf_redirect_tails, graph flags, W-node stages) */
 
 #define KF_OK 0
 #define KF_EINVAL (-1) /* bad argument / shape / alignment / null pointer */
@@ -210,6 +210,29 @@ int kf_merge_partials(kf_ctx *ctx, const float *o_part, const float *lse_part, f
  *   run-to-run identical and equal to the unfused path).  o_part / lse_part may be NULL (internal scratch). */
 int kf_attend(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, float *o_part, float *lse_part,
               kf_stream stream);
+
+/* (a3+a4, no allocation anywhere) kf_attend_static -- kf_attend for a caller that cannot supply memory for the range
+ *   partials and cannot allocate any.  Who that is: an attention node whose HBM is already handed out to KV pools down to
+ *   the last slot (the paper's A nodes hold nothing but KV) and that is pulled into a running decode loop;
+ *   a thread that must stay out of the CUDA allocator because cudaMalloc / cudaFree synchronise the device and would
+ *   stall the step graphs other streams are replaying; code living under a framework that owns all device memory through
+ *   its own caching allocator.  Same arguments and results as kf_attend(ctx, layer, q, o, lse, NULL, NULL, stream) --
+ *   bit for bit: the same plan, kernel and merge order -- but the range partials (o_j, lse_j of PAPER.md:147, :254) go to
+ *   a fixed array of KF_STATIC_SCRATCH_BYTES that is part of the library image (a file-scope __device__ array) instead
+ *   of to the workspace.  The call never calls cudaMalloc / cudaFree or any routine that allocates device or host memory.
+ *   LIMIT: max_requests * max_ranges_per_request * n_q_heads * (128 + 1) * 4 bytes (+ up to 255 of padding) must fit in
+ *     KF_STATIC_SCRATCH_BYTES, else KF_EINVAL and kf_last_cuda_error() says how many bytes were needed.
+ *   COST: every GPU on which this process uses the library holds those KF_STATIC_SCRATCH_BYTES from the moment the
+ *     library's code is loaded onto it until the process exits, used or not.
+ *   FIRST CALL PER GPU: looks the array's device address up (cudaGetSymbolAddress, with the ctx's device current) and
+ *     keeps it; that look-up is a set-up step which may make the runtime load code onto the GPU, so make the first call
+ *     on each GPU before starting any stream capture.  Later calls only launch.
+ *   SHARING: there is ONE array per GPU for all ctxs and threads.  It keeps whatever the previous call left; the kernel
+ *     never reads a partial it has not written in the same launch, so nothing needs clearing between calls.  Two calls
+ *     whose kernels may run at the same time on one GPU (different streams, different ctxs) write the same bytes and
+ *     corrupt each other's results: order them on one stream or with events, like the calls of one ctx. */
+#define KF_STATIC_SCRATCH_BYTES (16u << 20)
+int kf_attend_static(kf_ctx *ctx, int32_t layer, const void *q, float *o, float *lse, kf_stream stream);
 
 /* (a5) kf_step_commit -- len_r += 1 for every open, active request whose tail position had a route in this step
  *   (the step boundary; a request waiting for a slot stays where it is, see kf_token_boundary). */

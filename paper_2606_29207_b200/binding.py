@@ -16,7 +16,7 @@ KF_IMPL_AUTO, KF_IMPL_SIMPLE, KF_IMPL_TMA = 0, 1, 2
 EXPORTS = [
     "kf_version", "kf_strerror", "kf_last_cuda_error", "kf_pool_bytes", "kf_workspace_bytes", "kf_pool_offset",
     "kf_create", "kf_destroy", "kf_open_request", "kf_close_request", "kf_load_context", "kf_token_boundary",
-    "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_step_commit", "kf_layer_step", "kf_layer_step_host",
+    "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_attend_static", "kf_step_commit", "kf_layer_step", "kf_layer_step_host",
     "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count", "kf_worker_times",
     "kf_step_graph_create", "kf_step_graph_launch", "kf_step_graph_destroy", "kf_probe_read",
     "kf_step_graph_flags", "kf_step_graph_seq", "kf_step_graph_release", "kf_signal_roundtrip",
@@ -93,6 +93,7 @@ def load_library():
     L.kf_partial_attend.argtypes = [vp, i32, vp, ctypes.POINTER(ctypes.c_uint8), vp, vp, vp]
     L.kf_merge_partials.argtypes = [vp, vp, vp, vp, vp, vp]
     L.kf_attend.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
+    L.kf_attend_static.argtypes = [vp, i32, vp, vp, vp, vp]
     L.kf_step_commit.argtypes = [vp, vp]
     L.kf_layer_step.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
     L.kf_layer_step_host.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
@@ -280,6 +281,16 @@ class KFlume:
         self._check(self.lib.kf_attend(self.h, layer, self._f16(q, (self.B, self.Hq, 128)),
                                        self._f32(o, (self.B, self.Hq, 128)), self._f32(lse, (self.B, self.Hq)),
                                        _ptr(o_part), _ptr(lse_part), self._stream(stream)), "kf_attend")
+
+    def attend_static(self, layer: int, q, o, lse, stream=None):
+        """kf_attend with the range partials in the library's own fixed device array: for callers that can neither pass
+        scratch memory nor allocate it (see include/kflume.h).  Results equal attend(layer, q, o, lse) bit for bit."""
+        rc = self.lib.kf_attend_static(self.h, layer, self._f16(q, (self.B, self.Hq, 128)),
+                                       self._f32(o, (self.B, self.Hq, 128)), self._f32(lse, (self.B, self.Hq)),
+                                       self._stream(stream))
+        if rc != KF_OK:   # the size limit is reported as KF_EINVAL with the byte counts in the ctx's error text
+            raise KFlumeError(rc, f"kf_attend_static: {self.lib.kf_strerror(rc).decode()} "
+                                  f"{self.lib.kf_last_cuda_error(self.h).decode()}")
 
     def step_commit(self, stream=None):
         self._check(self.lib.kf_step_commit(self.h, self._stream(stream)), "kf_step_commit")
