@@ -301,7 +301,9 @@ int kf_step_graph_destroy(kf_graph *graph);
  *   they are host buffers) is visible to a host thread that has read the value.  gates != 0: before layer-step i of
  *   launch L (before its kf_kv_append reads k_new[i] / v_new[i] / q[i]) the graph waits until gate word i -- device
  *   memory inside the workspace -- is >= seq(L, i) (cyclic 32-bit comparison).  Both values are re-written into the
- *   graph's mem-op nodes at every launch (host-side update, no re-instantiation).  KF_ESTATE after the first launch;
+ *   graph's mem-op nodes at every launch (host-side update, no re-instantiation).  With gates != 0 the call zeroes the
+ *   gate words and SYNCHRONISES `stream` before it returns, so a release issued right afterwards -- on any stream, while
+ *   `stream` still has other work queued -- cannot be overwritten.  KF_ESTATE after the first launch;
  *   KF_EINVAL if ready_host is not pinned memory the GPU can address.
  * kf_step_graph_seq: the sequence number layer-step i will carry in the NEXT launch (0 on bad arguments).
  * kf_step_graph_release: writes `seq` to gate word i with a stream memory operation on `signal_stream`.  Everything the
@@ -377,7 +379,8 @@ int kf_policy_step(const kf_policy_config *cfg, int32_t n_partitions, const int6
  *   execute one after another (they share the workspace): one stream, or streams ordered by events.
  * Shapes: x, x_next [batch][hidden] fp16; q [batch][H_q][128], k_new / v_new [batch][H_kv][128] fp16 (the layouts
  *   kf_kv_append / kf_attend take); o [batch][H_q][128] fp32 (what kf_attend writes).  1 <= batch <= max_batch <= 128.
- *   hidden and ffn are multiples of 128, head_dim is 128.  All calls are asynchronous on `stream`, never synchronise,
+ *   hidden and ffn are multiples of 128, head_dim is 128.  Every tensor pointer must be 16-byte aligned (KF_EINVAL
+ *   otherwise: rows are read and written with vector accesses).  All calls are asynchronous on `stream`, never synchronise,
  *   never allocate, and can be captured into a CUDA graph. */
 #define KF_W_Q 0
 #define KF_W_KV 1

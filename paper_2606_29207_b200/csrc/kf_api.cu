@@ -135,7 +135,7 @@ Layout make_layout(const kf_config *c) {
     L.stage_o = take(B * Hq * kHeadDim * 4);
     L.stage_lse = take(B * Hq * 4);
     L.tmaps = take(P * 2 * 128);
-    L.gates = take((size_t)kMaxGraphLayerSteps * 4);
+    L.gates = take(((size_t)kMaxGraphLayerSteps + 1) * 4);  // + 1: the word kf_signal_roundtrip plays with
     L.worker_times = take((size_t)kMaxWorkers * 4 * 8);
     L.total = off;
     return L;

@@ -298,7 +298,11 @@ int kf_step_graph_flags(kf_graph *g, uint32_t *ready_host, int32_t gates, kf_str
     g->ready = ready_host;
     g->gates = gates != 0;
     if (g->gates) {  // gate words start below every sequence number
-        const cudaError_t e = cudaMemsetAsync(g->ctx->dev.gates, 0, (size_t)g->n * 4, (cudaStream_t)stream);
+        // ... and they do so BEFORE this call returns: a gate "may be released before the launch that waits on it", on
+        // another stream, so a memset still queued behind earlier work of `stream` could land after such a release, erase
+        // it and leave the graph waiting for ever.  The call is off the hot path; it waits for the memset.
+        cudaError_t e = cudaMemsetAsync(g->ctx->dev.gates, 0, (size_t)g->n * 4, (cudaStream_t)stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
         if (e != cudaSuccess) return cuda_fail(g->ctx, e);
     }
     if (ready_host)
@@ -436,7 +440,7 @@ int kf_signal_roundtrip(kf_ctx *ctx, int32_t iters, kf_stream exec_stream, kf_st
         return KF_EINVAL;
     if (!memops().ok) return KF_ECUDA;
     cudaStream_t es = (cudaStream_t)exec_stream, ss = (cudaStream_t)signal_stream;
-    uint32_t *gate = ctx->dev.gates + (kMaxGraphLayerSteps - 1);  // the last gate word: no step graph that size exists here
+    uint32_t *gate = ctx->dev.gates + kMaxGraphLayerSteps;  // a word of its own, behind the gates a step graph can use
     volatile uint32_t *ready = nullptr;
     cudaError_t e = cudaHostAlloc((void **)&ready, 64, cudaHostAllocMapped);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
@@ -497,6 +501,12 @@ int kf_signal_roundtrip(kf_ctx *ctx, int32_t iters, kf_stream exec_stream, kf_st
             break;
         }
         if (it >= 10) t.push_back(t1 - t0);
+    }
+    if (rc != KF_OK) {
+        // something went wrong with a graph possibly still waiting at the gate: open it for good with a plain copy (a
+        // value every wait of this call accepts) BEFORE synchronising the execution stream, or that would block for ever
+        static const uint32_t open_value = 0x7fffffffu;
+        cudaMemcpyAsync(gate, &open_value, 4, cudaMemcpyHostToDevice, ss);
     }
     cudaStreamSynchronize(ss);
     cudaStreamSynchronize(es);

@@ -86,7 +86,7 @@ __global__ void close_request_kernel(Dev d, int req) {
 }
 
 // (a1) route update: one warp scans the requests 32 at a time; lane 0 allocates in ascending order.
-// returns (in every lane) the number of ranges opened
+// returns (in every lane) the number of ranges opened, i.e. of route entries appended
 __device__ int token_boundary_warp(const Dev &d, int lane) {
     int opened = 0;
     for (int base = 0; base < d.B; base += 32) {
@@ -108,14 +108,18 @@ __device__ int token_boundary_warp(const Dev &d, int lane) {
         }
         const unsigned mr = __ballot_sync(0xffffffffu, redir);
         unsigned m = __ballot_sync(0xffffffffu, need) | mr;
-        opened += __popc(m);
+        // only allocations that SUCCEEDED change a route (and with it the work plan): a request that waits for a slot
+        // (reading 24) asks again at every boundary, and a redirect that finds no slot is dropped quietly -- neither may
+        // force a plan rebuild step after step
+        int done = 0;
         if (lane == 0) {
             while (m) {
                 const int b = __ffs(m) - 1;
                 m &= m - 1;
-                alloc_range(d, base + b, d.len[base + b], (mr >> b) & 1u);
+                done += alloc_range(d, base + b, d.len[base + b], (mr >> b) & 1u) ? 1 : 0;
             }
         }
+        opened += __shfl_sync(0xffffffffu, done, 0);
         __syncwarp();
     }
     if (lane < d.P) d.redirect[lane] = 0;  // the marks are consumed by this boundary (P <= 64: two passes)

@@ -359,11 +359,16 @@ __global__ void cast_o_kernel(const float *__restrict__ o, __half *__restrict__ 
 template <int NB, bool DUAL>
 static int launch_one(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGemmArgs &a, bool pdl, cudaStream_t s) {
     const int smem = wgemm_smem_bytes(NB, DUAL);
-    static bool configured = false;  // per instantiation
-    if (!configured) {
+    // the opt-in to > 48 KB of dynamic shared memory is a per-DEVICE property of the function: once per instantiation
+    // and device (a second GPU in the same process would otherwise launch without it and fail)
+    constexpr int kDevs = 64;
+    static bool configured[kDevs] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return KF_ECUDA;
+    if (dev < 0 || dev >= kDevs || !configured[dev]) {
         if (cudaFuncSetAttribute(wgemm_kernel<NB, DUAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
             return KF_ECUDA;
-        configured = true;
+        if (dev >= 0 && dev < kDevs) configured[dev] = true;
     }
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -375,7 +380,7 @@ static int launch_one(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGem
     cfg.stream = s;
     cfg.attrs = attr;
     cfg.numAttrs = pdl ? 1 : 0;  // safe behind any kernel: nothing before the kernel's griddepcontrol.wait touches global memory
-    cudaLaunchKernelEx(&cfg, wgemm_kernel<NB, DUAL>, tmW, tmX, a);
+    if (cudaLaunchKernelEx(&cfg, wgemm_kernel<NB, DUAL>, tmW, tmX, a) != cudaSuccess) return KF_ECUDA;
     // tiles shared between spans exist unless every span boundary is a tile boundary
     const int tiles = a.N / kWgTileN, total = tiles * a.nkb, per = (total + a.n_ctas - 1) / a.n_ctas;
     if (per % a.nkb == 0) return 1;
@@ -383,7 +388,7 @@ static int launch_one(const CUtensorMap &tmW, const CUtensorMap &tmX, const WGem
     cfg.blockDim = dim3(kWgTileN / 4, 8);
     cfg.dynamicSmemBytes = 0;
     cfg.numAttrs = 1;            // the fix-up always follows its GEMM
-    cudaLaunchKernelEx(&cfg, wgemm_fixup_kernel<DUAL>, a, (int)NB);
+    if (cudaLaunchKernelEx(&cfg, wgemm_fixup_kernel<DUAL>, a, (int)NB) != cudaSuccess) return KF_ECUDA;
     return 2;
 }
 

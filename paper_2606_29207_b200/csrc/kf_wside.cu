@@ -17,8 +17,6 @@ struct kf_wside {
     // workspace slices
     __half *o16, *y, *h;      // [B][Hq*d], [B][hidden], [B][ffn]
     float *partial;
-    int *counters;
-    CUtensorMap tm_w[1];      // placeholder to keep the struct POD-like; real maps live in `maps`
     CUtensorMap *maps;        // [L][5] weight maps (host copies, passed to kernels by value)
     cudaEvent_t ev[64];       // cross-stream dependencies of kf_pipeline_step
     int n_ev;
@@ -89,14 +87,6 @@ size_t partial_floats(const kf_wside_config *) {
     // every CTA of the persistent grid owns two slots of one (dual) accumulator tile [2][NB = 128][128] fp32
     return (size_t)kWgMaxCtas * 2 * 2 * kWgMaxBatch * kWgTileN;
 }
-size_t max_tiles(const kf_wside_config *c) {
-    size_t mx = 0;
-    for (int m = 0; m < 5; ++m) {
-        const size_t t = (m == kMatGU ? (size_t)c->ffn : rows_of(c, m)) / kWgTileN;
-        if (t > mx) mx = t;
-    }
-    return mx;
-}
 
 int fail(kf_wside *w, cudaError_t e) {
     snprintf(w->cuda_err, sizeof(w->cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
@@ -153,7 +143,10 @@ int gemm(kf_wside *w, int layer, int m, const void *x, int batch, __half *o0, in
     a.partial = w->partial;
     a.up_row_offset = dual ? c->ffn : 0;
     rc = launch_wgemm(w->maps[layer * 5 + m], tmX, a, nb, dual, pdl, s);
-    if (rc < 0) return rc;
+    if (rc < 0) {
+        if (rc == KF_ECUDA) fail(w, cudaGetLastError());  // a launch or its set-up was refused: keep the runtime's text
+        return rc;
+    }
     w->launches += rc;
     const cudaError_t e = cudaPeekAtLastError();
     if (e != cudaSuccess) {
@@ -189,8 +182,7 @@ size_t kf_wside_weight_offset(const kf_wside_config *cfg, int32_t layer, int32_t
 size_t kf_wside_workspace_bytes(const kf_wside_config *c) {
     if (!valid(c)) return 0;
     const size_t B = c->max_batch;
-    return up(B * c->n_q_heads * 128 * 2) + up(B * c->hidden * 2) + up(B * (size_t)c->ffn * 2) + up(partial_floats(c) * 4) +
-           up(max_tiles(c) * 4);
+    return up(B * c->n_q_heads * 128 * 2) + up(B * c->hidden * 2) + up(B * (size_t)c->ffn * 2) + up(partial_floats(c) * 4);
 }
 
 int kf_wside_create(kf_wside **out, const kf_wside_config *cfg, void *weights, void *workspace, size_t workspace_bytes) {
@@ -214,10 +206,7 @@ int kf_wside_create(kf_wside **out, const kf_wside_config *cfg, void *weights, v
     w->h = (__half *)ws;
     ws += up(B * (size_t)cfg->ffn * 2);
     w->partial = (float *)ws;
-    ws += up(partial_floats(cfg) * 4);
-    w->counters = (int *)ws;
-    cudaError_t e = cudaMemset(w->counters, 0, max_tiles(cfg) * 4);
-    if (e != cudaSuccess) return fail(w, e);
+    cudaError_t e = cudaSuccess;
     w->maps = new (std::nothrow) CUtensorMap[(size_t)cfg->n_layers * 5];
     if (!w->maps) return KF_EINVAL;
     for (int l = 0; l < cfg->n_layers; ++l)
@@ -262,19 +251,20 @@ const char *kf_wside_last_error(const kf_wside *w) { return w ? w->cuda_err : ""
 int64_t kf_wside_launch_count(const kf_wside *w) { return w ? w->launches : 0; }
 
 int kf_w_project_q(kf_wside *w, int32_t layer, const void *x, int32_t batch, void *q, kf_stream stream) {
-    if (bad_call(w, layer, batch) || !x || !q || ((uintptr_t)x & 15)) return KF_EINVAL;
+    if (bad_call(w, layer, batch) || !x || !q || ((uintptr_t)x & 15) || ((uintptr_t)q & 15)) return KF_EINVAL;
     const int qd = w->cfg.n_q_heads * 128;
     return gemm(w, layer, kMatQ, x, batch, (__half *)q, qd, qd, nullptr, 0, (cudaStream_t)stream);
 }
 
 int kf_w_project_kv(kf_wside *w, int32_t layer, const void *x, int32_t batch, void *k_new, void *v_new, kf_stream stream) {
-    if (bad_call(w, layer, batch) || !x || !k_new || !v_new || ((uintptr_t)x & 15)) return KF_EINVAL;
+    if (bad_call(w, layer, batch) || !x || !k_new || !v_new || (((uintptr_t)x | (uintptr_t)k_new | (uintptr_t)v_new) & 15))
+        return KF_EINVAL;
     const int kvd = w->cfg.n_kv_heads * 128;
     return gemm(w, layer, kMatKV, x, batch, (__half *)k_new, kvd, kvd, (__half *)v_new, kvd, (cudaStream_t)stream);
 }
 
 int kf_w_post_attention(kf_wside *w, int32_t layer, const float *o, int32_t batch, void *x_next, kf_stream stream) {
-    if (bad_call(w, layer, batch) || !o || !x_next || ((uintptr_t)o & 15)) return KF_EINVAL;
+    if (bad_call(w, layer, batch) || !o || !x_next || (((uintptr_t)o | (uintptr_t)x_next) & 15)) return KF_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
     const kf_wside_config *c = &w->cfg;
     const int qd = c->n_q_heads * 128;

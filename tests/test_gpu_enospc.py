@@ -68,15 +68,23 @@ def _step(kf, model, step, o, lse, expect_enospc):
         pos = np.arange(n)
         o_ref, lse_ref = oracle.attend(q[r], gen.gen_k(0, r, pos, HKV), gen.gen_v(0, r, pos, HKV))
         check_close(oh[r], lh[r], o_ref, lse_ref, f"step{step} r{r}")
+    # a waiting request is still answered, over the tokens it has committed (kflume.h, kf_token_boundary) -- step after
+    # step, whether the work plan was rebuilt at this boundary or kept (a failed allocation changes no route)
+    for r in range(B):
+        if model.len[r] > 0 and r not in served:
+            pos = np.arange(model.len[r])
+            o_ref, lse_ref = oracle.attend(q[r], gen.gen_k(0, r, pos, HKV), gen.gen_v(0, r, pos, HKV))
+            check_close(oh[r], lh[r], o_ref, lse_ref, f"step{step} waiting r{r}")
     model.step_commit()
     _same(kf, model)
     return served
 
 
+@pytest.mark.parametrize("refresh", [0, 1])     # 0: the plan is kept while nothing changes; 1: rebuilt at every boundary
 @pytest.mark.parametrize("impl", [KF_IMPL_SIMPLE, KF_IMPL_TMA])
-def test_request_waits_for_a_slot_and_resumes(impl):
+def test_request_waits_for_a_slot_and_resumes(impl, refresh):
     # one node, 3 slots, R = 4: r0 (4 tokens) and r1 (8 tokens) fill it; both tail ranges are full
-    cfg = make_config(HQ, HKV, 4, 1, 3, 4, 3, attend_impl=impl)
+    cfg = make_config(HQ, HKV, 4, 1, 3, 4, 3, attend_impl=impl, plan_refresh_steps=refresh)
     kf = KFlume(cfg)
     model = RoutingModel(1, 4, 3, 4, 3)
     _open(kf, model, 0, 4)

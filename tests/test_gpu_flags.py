@@ -188,3 +188,43 @@ def test_readiness_flags_without_gates_and_roundtrip_latency():
         assert 0.5 < mn <= med < 2000.0, (med, mn)                  # microseconds
         assert kf.status() == KF_OK
     ses.close()
+
+
+def test_release_right_after_flags_survives_while_the_capture_stream_is_busy():
+    # kflume.h: "a gate may be released before the launch that waits on it".  kf_step_graph_flags zeroes the gate words
+    # on `stream`; if that memset could still be queued behind earlier work when a release on the signalling stream
+    # lands, it would erase the release and the launch below would wait for ever.  Keep `side` busy (a long device-side
+    # spin), call flags(), release at once, and only then let the stream drain.
+    wl = Workload("flags_early", 32, 8, 64, 2, [200, 33, 65])
+    ses = Session(wl, steps=2)
+    ses.prepare()
+    kf = ses.kf
+    side, signal = torch.cuda.Stream(), torch.cuda.Stream()
+    ready = torch.zeros(1, dtype=torch.int32).pin_memory()
+    with torch.cuda.stream(side):
+        q, (kn, vn) = ses.q_for(0, 0), ses.kv_new_for(0, 0)
+        g = kf.step_graph_create([0], [q], [kn], [vn], [ses.o], [ses.lse])
+        side.synchronize()
+        ses.o.fill_(float("nan"))
+        torch.cuda._sleep(400_000_000)                              # ~0.2 s of queued work in front of flags()
+        g.flags(ready, gates=True)                                  # no synchronize() here, on purpose
+        seq = g.seq(0)
+        g.release(0, seq, signal)                                   # early release, before the launch exists
+        signal.synchronize()
+        g.launch()
+        t0 = time.perf_counter()
+        while not side.query() and time.perf_counter() - t0 < 20.0:
+            time.sleep(0.005)
+        done = side.query()
+        if not done:                                                # never leave the GPU waiting at a gate
+            g.release(0, seq, signal)
+            side.synchronize()
+        assert done, "the early release was erased: the graph was still waiting at its gate after 20 s"
+        assert int(ready[0]) == seq
+        assert kf.status() == KF_OK
+        o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+        for r, S0 in enumerate(wl.contexts):
+            o_ref, lse_ref = oracle_request(wl, 0, r, 0, S0)
+            check_close(o[r], lse[r], o_ref, lse_ref, f"early release r{r}")
+        g.destroy()
+    ses.close()
