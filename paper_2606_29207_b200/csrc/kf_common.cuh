@@ -127,8 +127,7 @@ struct Dev {
     unsigned char *pool[kMaxPartitions];
     size_t v_off;        // byte offset of the V half of a pool
     const void *tmaps;   // [P][2] CUtensorMap (K, V) in device memory, 128-byte stride
-    uint32_t *gates;     // [kMaxGraphLayerSteps] gate words of the signalled step graph (kf_step_graph_flags), + 1 word
-                         // of its own for the kf_signal_roundtrip diagnostic
+    uint32_t *gates;     // [kMaxGraphLayerSteps] gate words of the signalled step graph (kf_step_graph_flags)
     long long *worker_times;  // [kMaxWorkers][4]: {smid, t_start, t_first_tile, t_end} (globaltimer ns), diagnostics
 };
 

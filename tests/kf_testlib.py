@@ -40,8 +40,16 @@ def oracle_request(wl, layer, req, step, n_tokens, heads=None, scale=None, range
     q = gen.gen_q(layer, req, step, wl.n_q_heads, wl.seed)
     if K is None:
         K, V = host_kv(wl, layer, req, n_tokens)
+    if heads is None:
+        # all heads: ONE call on the full [H_q] / [H_kv] tensors, so the oracle's own GQA mapping (query head h reads KV
+        # head h / G) is the one under test, not a restatement of it here
+        o, lse = oracle.attend(q, K, V, scale)
+        if not ranges:
+            return o, lse
+        op, lp = oracle.attend_ranges(q, K, V, wl.range_tokens, scale)
+        return o, lse, op, lp
     G = wl.group
-    heads = list(range(wl.n_q_heads)) if heads is None else list(heads)
+    heads = list(heads)
     o = np.zeros((len(heads), 128))
     lse = np.zeros(len(heads))
     op = lp = None

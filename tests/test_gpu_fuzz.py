@@ -66,3 +66,41 @@ def test_random_decode_loops(block):
     rnd = random.Random(1000 + block)
     for i in range(10):
         _one_case(rnd, 10 * block + i)
+
+
+@pytest.mark.parametrize("G", [5, 7])
+@pytest.mark.parametrize("impl", [KF_IMPL_SIMPLE, KF_IMPL_TMA])
+def test_odd_group_sizes(impl, G):
+    # kf_config admits every G = H_q / H_kv in 1..8; the random draws above only reach {1, 2, 3, 4, 6, 8}.  G = 5 and 7
+    # leave the last rows of the kernel's 8-row query tile empty and make the merge tasks' head chunks ragged.
+    # Ragged contexts over several ranges and partitions, three decode steps, fused / unfused / one launch; routes vs the
+    # integer model, every request and every range partial vs the oracle (which maps h -> h / G itself).
+    Hkv = 2
+    wl = Workload(f"odd_g{G}", Hkv * G, Hkv, 32, 3, [1, 17, 32, 33, 100, 257], n_steps=3)
+    ses = Session(wl, impl=impl, steps=3)
+    ses.prepare()
+    kf = ses.kf
+    model = RoutingModel(3, 32, wl.batch, kf.Jmax, kf.cfg.slots_per_partition)
+    for r, n in enumerate(ses.len0):
+        model.open_request(r, n)
+    for step in range(3):
+        kf.token_boundary()
+        model.token_boundary()
+        q = ses.q_for(0, step)
+        k_new, v_new = ses.kv_new_for(0, step)
+        ses.layer_step(0, q, k_new, v_new, fused=step != 1, want_partials=True,
+                       one_launch=step == 2 and impl == KF_IMPL_TMA)
+        kf.step_commit()
+        model.step_commit()
+        assert kf.status() == KF_OK
+        o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+        op, lp = ses.o_part.cpu().numpy(), ses.lse_part.cpu().numpy()
+        for r, S0 in enumerate(wl.contexts):
+            o_ref, lse_ref, op_ref, lp_ref = oracle_request(wl, 0, r, step, S0 + step, ranges=True)
+            check_close(o[r], lse[r], o_ref, lse_ref, f"G{G} step{step} r{r}")
+            J = op_ref.shape[0]
+            check_close(op[r, :J], lp[r, :J], op_ref, lp_ref, f"G{G} step{step} r{r} partials")
+    snap, ms = kf.route_snapshot(), model.snapshot()
+    for key in ("len", "n_ranges", "part", "slot", "free_head", "rr_cursor"):
+        assert snap[key] == ms[key], key
+    ses.close()
