@@ -202,15 +202,16 @@ def oracle_sample(wl, lens_before, budget_s, have_gpu):
     return chosen, data, desc
 
 
-def oracle_run(wl, chosen, data, step):
-    """One timed pass of the oracle over the sample.  Returns (seconds, {request: (o*, lse*)})."""
+def oracle_run(wl, chosen, data, step, n_threads=0):
+    """One timed pass of the oracle over the sample (n_threads = 0: the oracle's default, all host cores).
+    Returns (seconds, {request: (o*, lse*)})."""
     import oracle
     from kf_inputs import gen
     qs = [gen.gen_q(0, r, step, wl.n_q_heads, wl.seed) for r, _ in chosen]
     out = {}
     t = time.perf_counter()
     for (r, n), (K, V), q in zip(chosen, data, qs):
-        out[r] = oracle.attend(q, K, V)
+        out[r] = oracle.attend(q, K, V, n_threads=n_threads)
     return time.perf_counter() - t, out
 
 
@@ -252,13 +253,20 @@ def run_reference(args):
 
 
 def run_route_install(args):
-    """--route-install: latency of a scale event (kf_set_active_partitions, the paper's route install: 7.2 us on its
+    """--route-install: one JSON line with signalling_record()."""
+    import torch
+    print(json.dumps(signalling_record(torch.device("cuda:0"), args.workload)))
+    return 0
+
+
+def signalling_record(dev, workload="cfg3"):
+    """Latency of a scale event (kf_set_active_partitions, the paper's route install: 7.2 us on its
     CPU) and of kf_token_boundary with a kept / a rebuilt work plan.  Medians; one JSON line."""
     import statistics
     import torch
     from kf_inputs import workloads
     from paper_2606_29207_b200.workload import Session
-    wl = workloads.by_name(args.workload)
+    wl = workloads.by_name(workload)
     P = wl.n_partitions
 
     def event_us(fn):
@@ -307,27 +315,28 @@ def run_route_install(args):
     for _ in range(60):
         e.append(event_us(lambda: None)[0])
     out["empty_event_pair_us"] = statistics.median(e)
-    print(json.dumps(out))
-    return 0
+    out["paper_route_install_us"] = 7.2          # PAPER.md:308 (its CPU routing loop; context, another machine)
+    return out
 
 
 
-def run_pipeline(args):
-    """--pipeline: W-side stages + M = 2 inter-layer kernel pipelining on ONE B200 (PAPER.md:252-280,
+def pipeline_cases(cases, sms_list, n_layers, want_parity=True):
+    """W-side stages + M = 2 inter-layer kernel pipelining on ONE B200 (PAPER.md:252-280,
     Fig. 11): for each workload (two microbatches of B_mu requests at context S, Llama-3.1-8B shape, synthetic weights)
     measure T_p (Q + K/V projection), T_f (W_O + SwiGLU FFN), T_A (append + attend, as a function of the attend
     kernel's SM budget), the serial and the pipelined step, and compare the measured ratio with the paper's model
-    G_pipe = (T_p + T_A + T_f) / max(T_p + T_f, T_A).  One JSON line."""
+    G_pipe = (T_p + T_A + T_f) / max(T_p + T_f, T_A).  sms_list: attend SM budgets to try; None = the one
+    `workload.pipeline_attend_sms` picks from the byte counts.  After the timed replays of a case ONE fresh pipelined step
+    (layer 0) is compared with the oracle chain.  Returns the dict `--pipeline` prints."""
     import statistics
     import torch
     from kf_inputs import gen_device, workloads
     from kf_inputs.workloads import Workload
-    from paper_2606_29207_b200.workload import Session, make_wside
+    from paper_2606_29207_b200.workload import Session, make_wside, pipeline_attend_sms
 
     dev = torch.device("cuda:0")
     torch.cuda.set_device(dev)
     hidden, Hq, Hkv, ffn = 4096, 32, 8, 14336
-    n_layers = args.pipe_layers
     Lw = 2                                           # physical weight layers (436 MB each >> L2), aliased
     w = make_wside(hidden, Hq, Hkv, ffn, n_layers=Lw, max_batch=128)
     weight_bytes_layer = sum(2 * a * b for a, b in (w.shape(i) for i in range(6)))
@@ -355,13 +364,15 @@ def run_pipeline(args):
         del g
         return statistics.median(x.elapsed_time(y) for x, y in ts) * 1e3 / inner
 
-    cases = [tuple(int(v) for v in c.split("x")) for c in args.pipe_cases.split(",")]
-    sms_list = [int(v) for v in args.pipe_sms.split(",")]
     rows = []
+    sms_arg = sms_list
     for (Bm, S) in cases:
         R, P = 8192, 4
         rec = {"B_mu": Bm, "seq": S, "microbatches": 2, "layers_per_step": n_layers}
         best = None
+        # without a sweep: all SMs (the serial baseline and T_A alone on the GPU) and the budget the rule picks
+        sms_list = sms_arg if sms_arg else [148, pipeline_attend_sms(Bm * S * 2 * Hkv * 128 * 2, weight_bytes_layer)]
+        rec["attend_sms_rule"] = None if sms_arg else sms_list[1]
         for sms in sms_list:
             wls = [Workload(f"mb{m}_b{Bm}_s{S}", Hq, Hkv, R, P, [S] * Bm, seed=260629207 + m) for m in range(2)]
             total_steps = 40
@@ -405,6 +416,10 @@ def run_pipeline(args):
                         run()
                     ts = []
                     for i in range(8):
+                        # x is overwritten in place by every layer and there is no norm between the layers: start every
+                        # replay from the seeded hidden state, or fp16 would saturate after a few replays
+                        for b_, x_ in zip(bufs, x0):
+                            b_["x"].copy_(x_)
                         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                         a.record(ws)
                         g.replay()
@@ -414,7 +429,9 @@ def run_pipeline(args):
                     torch.cuda.synchronize(dev)
                     del g
                     w.set_sms(0)
+                    finite.append(all(bool(torch.isfinite(b_["x"]).all()) for b_ in bufs))
                     return statistics.median(x.elapsed_time(y) for x, y in ts) * 1e3
+                finite = []
                 ser = step_us(0)
                 pip = step_us(1)
                 for s_ in sess:
@@ -425,7 +442,8 @@ def run_pipeline(args):
             gc.collect()
             torch.cuda.empty_cache()
             per = {"attend_sms": sms, "T_A_us": t_a, "serial_us_per_layer_mb": ser / (2 * n_layers),
-                   "pipelined_us_per_layer_mb": pip / (2 * n_layers), "measured_ratio": ser / pip}
+                   "pipelined_us_per_layer_mb": pip / (2 * n_layers), "measured_ratio": ser / pip,
+                   "x_finite_after_step": all(finite)}
             rec.setdefault("by_sms", []).append(per)
             if best is None or per["pipelined_us_per_layer_mb"] < best["pipelined_us_per_layer_mb"]:
                 best = per
@@ -443,11 +461,134 @@ def run_pipeline(args):
         rec["one_gpu_hbm_floor_us"] = (weight_bytes_layer + kv_bytes) / (peak * 1e9) * 1e6
         rec["W_side_GBs"] = weight_bytes_layer / ((tp + tf) * 1e-6) / 1e9
         rec["pipelined_GBs"] = (weight_bytes_layer + kv_bytes) / (best["pipelined_us_per_layer_mb"] * 1e-6) / 1e9
+        if want_parity:
+            rec["parity"] = pipeline_parity(w, Bm, S, R, P, best["attend_sms"], ws, as_)
         rows.append(rec)
     w.close()
-    print(json.dumps({"mode": "pipeline", "model": "Llama-3.1-8B shape (hidden 4096, 32/8 heads, ffn 14336), synthetic weights",
-                      "weight_bytes_per_layer": weight_bytes_layer, "peak_gbs": peak, "peak_source": peak_src,
-                      "cases": rows}))
+    return {"mode": "pipeline", "model": "Llama-3.1-8B shape (hidden 4096, 32/8 heads, ffn 14336), synthetic weights",
+            "weight_bytes_per_layer": weight_bytes_layer, "peak_gbs": peak, "peak_source": peak_src, "cases": rows}
+
+
+_W_HOST = {}
+
+
+def pipeline_parity(w, Bm, S, R, P, sms, ws, as_):
+    """PARITY of the timed pipeline configuration, after its timing: fresh sessions (so the KV context is the generator's,
+    not what the timed replays appended), the seeded hidden state, ONE pipelined kf_pipeline_step through layer 0 with the
+    SM split that was timed -- and x' of two requests per microbatch against the oracle chain project -> append ->
+    attend -> W_O -> SwiGLU FFN on the same inputs (tolerance: DESIGN.md section 6, the x' gate)."""
+    import numpy as np
+    import torch
+    import oracle
+    from oracle import wside as ow
+    from kf_inputs import gen_device
+    from kf_inputs.workloads import Workload
+    from paper_2606_29207_b200 import KF_W_DOWN, KF_W_GATE, KF_W_KV, KF_W_O, KF_W_Q, KF_W_UP
+    from paper_2606_29207_b200.workload import Session
+    hidden, Hq, Hkv = 4096, 32, 8
+    if "W" not in _W_HOST:
+        _W_HOST["W"] = {k: w.weight(0, k).cpu().numpy() for k in (KF_W_Q, KF_W_KV, KF_W_O, KF_W_GATE, KF_W_UP, KF_W_DOWN)}
+    W = _W_HOST["W"]
+    wls = [Workload(f"mb{m}_b{Bm}_s{S}", Hq, Hkv, R, P, [S] * Bm, seed=260629207 + m) for m in range(2)]
+    sess = [Session(wl, n_layers_phys=1, steps=2, attend_sms=0 if sms >= 148 else sms) for wl in wls]
+    for s_ in sess:
+        s_.prepare()
+    dev = sess[0].device
+    with torch.cuda.stream(ws):
+        xs = [gen_device.fill_x(0, Bm, 0, hidden, seed=wl.seed) for wl in wls]
+        x0 = [x.cpu().numpy() for x in xs]
+        bufs = [{"q": torch.zeros((Bm, Hq, 128), dtype=torch.float16, device=dev),
+                 "k": torch.zeros((Bm, Hkv, 128), dtype=torch.float16, device=dev),
+                 "v": torch.zeros((Bm, Hkv, 128), dtype=torch.float16, device=dev),
+                 "o": torch.zeros((Bm, Hq, 128), dtype=torch.float32, device=dev),
+                 "lse": torch.zeros((Bm, Hq), dtype=torch.float32, device=dev)} for _ in wls]
+        w.set_sms(148 - sms if sms < 148 else 0)
+        ws.synchronize()
+        w.pipeline_step([s_.kf for s_ in sess], [0], xs, [b["q"] for b in bufs], [b["k"] for b in bufs],
+                        [b["v"] for b in bufs], [b["o"] for b in bufs], [b["lse"] for b in bufs], 1, ws, as_)
+        ws.synchronize()
+        as_.synchronize()
+        w.set_sms(0)
+        got = [x.cpu().numpy().astype(np.float64) for x in xs]
+        ok_state = all(s_.kf.status() == 0 for s_ in sess)
+    rows = [0, Bm - 1]
+    xin = np.concatenate([x0[m][rows] for m in range(2)])                       # [4][hidden]
+    pr = ow.project(xin, W[KF_W_Q], W[KF_W_KV])
+    o = np.zeros((len(xin), Hq * 128))
+    for i in range(len(xin)):
+        m, r = divmod(i, len(rows))
+        K, V = _host_kv(wls[m], rows[r], S - 1, True)
+        K = np.concatenate([K, pr["k16"][i].reshape(Hkv, 1, 128)], 1)
+        V = np.concatenate([V, pr["v16"][i].reshape(Hkv, 1, 128)], 1)
+        o[i] = oracle.attend(pr["q16"][i].reshape(Hq, 128), np.ascontiguousarray(K), np.ascontiguousarray(V))[0].reshape(-1)
+    ref = ow.post_attention(o, W[KF_W_O], W[KF_W_GATE], W[KF_W_UP], W[KF_W_DOWN])["x"]
+    g = np.concatenate([got[m][rows] for m in range(2)])
+    rms = float(np.sqrt(np.mean(ref * ref)))
+    ratio = float((np.abs(g - ref) / (np.abs(ref) + rms + 1e-12)).max())
+    finite = bool(all(np.isfinite(x).all() for x in got))
+    for s_ in sess:
+        s_.close()
+    # DESIGN.md section 6: the chain gate.  Unlike x' from an exact o (5 u), this chain carries the attend kernel's own
+    # P-rounding noise (1..3 u of rms(o)) through W_O and the SwiGLU doubling: 4.4..6 u measured, gate 20 u
+    gate = 1e-2
+    return {"ok": bool(finite and ok_state and ratio <= gate), "max_err_over_ref_plus_rms": ratio, "gate": gate,
+            "rows": len(xin), "x_finite": finite, "attend_sms": sms, "gemm_ctas": 148 - sms if sms < 148 else 148,
+            "what": "one pipelined kf_pipeline_step (layer 0) from the seeded x, rows 0 and B-1 of both microbatches, vs "
+                    "oracle project -> append -> attend -> W_O -> SwiGLU FFN"}
+
+
+def compact_pipeline(full):
+    """The `pipeline` record of the default line: one entry per case, numbers only."""
+    out = []
+    for c in full["cases"]:
+        b = c["best"]
+        out.append(_round({"B_mu": c["B_mu"], "seq": c["seq"], "T_p_us": c["T_p_us"], "T_f_us": c["T_f_us"], "T_A_us": c["T_A_us"],
+                           "serial_us": c["serial_us_per_layer_mb"], "pipelined_us": b["pipelined_us_per_layer_mb"],
+                           "attend_sms": b["attend_sms"], "attend_sms_rule": c.get("attend_sms_rule"),
+                           "measured_ratio": c["measured_ratio_best"],
+                           "model_G_pipe": c["model_G_pipe"], "one_gpu_hbm_floor_us": c["one_gpu_hbm_floor_us"],
+                           "pipelined_over_floor": b["pipelined_us_per_layer_mb"] / c["one_gpu_hbm_floor_us"],
+                           "x_finite": b["x_finite_after_step"],
+                           "parity": {k: c["parity"][k] for k in ("ok", "max_err_over_ref_plus_rms", "gate", "rows")}
+                           if c.get("parity") else None}))
+    return {"layers_per_step": full["cases"][0]["layers_per_step"] if full["cases"] else None, "microbatches": 2,
+            "unit": "us per (layer, microbatch)", "cases": out}
+
+
+def run_pipeline(args):
+    """--pipeline: the full table (every case x every SM budget of --pipe-sms, or the rule's budget with --pipe-sms rule)."""
+    cases = [tuple(int(v) for v in c.split("x")) for c in args.pipe_cases.split(",")]
+    sms_list = None if args.pipe_sms == "rule" else [int(v) for v in args.pipe_sms.split(",")]
+    print(json.dumps(pipeline_cases(cases, sms_list, args.pipe_layers)))
+    return 0
+
+
+
+
+def run_wside_once(args):
+    """--wside-once: every W-side stage once per batch size (after one untimed round), eagerly, on the 8B layer shape.
+    Exists to be run under `ncu -k regex:wgemm`: the captures of wgemm_kernel / wgemm_fixup_kernel under profiles/."""
+    import torch
+    from kf_inputs import gen_device
+    from paper_2606_29207_b200.workload import make_wside
+    hidden, Hq, Hkv, ffn = 4096, 32, 8, 14336
+    w = make_wside(hidden, Hq, Hkv, ffn, n_layers=1, max_batch=128)
+    torch.cuda.synchronize()
+    n0 = w.launch_count()
+    for batch in (16, 128):
+        x = gen_device.fill_x(0, batch, 0, hidden)
+        q = torch.empty((batch, Hq, 128), dtype=torch.float16, device="cuda")
+        k = torch.empty((batch, Hkv, 128), dtype=torch.float16, device="cuda")
+        v = torch.empty_like(k)
+        o = torch.randn((batch, Hq, 128), dtype=torch.float32, device="cuda")
+        xn = torch.empty((batch, hidden), dtype=torch.float16, device="cuda")
+        for _ in range(2):
+            w.project_q(0, x, q)
+            w.project_kv(0, x, k, v)
+            w.post_attention(0, o, xn)
+            torch.cuda.synchronize()
+    print(json.dumps({"mode": "wside-once", "launches": w.launch_count() - n0}))
+    w.close()
     return 0
 
 
@@ -569,7 +710,8 @@ def measure_static(ses, wl, dev, reps=60, warm=5):
             "repetitions": reps}
 
 
-def measure(args, wl_name, steps, warmup, e2e_steps, dev, dist, rank, world, local, want_cpu, want_probe=True):
+def measure(args, wl_name, steps, warmup, e2e_steps, dev, dist, rank, world, local, want_cpu, want_probe=True,
+            cpu_budget_s=15.0):
     """Everything bench.py reports for ONE workload; returns the record (rank 0) or None."""
     import torch
     from kf_inputs import workloads
@@ -801,7 +943,7 @@ def measure(args, wl_name, steps, warmup, e2e_steps, dev, dist, rank, world, loc
         import numpy as np
         import oracle
         lens_now = [n + step for n in lens]
-        chosen, data, desc = oracle_sample(wl, lens_now, 15.0, True)
+        chosen, data, desc = oracle_sample(wl, lens_now, cpu_budget_s, True)
         timed_step(inputs(step))                    # physical layer of the last layer-step: layer_ids[-1]
         torch.cuda.synchronize(dev)
         assert kf.status() == 0
@@ -809,7 +951,12 @@ def measure(args, wl_name, steps, warmup, e2e_steps, dev, dist, rank, world, loc
         dt, ref = oracle_run(wl, chosen, data, step)
         nbytes = sum(n for _, n in chosen) * wl.kv_bytes_per_token()
         cpu = {"value": nbytes / dt / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-               "sample": f"{desc}, decode step {step}, {dt:.2f} s", "seconds": dt}
+               "sample": f"{desc}, decode step {step}, {dt:.2f} s", "seconds": dt,
+               "sample_short": f"{len(chosen)} of {B} requests, {sum(n for _, n in chosen)} context tokens"
+                               + ("" if all(n == lens_now[r] + 1 for r, n in chosen) else " (prefix)")}
+        if wl.name == "cfg1":       # SURVEY 8(d) "CPU baseline": the smallest config also on ONE thread
+            dt1, _ = oracle_run(wl, chosen, data, step, n_threads=1)
+            cpu["one_thread"] = {"value": nbytes / dt1 / 1e9, "seconds": dt1, "cores": 1}
         if layer_ids[-1] == 0 and all(n == lens_now[r] + 1 for r, n in chosen):
             eo = max(float(np.abs(o_gpu[r] - ref[r][0]).max()) for r, _ in chosen)
             el = max(float((np.abs(lse_gpu[r] - ref[r][1]) / np.maximum(1.0, np.abs(ref[r][1]))).max())
@@ -842,16 +989,13 @@ def measure(args, wl_name, steps, warmup, e2e_steps, dev, dist, rank, world, loc
         "config": {"workload": wl.name, "note": wl.note, "batch": B, "n_q_heads": Hq, "n_kv_heads": Hkv,
                    "range_tokens": wl.range_tokens, "n_partitions": wl.n_partitions, "layers_logical": n_layers,
                    "layers_physical": L_phys, "context_tokens_step0": sum(lens) + B,
-                   "l2": "inputs larger than L2 (KV read per layer-step >> 126 MB); no flush needed" if not flush and
+                   "l2": "inputs larger than L2 (KV per layer-step >> 126 MB), no flush" if not flush and
                          kv_bytes / (steps * n_layers) > 4 * 126e6 else
-                         "KV fits L2: 512 MiB written between timed steps, outside the per-step CUDA-event windows "
-                         "(value, ms_per_step, roofline are L2-cold; warm_ms_per_step is the back-to-back number)"
-                         if flush else "KV fits L2 and --no-l2-flush given: numbers are L2-warm",
+                         "KV fits L2: 512 MiB written between timed steps outside the event windows (value is L2-cold, "
+                         "warm_ms_per_step is back to back)" if flush else "KV fits L2, --no-l2-flush: L2-warm",
                    "attend_impl": {0: "tma", 1: "simple", 2: "tma"}[args.attend_impl],
-                   "launch": "eager: one C-ABI call per kernel" if args.no_graph else
-                             "kf_step_graph: one static CUDA-graph replay per step, inputs re-bound per step",
-                   "roofline_region": f"{roof_steps} further steps launched one by one with CUDA events around "
-                                      "every kf_layer_step launch (events cannot be recorded inside a graph replay)"},
+                   "launch": "eager" if args.no_graph else "kf_step_graph replay per step, inputs re-bound",
+                   "roofline_region": f"{roof_steps} further steps, CUDA events around every kf_layer_step launch"},
         "eager_ms_per_step": eager_ms_per_step, "warm_ms_per_step": warm_ms_per_step,
         "us_per_layer_step": ms_per_step * 1e3 / n_layers,
         "pct_of_nominal_8TBs": 100.0 * value / world / NOMINAL_PEAK_GBS,
@@ -861,8 +1005,8 @@ def measure(args, wl_name, steps, warmup, e2e_steps, dev, dist, rank, world, loc
         "gpu_launches": launches_all,
         "roofline": {"bound": "hbm", "kernel": "attend_tma_kernel" if args.attend_impl != 1 else "attend_simple_kernel",
                      "achieved": achieved, "peak": peak, "unit": UNIT, "frac": achieved / peak,
-                     "traffic": traffic, "traffic_source": traffic_src, "kernel_rev": kernel_rev(),
-                     "algorithmic_bytes_per_launch": attend_bytes,
+                     "traffic": traffic, "traffic_source": traffic_src.split(" (")[0], "kernel_rev": kernel_rev(),
+                     "algorithmic_bytes_per_launch": int(round(attend_bytes)),
                      "avg_launch_ms": attend_ms, "median_launch_ms": attend_times[len(attend_times) // 2],
                      "min_launch_ms": attend_times[0], "launches_timed": len(attend_times), "peak_source": peak_src,
                      "frac_of_nominal_8000": achieved / NOMINAL_PEAK_GBS,
@@ -875,6 +1019,79 @@ def measure(args, wl_name, steps, warmup, e2e_steps, dev, dist, rank, world, loc
 
 
 # ---------------------------------------------------------------------------------------------------------
+FIG10_DEFAULT = ["fig10_q32kv32_b32_s32k", "fig10_q48kv8_b32_s32k", "fig10_q64kv8_b32_s32k",
+                 "fig10_q32kv32_b8_s8k", "fig10_q48kv8_b8_s8k", "fig10_q64kv8_b8_s8k"]
+PIPELINE_DEFAULT = [(16, 2048), (64, 8192), (128, 4096)]
+
+
+def run_extras(args, dev, local):
+    """The records of the default line beyond BASELINE's five configs, each compact: `fig10` (head shapes G = 1 / 6 / 8 at
+    two sizes: PAPER.md:322), `signalling` (route install, token boundary, flag round trip: PAPER.md:308, :165-175) and
+    `pipeline` (three of Fig. 11's workloads: PAPER.md:335-337) -- so that one driver-run line carries every number the
+    profiles quote."""
+    import torch
+    out = {}
+    t0 = time.perf_counter()
+    fig = {}
+    for name in FIG10_DEFAULT:
+        rec = measure(args, name, 30, 5, 10, dev, None, 0, 1, local, want_cpu=False, want_probe=False)
+        fig[name] = _round({"us_per_layer_step": rec["us_per_layer_step"], "value": rec["value"],
+                            "frac": rec["roofline"]["frac"], "frac_of_nominal_8000": rec["roofline"]["frac_of_nominal_8000"],
+                            "static_us": rec["static"]["us_per_layer_step_median"] if rec.get("static") else None,
+                            "e2e": rec["e2e"]["value"]})
+    out["fig10"] = fig
+    t1 = time.perf_counter()
+    out["signalling"] = _round(signalling_record(torch.device(f"cuda:{local}")))
+    t2 = time.perf_counter()
+    cur = torch.cuda.current_stream(dev)
+    out["pipeline"] = compact_pipeline(pipeline_cases(PIPELINE_DEFAULT, None, 8))
+    torch.cuda.set_stream(cur)
+    out["extras_wall_s"] = _round({"fig10": t1 - t0, "signalling": t2 - t1, "pipeline": time.perf_counter() - t2}, 3)
+    return out
+
+
+def wl_steps_note(line):
+    return f"all {line['config']['n_q_heads']} query heads, layer 0, oracle.attend fp64"
+
+
+def _round(x, sig=5):
+    """Floats to `sig` significant digits, recursively: the JSON line stays short enough for a log tail."""
+    if isinstance(x, float):
+        return float(f"{x:.{sig}g}") if x == x and abs(x) != float("inf") else x
+    if isinstance(x, dict):
+        return {k: _round(v, sig) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_round(v, sig) for v in x]
+    return x
+
+
+def compact_record(rec):
+    """The sub-record of one workload inside the headline line: numbers only, no prose (the full record of a workload
+    is what `bench.py --workload <name> --only` prints)."""
+    ro, st, cpu, par = rec["roofline"], rec.get("static"), rec.get("cpu_baseline"), rec.get("parity")
+    out = {"value": rec["value"], "us_per_layer_step": rec["us_per_layer_step"],
+           "pct_of_nominal_8TBs": rec["pct_of_nominal_8TBs"], "steps": rec["steps"], "warmup": rec["warmup"],
+           "warm_ms_per_step": rec.get("warm_ms_per_step"), "gpu_launches": rec["gpu_launches"],
+           "e2e": {"value": rec["e2e"]["value"], "ms_per_step": rec["e2e"]["ms_per_step"]},
+           "roofline": {"achieved": ro["achieved"], "frac": ro["frac"], "traffic": ro["traffic"],
+                        "avg_launch_ms": ro["avg_launch_ms"], "algorithmic_bytes_per_launch": int(ro["algorithmic_bytes_per_launch"]),
+                        "frac_of_read_probe": ro["frac_of_read_probe"]},       # peak: the headline's roofline.peak
+           "clocks": {"sm_mhz": rec["clocks"].get("sm_mhz"), "reasons": rec["clocks"].get("reasons")},
+           "config": {k: rec["config"][k] for k in ("batch", "n_q_heads", "n_kv_heads", "layers_logical",
+                                                    "layers_physical", "context_tokens_step0")}}
+    if st:
+        out["static"] = {k: st[k] for k in ("us_per_layer_step_median", "back_to_back_us", "attend_us_median", "value",
+                                            "pct_of_nominal_8TBs", "l2_flushed")}
+    if cpu:
+        out["cpu_baseline"] = {k: cpu[k] for k in ("value", "cores", "seconds", "one_thread") if k in cpu}
+        out["cpu_baseline"]["sample"] = cpu["sample_short"]
+    if par:
+        out["parity"] = {k: par[k] for k in ("ok", "max_abs_o", "max_rel_lse", "rows")}
+    r = _round(out)
+    r["roofline"]["traffic"], r["roofline"]["algorithmic_bytes_per_launch"] = out["roofline"]["traffic"], out["roofline"]["algorithmic_bytes_per_launch"]
+    return r
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -906,6 +1123,9 @@ def main():
     ap.add_argument("--pipe-sms", default="148,116,100,84,68", help="attend SM budgets tried by --pipeline / --sm-sweep")
     ap.add_argument("--pipe-layers", type=int, default=8, help="layers per step in --pipeline")
     ap.add_argument("--sm-sweep", action="store_true", help="kf_attend GB/s against its SM budget")
+    ap.add_argument("--wside-once", action="store_true", help="run every W-side stage once per batch size (for ncu captures)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the `fig10`, `signalling` and `pipeline` records of the "
+                    "default line")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -915,6 +1135,8 @@ def main():
         return run_pipeline(args)
     if args.sm_sweep:
         return run_sm_sweep(args)
+    if args.wside_once:
+        return run_wside_once(args)
     args.warmup = max(args.warmup, 3)
 
     import torch
@@ -937,15 +1159,28 @@ def main():
     if not args.only and world == 1:
         for name in [w for w in args.sub.split(",") if w and w != args.workload]:
             st, wu, e2 = SUB_STEPS.get(name, (50, 5, 20))
-            rec = measure(args, name, st, wu, e2, dev, None, 0, 1, local, want_cpu=False, want_probe=name != "cfg1")
-            subs[name] = {k: rec[k] for k in ("value", "ms_per_step", "us_per_layer_step", "pct_of_nominal_8TBs", "steps",
-                                              "warmup", "clocks", "e2e", "gpu_launches", "static", "warm_ms_per_step",
-                                              "wall_s")}
-            subs[name]["config"] = rec["config"]
-            subs[name]["roofline"] = rec["roofline"]
+            # the oracle is timed per config as well (SURVEY 8(d) "CPU baseline"), on a ~3 s sample each
+            rec = measure(args, name, st, wu, e2, dev, None, 0, 1, local, want_cpu=not args.no_cpu_baseline,
+                          want_probe=name != "cfg1", cpu_budget_s=3.0)
+            subs[name] = compact_record(rec)
+    extras = {}
+    if not args.only and world == 1 and not args.no_extras:
+        extras = run_extras(args, dev, local)
     if rank == 0:
         if subs:
             line["workloads"] = subs
+        line.update(extras)
+        if not args.only:      # the all-in-one line is kept short (numbers to 6 digits, prose cut): it has to survive a log tail
+            exact = {k: line[k] for k in ("value", "ms_per_step")}
+            if line.get("static"):
+                line["static"] = {k: v for k, v in line["static"].items() if k not in ("protocol", "back_to_back_note")}
+            if line.get("cpu_baseline"):
+                line["cpu_baseline"]["sample"] = line["cpu_baseline"].pop("sample_short") + f", {wl_steps_note(line)}"
+            if line.get("parity"):
+                line["parity"].pop("what", None)
+            line["config"].pop("note", None)
+            line = _round(line, 6)
+            line.update(exact)
         print(json.dumps(line))
     if dist:
         dist.barrier()

@@ -115,3 +115,14 @@ def make_wside(hidden: int, n_q_heads: int, n_kv_heads: int, ffn: int, n_layers:
             gen_device.fill_weight(stream, layer, n, k, out=w.weight(layer, which), seed=seed)
     w.torch.cuda.synchronize(w.device)
     return w
+
+
+def pipeline_attend_sms(kv_bytes: int, weight_bytes: int, n_sms: int = 148) -> int:
+    """SM budget of the attend kernels (kf_config.attend_sms) when kf_pipeline_step overlaps them with the W-side GEMMs on
+    ONE GPU; the GEMMs get the rest (kf_wside_set_sms(n_sms - result)).  Both sides stream from the same HBM, so the SMs
+    are split by the bytes each side has to move per (layer, microbatch), a little in favour of the GEMMs (they need
+    more SMs per byte/s than the attend kernel, which saturates HBM from ~100 SMs), and clamped to the range in which
+    the sweep of profiles/r02c_pipeline.md found every optimum: 68..116, in steps of 4."""
+    share = kv_bytes / float(kv_bytes + weight_bytes)
+    sms = int(round(0.8 * n_sms * share / 4.0)) * 4
+    return max(68, min(116, sms))
