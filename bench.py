@@ -299,6 +299,8 @@ def signalling_record(dev, workload="cfg3"):
             kf.set_active_partitions([1] * P)
             out["set_active_event_us"] = statistics.median(ev)
             out["set_active_host_enqueue_us"] = statistics.median(host)
+            # the same install issued from C inside the library (no ctypes, no torch stream look-up in the way)
+            out["route_install_c_enqueue_us"], out["route_install_c_complete_us"] = kf.route_install_latency(2000)
         ev = []
         for _ in range(60):
             ev.append(event_us(kf.token_boundary)[0])

@@ -49,7 +49,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 210 /* 0.2.1: + kf_attend_static (0.2.0: kf_layer_step, kf_redirect_tails, graph flags, W-node stages) */
+#define KF_VERSION 220 /* 0.2.2: + kf_route_install_latency (0.2.1: kf_attend_static; 0.2.0: kf_layer_step, redirects, graph flags, W-node stages) */
 
 #define KF_OK 0
 #define KF_EINVAL (-1) /* bad argument / shape / alignment / null pointer */
@@ -442,7 +442,14 @@ int kf_pipeline_step(kf_wside *w, kf_ctx *const *ctxs, int32_t n_micro, int32_t 
  * kf_signal_roundtrip: latency of the signalling path above, `iters` times: a two-node graph [wait gate >= seq] ->
  *   [write seq to a pinned host word] is launched on exec_stream, the host releases the gate on signal_stream and
  *   spins on the host word.  *median_us / *min_us [host] = host enqueue + GPU reaction + write visible to the host: an
- *   upper bound on "GPU store -> host sees it".  Synchronises both streams. */
+ *   upper bound on "GPU store -> host sees it".  Synchronises both streams.
+ * kf_route_install_latency: what a route install costs when issued from C (the paper's CPU routing loop installs a route
+ *   in 7.2 us): `iters` times the active set is replaced by a neighbouring one with the kernel
+ *   kf_set_active_partitions launches.  *enqueue_us_median [host] = host time of the launch call alone;
+ *   *complete_us_median [host] = launch + stream synchronise (the set is in device memory, every later kernel sees it).
+ *   The active set found at entry is re-published before the call returns.  Synchronises `stream`. */
+int kf_route_install_latency(kf_ctx *ctx, int32_t iters, kf_stream stream, double *enqueue_us_median,
+                             double *complete_us_median);
 int kf_plan_info(kf_ctx *ctx, int32_t *out, kf_stream stream);
 int kf_signal_roundtrip(kf_ctx *ctx, int32_t iters, kf_stream exec_stream, kf_stream signal_stream, double *median_us,
                         double *min_us);

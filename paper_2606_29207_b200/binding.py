@@ -19,7 +19,7 @@ EXPORTS = [
     "kf_kv_append", "kf_partial_attend", "kf_merge_partials", "kf_attend", "kf_attend_static", "kf_step_commit", "kf_layer_step", "kf_layer_step_host",
     "kf_route_snapshot", "kf_status", "kf_plan_info", "kf_launch_count", "kf_worker_times",
     "kf_step_graph_create", "kf_step_graph_launch", "kf_step_graph_destroy", "kf_probe_read",
-    "kf_step_graph_flags", "kf_step_graph_seq", "kf_step_graph_release", "kf_signal_roundtrip",
+    "kf_step_graph_flags", "kf_step_graph_seq", "kf_step_graph_release", "kf_signal_roundtrip", "kf_route_install_latency",
     "kf_set_active_partitions", "kf_redirect_tails", "kf_route_begins", "kf_partition_state", "kf_set_active_requests",
     "kf_policy_bytes_per_token", "kf_policy_threshold", "kf_policy_initial_nodes", "kf_policy_step",
     "kf_wside_weight_bytes", "kf_wside_weight_offset", "kf_wside_workspace_bytes", "kf_wside_create", "kf_wside_destroy",
@@ -110,6 +110,7 @@ def load_library():
     L.kf_step_graph_seq.argtypes, L.kf_step_graph_seq.restype = [vp, i32], ctypes.c_uint32
     L.kf_step_graph_release.argtypes = [vp, i32, ctypes.c_uint32, vp]
     L.kf_signal_roundtrip.argtypes = [vp, i32, vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+    L.kf_route_install_latency.argtypes = [vp, i32, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     L.kf_set_active_partitions.argtypes = [vp, ctypes.POINTER(ctypes.c_uint8), vp]
     L.kf_redirect_tails.argtypes = [vp, ctypes.POINTER(ctypes.c_uint8), vp]
     L.kf_route_begins.argtypes = [vp, ctypes.POINTER(ctypes.c_int32), vp]
@@ -323,6 +324,13 @@ class KFlume:
         n = ctypes.c_size_t(0)
         self._check(self.lib.kf_probe_read(self.h, _ptr(sink), ctypes.byref(n), self._stream(stream)), "kf_probe_read")
         return int(n.value)
+
+    def route_install_latency(self, iters: int, stream=None):
+        """kf_route_install_latency: (enqueue_us, complete_us) medians of a route install issued from C."""
+        q, c = ctypes.c_double(), ctypes.c_double()
+        self._check(self.lib.kf_route_install_latency(self.h, iters, self._stream(stream), ctypes.byref(q),
+                                                      ctypes.byref(c)), "kf_route_install_latency")
+        return q.value, c.value
 
     def signal_roundtrip(self, iters: int, exec_stream, signal_stream):
         """kf_signal_roundtrip: (median_us, min_us) of gate release -> readiness flag seen by the host."""

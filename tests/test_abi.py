@@ -29,7 +29,7 @@ def test_every_declared_symbol_is_exported():
 
 def test_version_and_strerror():
     lib = load_library()
-    assert lib.kf_version() == 210
+    assert lib.kf_version() == 220
     assert lib.kf_strerror(0) == b"ok"
     for code in (-1, -2, -3, -4):
         assert lib.kf_strerror(code) not in (b"ok", b"unknown error")
@@ -85,6 +85,7 @@ def test_null_ctx_calls_return_einval():
     assert lib.kf_step_graph_seq(None, 0) == 0
     assert lib.kf_w_project_q(None, 0, None, 1, None, None) == -1
     assert lib.kf_attend_static(None, 0, None, None, None, None) == -1
+    assert lib.kf_route_install_latency(None, 1, None, None, None) == -1
     assert lib.kf_wside_launch_count(None) == 0
 
 

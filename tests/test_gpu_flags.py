@@ -228,3 +228,32 @@ def test_release_right_after_flags_survives_while_the_capture_stream_is_busy():
             check_close(o[r], lse[r], o_ref, lse_ref, f"early release r{r}")
         g.destroy()
     ses.close()
+
+
+def test_route_install_latency_probe_restores_the_active_set():
+    # kf_route_install_latency toggles the active set `iters` times from C and must leave the one it found
+    wl = Workload("install_probe", 32, 8, 64, 5, [100, 17, 64])
+    ses = Session(wl, steps=2)
+    ses.prepare()
+    kf = ses.kf
+    kf.set_active_partitions([1, 0, 1, 1, 0])
+    before = kf.partition_state()
+    n0 = kf.launch_count()
+    enq, done = kf.route_install_latency(300)
+    assert 0.0 < enq <= done < 5000.0, (enq, done)
+    assert kf.launch_count() - n0 >= 311
+    after = kf.partition_state()
+    assert after["active"] == before["active"] == [1, 0, 1, 1, 0]
+    assert kf.status() == KF_OK
+    # and decoding goes on as if nothing had happened
+    kf.token_boundary()
+    q = ses.q_for(0, 0)
+    k_new, v_new = ses.kv_new_for(0, 0)
+    ses.layer_step(0, q, k_new, v_new)
+    kf.step_commit()
+    assert kf.status() == KF_OK
+    o, lse = ses.o.cpu().numpy(), ses.lse.cpu().numpy()
+    for r, S0 in enumerate(wl.contexts):
+        o_ref, lse_ref = oracle_request(wl, 0, r, 0, S0)
+        check_close(o[r], lse[r], o_ref, lse_ref, f"after the probe r{r}")
+    ses.close()
